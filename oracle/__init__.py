@@ -1,0 +1,165 @@
+"""TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes front end of the f64 single-threaded CPU oracle in ``vjp_oracle.c`` (see that file's
+header for what it computes and which passage of arxiv/paper_2310_03568 each function
+follows).  Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package; it imports nothing from the CUDA package
+``paper_2310_03568_b200`` and the product never imports it.
+
+All inputs are converted to float64 / int64 numpy arrays (f32 -> f64 is exact, so comparisons,
+zero tests, argmins and sort order are the same in both precisions); all outputs are float64 /
+int64 numpy arrays.  Scan arrays are ``[n]`` or ``[n, d]`` (row-major, a q-by-q matrix element
+is stored row-major).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "vjp_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+ADD, MIN, MAX, MUL, LINREC, MATMUL, SATADD = range(7)
+OPS = {"add": ADD, "min": MIN, "max": MAX, "mul": MUL, "linrec": LINREC,
+       "matmul": MATMUL, "satadd": SATADD}
+
+
+def build(force: bool = False) -> str:
+    """Compile vjp_oracle.c with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _i64(a):
+    return np.ascontiguousarray(np.asarray(a), dtype=np.int64)
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError("oracle %s failed with status %d" % (what, rc))
+
+
+def _opcode(op):
+    return OPS[op] if isinstance(op, str) else int(op)
+
+
+def _scan_shape(op, q, xs):
+    d = _load().orc_scan_arity(op, q)
+    if d < 0:
+        raise ValueError("not a scan operator")
+    n = xs.size // d
+    if xs.size != n * d:
+        raise ValueError("xs size is not a multiple of the operator arity %d" % d)
+    return n, d
+
+
+def scan_forward(op, xs, q: int = 0):
+    """Inclusive scan."""
+    op = _opcode(op)
+    xs = _f64(xs)
+    n, _ = _scan_shape(op, q, xs)
+    ys = np.empty_like(xs)
+    _check(_load().orc_scan_forward(op, q, ctypes.c_int64(n), _p(xs), _p(ys)), "scan_forward")
+    return ys
+
+
+def vjp_scan(op, xs, ys_bar, q: int = 0):
+    """Input adjoints of the inclusive scan (return sweep P:L553-558)."""
+    op = _opcode(op)
+    xs, ys_bar = _f64(xs), _f64(ys_bar)
+    if xs.shape != ys_bar.shape:
+        raise ValueError("xs and ys_bar differ in shape")
+    n, _ = _scan_shape(op, q, xs)
+    xs_bar = np.zeros_like(xs)
+    _check(_load().orc_scan_vjp(op, q, ctypes.c_int64(n), _p(xs), _p(ys_bar), _p(xs_bar)), "scan_vjp")
+    return xs_bar
+
+
+def reduce_by_index_forward(op, num_bins, is_, vs, S: float = 0.0):
+    """reduce_by_index over a neutral-initialised histogram."""
+    op = _opcode(op)
+    is_, vs = _i64(is_), _f64(vs)
+    hist = np.empty(num_bins, dtype=np.float64)
+    _check(_load().orc_rbi_forward(op, ctypes.c_double(S), ctypes.c_int64(is_.size),
+                                   ctypes.c_int64(num_bins), _p(is_), _p(vs), _p(hist)), "rbi_forward")
+    return hist
+
+
+def vjp_rbi_add(num_bins, is_, hist_bar):
+    is_, hist_bar = _i64(is_), _f64(hist_bar)
+    vs_bar = np.empty(is_.size, dtype=np.float64)
+    _check(_load().orc_rbi_vjp_add(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_),
+                                   _p(hist_bar), _p(vs_bar)), "rbi_vjp_add")
+    return vs_bar
+
+
+def vjp_rbi_minmax(op, num_bins, is_, vs, hist_bar):
+    """Returns (vs_bar, arg[w] int64 with n for an empty bin, ext[w])."""
+    op = _opcode(op)
+    is_, vs, hist_bar = _i64(is_), _f64(vs), _f64(hist_bar)
+    vs_bar = np.empty(is_.size, dtype=np.float64)
+    arg = np.empty(num_bins, dtype=np.int64)
+    ext = np.empty(num_bins, dtype=np.float64)
+    _check(_load().orc_rbi_vjp_minmax(op, ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_),
+                                      _p(vs), _p(hist_bar), _p(arg), _p(ext), _p(vs_bar)), "rbi_vjp_minmax")
+    return vs_bar, arg, ext
+
+
+def vjp_rbi_mul(num_bins, is_, vs, hist_bar):
+    """Returns (vs_bar, zeros[w] int64, prod_nz[w])."""
+    is_, vs, hist_bar = _i64(is_), _f64(vs), _f64(hist_bar)
+    vs_bar = np.empty(is_.size, dtype=np.float64)
+    zeros = np.empty(num_bins, dtype=np.int64)
+    prod = np.empty(num_bins, dtype=np.float64)
+    _check(_load().orc_rbi_vjp_mul(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(vs),
+                                   _p(hist_bar), _p(zeros), _p(prod), _p(vs_bar)), "rbi_vjp_mul")
+    return vs_bar, zeros, prod
+
+
+def vjp_rbi_general(op, num_bins, is_, vs, hist_bar, S: float = 0.0, with_lr: bool = False):
+    """General-case rule, eq. 5.  Returns vs_bar, or (vs_bar, ls, rs)."""
+    op = _opcode(op)
+    is_, vs, hist_bar = _i64(is_), _f64(vs), _f64(hist_bar)
+    n = is_.size
+    vs_bar = np.empty(n, dtype=np.float64)
+    ls = np.empty(n, dtype=np.float64) if with_lr else None
+    rs = np.empty(n, dtype=np.float64) if with_lr else None
+    _check(_load().orc_rbi_vjp_general(op, ctypes.c_double(S), ctypes.c_int64(n), ctypes.c_int64(num_bins),
+                                       _p(is_), _p(vs), _p(hist_bar), _p(vs_bar), _p(ls), _p(rs)),
+           "rbi_vjp_general")
+    return (vs_bar, ls, rs) if with_lr else vs_bar
+
+
+def rbi_sort_perm(num_bins, is_):
+    """Stable sort by clamped key (Fig. 4).  Returns (sorted_keys, perm)."""
+    is_ = _i64(is_)
+    sk = np.empty(is_.size, dtype=np.int64)
+    perm = np.empty(is_.size, dtype=np.int64)
+    _check(_load().orc_rbi_sort_perm(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(sk),
+                                     _p(perm)), "rbi_sort_perm")
+    return sk, perm
