@@ -1,0 +1,162 @@
+/*
+ * vjp_b200.h -- C ABI of the B200-native library for the reverse-mode vector-Jacobian
+ * products (VJPs) of inclusive scan and reduce-by-index (generalised histogram).
+ *
+ * Method: arxiv/paper_2310_03568, "Reverse-Mode AD of Reduce-by-Index and Scan in Futhark".
+ * "P:Lnnn" below is a line of the paper text; Qn is a reading listed in DESIGN.md.
+ *
+ * Conventions common to every entry point
+ *   - Pointers named xs, ys, ys_bar, xs_bar, is, vs, hist, hist_bar, vs_bar, arg, ext, zeros,
+ *     prod_nz, sorted_keys, perm and ws are DEVICE pointers owned by the caller, 16-byte
+ *     aligned (a torch allocation is).  The library never allocates, frees or synchronises:
+ *     a call validates its arguments on the host, enqueues kernels / memsets on `stream`
+ *     (a cudaStream_t passed as void*; NULL = the legacy default stream) and returns.
+ *     The *_host entry points are the exception: their data pointers are HOST pointers, they
+ *     copy host->device, run the same kernels, copy the result back and synchronise `stream`.
+ *   - Scan elements are [n][d] contiguous row-major, d = vjp_scan_arity(op): 1 ('+', '*'),
+ *     2 (linear recurrence (a,b)), 4 (2x2 row-major matrix), 25 (5x5 row-major matrix).
+ *   - Bin indices `is` are int64.  An index outside [0, num_bins) -- negative
+ *     included -- is ignored by the primal and receives adjoint exactly 0 (P:L335-336,
+ *     P:L361-362; Q3).
+ *   - Outputs are overwritten with the adjoint CONTRIBUTION (the paper's "+=" target taken
+ *     as zero, Q1).  Outputs must not alias inputs.
+ *   - `ws` is scratch of at least *_workspace_bytes(...) bytes; its contents need not be
+ *     initialised and are garbage afterwards.  Two calls that may overlap in time need two
+ *     workspaces.
+ *   - Return value: VJP_OK (0) or a negative vjp_status_t; on error nothing was enqueued
+ *     (VJP_ERR_CUDA excepted: a launch failed part-way).  n == 0 is VJP_OK and a no-op
+ *     (reduce_by_index_forward still neutral-initialises hist).  NaN inputs are unsupported.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with
+ *     VJP_ERR_CUDA.
+ */
+#ifndef VJP_B200_H
+#define VJP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    VJP_OK = 0,
+    VJP_ERR_INVALID_ARG = -1, /* NULL pointer, negative size, unknown op / dtype            */
+    VJP_ERR_UNSUPPORTED = -2, /* op not defined for this combinator / dtype, n too large     */
+    VJP_ERR_WORKSPACE = -3,   /* ws_bytes smaller than the *_workspace_bytes query          */
+    VJP_ERR_CUDA = -4         /* a CUDA runtime call or launch failed                        */
+} vjp_status_t;
+
+typedef enum {
+    VJP_OP_ADD = 0,     /* a + b, neutral 0.                       scan + reduce-by-index   */
+    VJP_OP_MIN = 1,     /* min, neutral +inf, lowest index on ties. rbi only       */
+    VJP_OP_MAX = 2,     /* max, neutral -inf, lowest index on ties (Q4).     rbi only       */
+    VJP_OP_MUL = 3,     /* a * b, neutral 1, exact with zeros.     scan + reduce-by-index   */
+    VJP_OP_LINREC = 4,  /* (A,B)(+)(a,b) = (a*A, a*B+b), neutral (1,0) (BASELINE
+                           config 3).  scan only (not commutative)                   */
+    VJP_OP_MATMUL2 = 5, /* 2x2 row-major matrix product R x X, neutral I.  scan only */
+    VJP_OP_MATMUL5 = 6, /* 5x5 row-major matrix product.                            scan only */
+    VJP_OP_SATADD = 7   /* min(a+b, S) on non-negative reals, neutral 0 (Q16).
+                           reduce-by-index only; always the general rule (Fig. 4)            */
+} vjp_opcode_t;
+
+typedef enum { VJP_F32 = 0, VJP_F64 = 1 } vjp_dtype_t;
+
+/* Operator descriptor. */
+typedef struct {
+    int32_t code;          /* vjp_opcode_t                                                    */
+    int32_t dtype;         /* vjp_dtype_t of xs / vs and of every real-valued output          */
+    double param;          /* S for VJP_OP_SATADD, ignored otherwise                          */
+    int32_t force_general; /* reduce-by-index only: != 0 routes '+', '*', min, max through the
+                              general rule (sort + segmented scans, Fig. 4) instead
+                              of their specialisation                            */
+    int32_t reserved;      /* must be 0                                                       */
+} vjp_op_t;
+
+/* Scalars per scan element for op, or -1 if op is not a scan operator. */
+int vjp_scan_arity(const vjp_op_t *op);
+
+/* Library build information ("sm_100a ..." string, static storage). */
+const char *vjp_version(void);
+
+/* ------------------------------------------------------------------------------ scan ----- */
+
+size_t vjp_scan_workspace_bytes(const vjp_op_t *op, int64_t n);
+
+/* Primal inclusive scan ys[i] = xs[0] (.) ... (.) xs[i].  Single-pass
+ * decoupled-look-back kernel.  Exists for the AD-overhead denominator.
+ * Supported: ADD (f32, f64), MUL (f32, f64), LINREC (f32), MATMUL2 (f32), MATMUL5 (f32). */
+int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
+                 void *ws, size_t ws_bytes, void *stream);
+
+/* Input adjoints of the inclusive scan: xs_bar = J^T ys_bar (Fig. 7; return sweep
+ * P:L553-558).
+ *   ADD:   xs_bar = reverse inclusive sum of ys_bar; xs may be NULL.
+ *   other: forward tile prefixes r_{i-1} are recomputed from xs (no tape), then ONE
+ *          fused reverse kernel forms the Jacobians on the fly (never stored), runs
+ *          the reverse linear-recurrence scan rbar_i = ys_bar_i + J_i^T rbar_{i+1} with lin_o
+ *           in its redundant-block-diagonal form, and applies the
+ *          final map xs_bar_i = (d(r_{i-1} (.) x_i)/d x_i)^T rbar_i. */
+int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar,
+             void *ws, size_t ws_bytes, void *stream);
+
+/* Same, with HOST pointers for xs, ys_bar, xs_bar.  dev_scratch is a DEVICE buffer of at least
+ * vjp_scan_host_scratch_bytes() bytes (holds the three arrays and the workspace). */
+size_t vjp_scan_host_scratch_bytes(const vjp_op_t *op, int64_t n);
+int vjp_scan_host(const vjp_op_t *op, int64_t n, const void *xs_host, const void *ys_bar_host,
+                  void *xs_bar_host, void *dev_scratch, size_t dev_scratch_bytes, void *stream);
+
+/* ------------------------------------------------------------------- reduce-by-index ----- */
+
+size_t vjp_reduce_by_index_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t num_bins);
+
+/* Primal reduce_by_index over a neutral-initialised histogram (P:L332-336 after the rewrite of
+ * there is no hist_0 argument).  hist[num_bins] is fully written.
+ * Supported: ADD (f32, f64), MIN, MAX, MUL, SATADD (f32). */
+int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                            const void *vs, void *hist, void *ws, size_t ws_bytes, void *stream);
+
+/* Input adjoints vs_bar[n] of reduce_by_index w.r.t. vs, given hist_bar[num_bins].
+ *   ADD:      gather vs_bar[i] = hist_bar[is[i]]; vs may be NULL.  Bit-exact copy.
+ *   MIN/MAX:  lifted primal (index, value) per bin, lowest index on ties (Fig. 5),
+ *             then vs_bar = 0 and vs_bar[arg[k]] = hist_bar[k].  Bit-exact copy.
+ *   MUL:      lifted primal (zero count, product of non-zeros) (Fig. 3),
+ *             then the three-way map of P:L208-219 / P:L243-246.
+ *   SATADD or force_general: stable radix sort by clamped bin, forward and reverse segmented
+ *             exclusive scans, per-element derivative of l (.) x (.) r, un-permute
+ *             (Fig. 4, eq. 5).
+ * n must be < 2^32 - 1 (packed 32-bit positions). */
+int vjp_reduce_by_index(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                        const void *vs, const void *hist_bar, void *vs_bar,
+                        void *ws, size_t ws_bytes, void *stream);
+
+/* Same, with HOST pointers for is, vs, hist_bar, vs_bar. */
+size_t vjp_reduce_by_index_host_scratch_bytes(const vjp_op_t *op, int64_t n, int64_t num_bins);
+int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
+                             const int64_t *is_host, const void *vs_host,
+                             const void *hist_bar_host, void *vs_bar_host,
+                             void *dev_scratch, size_t dev_scratch_bytes, void *stream);
+
+/* Inspection entry points: the integer-valued intermediates, for bit-exact comparison. */
+
+/* MIN / MAX lifted primal (Fig. 5): arg[k] = lowest index attaining the extremum of bin k, or n
+ * for an empty bin; ext[k] = the extremum (+-inf for an empty bin), dtype f32. */
+int rbi_argext(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is, const void *vs,
+               int64_t *arg, void *ext, void *ws, size_t ws_bytes, void *stream);
+
+/* MUL lifted primal: zeros[k] = #{i : is[i]=k, vs[i]==0} (IEEE equality, Q7),
+ * prod_nz[k] = product of the non-zero members (1 if none), dtype f32. */
+int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                  const void *vs, int64_t *zeros, void *prod_nz, void *ws, size_t ws_bytes,
+                  void *stream);
+
+/* Stable sort of (key', iota) by key' = is[i] if in range else num_bins (Fig. 4 P:L350-351;
+ * Q18).  sorted_keys[n], perm[n] are int64.  Workspace: that of the general rule
+ * (query with op.code = VJP_OP_SATADD). */
+int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
+                  int64_t *perm, void *ws, size_t ws_bytes, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VJP_B200_H */

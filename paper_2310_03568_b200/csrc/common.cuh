@@ -1,0 +1,312 @@
+// common.cuh -- device-side building blocks shared by every kernel of the library:
+// word-wise warp shuffles of arbitrary POD states, ordered block scans of a monoid,
+// the decoupled look-back protocol, and row-padded shared-memory tile staging with
+// 128-bit global accesses.  sm_100a only.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace vjp {
+
+constexpr unsigned FULL_MASK = 0xffffffffu;
+constexpr int NUM_SMS_B200 = 148;
+
+#define VJP_DEVINL __device__ __forceinline__
+
+// ------------------------------------------------------------------ memory ordering ----
+
+VJP_DEVINL void st_release_s32(int *p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+VJP_DEVINL int ld_acquire_s32(const int *p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+VJP_DEVINL unsigned ld_relaxed_u32(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+VJP_DEVINL void st_relaxed_u32(unsigned *p, unsigned v) {
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// streaming 128-bit accesses (data touched once: do not keep it in L1)
+VJP_DEVINL uint4 ldg_stream(const uint4 *p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p));
+    return r;
+}
+VJP_DEVINL void stg_stream(uint4 *p, const uint4 &v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x),
+                 "r"(v.y), "r"(v.z), "r"(v.w)
+                 : "memory");
+}
+
+// ------------------------------------------------------------------ POD word helpers ---
+
+// Copy a POD state to / from global memory through L2 (look-back payloads: written once by one
+// block, read by others after an acquire on the tile's flag).
+template <class S>
+VJP_DEVINL void store_state_cg(S *dst, const S &s) {
+    static_assert(sizeof(S) % 4 == 0, "state must be a whole number of 32-bit words");
+    constexpr int W = sizeof(S) / 4;
+    const uint32_t *a = reinterpret_cast<const uint32_t *>(&s);
+    uint32_t *d = reinterpret_cast<uint32_t *>(dst);
+#pragma unroll
+    for (int i = 0; i < W; i++) __stcg(d + i, a[i]);
+}
+template <class S>
+VJP_DEVINL S load_state_cg(const S *src) {
+    constexpr int W = sizeof(S) / 4;
+    S r;
+    uint32_t *b = reinterpret_cast<uint32_t *>(&r);
+    const uint32_t *p = reinterpret_cast<const uint32_t *>(src);
+#pragma unroll
+    for (int i = 0; i < W; i++) b[i] = __ldcg(p + i);
+    return r;
+}
+template <class S>
+VJP_DEVINL S shfl_state(const S &s, int src_lane) {
+    constexpr int W = sizeof(S) / 4;
+    S r;
+    const uint32_t *a = reinterpret_cast<const uint32_t *>(&s);
+    uint32_t *b = reinterpret_cast<uint32_t *>(&r);
+#pragma unroll
+    for (int i = 0; i < W; i++) b[i] = __shfl_sync(FULL_MASK, a[i], src_lane);
+    return r;
+}
+template <class S>
+VJP_DEVINL void store_state_smem(uint32_t *dst, const S &s) {
+    constexpr int W = sizeof(S) / 4;
+    const uint32_t *a = reinterpret_cast<const uint32_t *>(&s);
+#pragma unroll
+    for (int i = 0; i < W; i++) dst[i] = a[i];
+}
+template <class S>
+VJP_DEVINL S load_state_smem(const uint32_t *src) {
+    constexpr int W = sizeof(S) / 4;
+    S r;
+    uint32_t *b = reinterpret_cast<uint32_t *>(&r);
+#pragma unroll
+    for (int i = 0; i < W; i++) b[i] = src[i];
+    return r;
+}
+
+// ------------------------------------------------------------------ ordered block scan -
+//
+// A monoid M provides   typename M::State (POD, whole words),
+//                       static State identity(),
+//                       static State combine(const State& earlier, const State& later).
+// "earlier / later" refer to PROCESSING order.  With REVT = false thread t has processing rank
+// t; with REVT = true thread t has rank NT-1-t (a scan that runs from the end of the tile).
+
+template <class M, int NT>
+struct BlockScan {
+    using S = typename M::State;
+    static constexpr int NW = NT / 32;
+    static constexpr int SW = sizeof(S) / 4;
+    // shared scratch: NW warp totals + 1 block total, as words
+    static constexpr int SMEM_WORDS = (NW + 1) * SW;
+
+    // Exclusive scan of one state per thread.  Returns the exclusive prefix of this thread
+    // (within the block) and the block total in `total` (valid in every thread).
+    template <bool REVT>
+    static VJP_DEVINL S exclusive(const S &local, S &total, uint32_t *scratch) {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const int plane = REVT ? 31 - lane : lane;
+        const int pwarp = REVT ? NW - 1 - warp : warp;
+        __syncthreads();  // scratch may still be read by a previous call
+        S incl = local;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            S o = shfl_state(incl, REVT ? lane + off : lane - off);
+            if (plane >= off) incl = M::combine(o, incl);
+        }
+        // exclusive within the warp
+        S ex = shfl_state(incl, REVT ? lane + 1 : lane - 1);
+        if (plane == 0) ex = M::identity();
+        if (plane == 31) store_state_smem(scratch + pwarp * SW, incl);
+        __syncthreads();
+        if (warp == 0) {
+            // lane l holds the total of processing-warp l; Kogge-Stone over NW lanes
+            S wt = (lane < NW) ? load_state_smem<S>(scratch + lane * SW) : M::identity();
+            S wi = wt;
+#pragma unroll
+            for (int off = 1; off < NW; off <<= 1) {
+                S o = shfl_state(wi, lane - off);
+                if (lane >= off) wi = M::combine(o, wi);
+            }
+            S wex = shfl_state(wi, lane - 1);
+            if (lane == 0) wex = M::identity();
+            __syncwarp();
+            if (lane < NW) store_state_smem(scratch + lane * SW, wex);
+            if (lane == NW - 1) store_state_smem(scratch + NW * SW, wi);
+        }
+        __syncthreads();
+        total = load_state_smem<S>(scratch + NW * SW);
+        if (pwarp > 0) {
+            S wp = load_state_smem<S>(scratch + pwarp * SW);
+            ex = M::combine(wp, ex);
+        }
+        return ex;
+    }
+};
+
+// ------------------------------------------------------------------ decoupled look-back -
+//
+// Tile status of processing-order tile p: flags[p] in {EMPTY, AGG, PREFIX}; agg[p] / incl[p]
+// hold the tile aggregate / the inclusive prefix through tile p.  Writers publish the payload
+// with L2 stores, then release-store the flag; readers acquire-load the flag, then read the
+// payload with L2 loads.  Tiles take their processing index from an atomic ticket, so every
+// predecessor of a running tile is itself running or finished (forward progress).
+
+enum : int { TILE_EMPTY = 0, TILE_AGG = 1, TILE_PREFIX = 2 };
+
+template <class S>
+struct TileStatus {
+    int *flags;  // [num_tiles], zeroed before the launch
+    S *agg;      // [num_tiles]
+    S *incl;     // [num_tiles]
+};
+
+template <class S>
+VJP_DEVINL void publish_tile(const TileStatus<S> &st, int p, const S &value, bool is_prefix) {
+    store_state_cg((is_prefix ? st.incl : st.agg) + p, value);
+    __threadfence();
+    st_release_s32(st.flags + p, is_prefix ? TILE_PREFIX : TILE_AGG);
+}
+
+// Called by ALL 32 lanes of one warp.  Returns (in every lane) the fold of tiles 0..p-1 in
+// processing order.  `LoadAgg(q)` / `LoadIncl(q)` fetch the payloads of tile q.
+template <class M, class LoadAgg, class LoadIncl>
+VJP_DEVINL typename M::State lookback_warp(const int *flags, int p, LoadAgg load_agg,
+                                           LoadIncl load_incl) {
+    using S = typename M::State;
+    const int lane = threadIdx.x & 31;
+    S acc = M::identity();
+    int base = p - 1;
+    while (true) {
+        const int q = base - lane;
+        int f = TILE_PREFIX;  // tiles before the first one: an identity prefix
+        if (q >= 0) {
+            f = ld_acquire_s32(flags + q);
+        }
+        while (__any_sync(FULL_MASK, f == TILE_EMPTY)) {
+            if (f == TILE_EMPTY) {
+                __nanosleep(32);
+                f = ld_acquire_s32(flags + q);
+            }
+        }
+        const unsigned pm = __ballot_sync(FULL_MASK, f == TILE_PREFIX);
+        const int first = __ffs(pm) - 1;  // nearest tile with a full prefix; -1 if none
+        S s = M::identity();
+        if (first < 0 || lane <= first) {
+            if (q >= 0) s = (f == TILE_PREFIX) ? load_incl(q) : load_agg(q);
+        }
+        // ordered fold over the window: higher lanes are earlier tiles
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            S o = shfl_state(s, lane + off);
+            if (lane + off < 32) s = M::combine(o, s);
+        }
+        s = shfl_state(s, 0);
+        acc = M::combine(s, acc);
+        if (pm != 0) break;
+        base -= 32;
+    }
+    return acc;
+}
+
+// ------------------------------------------------------------------ tile staging -------
+//
+// A tile is NT rows (one per thread) of RW 32-bit words; in shared memory a row has a pitch
+// of RW + PAD words, PAD in {0, 4} chosen so that the number of 16-byte chunks per row is odd:
+// then a warp's LDS.128 / STS.128 of "chunk c of my row" is bank-conflict-free.  Global <->
+// shared copies move whole 16-byte chunks, consecutive lanes on consecutive chunks (coalesced).
+
+template <int NT, int RW>
+struct TileStage {
+    static_assert(RW % 4 == 0, "row must be a whole number of 16-byte chunks");
+    static constexpr int CPR = RW / 4;                       // chunks per row
+    static constexpr int PITCH_C = (CPR % 2 == 0) ? CPR + 1 : CPR;  // pitch in chunks
+    static constexpr int TILE_WORDS = NT * RW;
+    static constexpr int TILE_CHUNKS = NT * CPR;
+    static constexpr int SMEM_BYTES = NT * PITCH_C * 16;
+
+    // global (tile-relative chunk index) -> shared chunk index
+    static VJP_DEVINL int smem_chunk(int c) { return (c / CPR) * PITCH_C + (c % CPR); }
+
+    // Load `valid_words` words (<= TILE_WORDS) starting at `g` (16-byte aligned) into the staged
+    // layout; the rest of the tile is filled with the word pattern fill[w % FW].
+    template <int FW>
+    static VJP_DEVINL void load(uint4 *smem, const uint32_t *__restrict__ g, int valid_words,
+                                const uint32_t (&fill)[FW]) {
+        static_assert(RW % FW == 0, "fill pattern must tile a row");
+        const uint4 *g4 = reinterpret_cast<const uint4 *>(g);
+        if (valid_words == TILE_WORDS) {
+#pragma unroll
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) smem[smem_chunk(c)] = ldg_stream(g4 + c);
+        } else {
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) {
+                uint32_t w[4];
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const int wi = c * 4 + j;
+                    w[j] = (wi < valid_words) ? __ldg(g + wi) : fill[wi % FW];
+                }
+                smem[smem_chunk(c)] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+        }
+    }
+
+    // Store the first `valid_words` words of the staged tile to `g`.
+    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words) {
+        uint4 *g4 = reinterpret_cast<uint4 *>(g);
+        if (valid_words == TILE_WORDS) {
+#pragma unroll
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) stg_stream(g4 + c, smem[smem_chunk(c)]);
+        } else {
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) {
+                const uint4 v = smem[smem_chunk(c)];
+                const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const int wi = c * 4 + j;
+                    if (wi < valid_words) g[wi] = w[j];
+                }
+            }
+        }
+    }
+
+    // Row access for the owning thread: whole row <-> registers.
+    static VJP_DEVINL void read_row(const uint4 *smem, int row, uint32_t (&r)[RW]) {
+#pragma unroll
+        for (int c = 0; c < CPR; c++) {
+            const uint4 v = smem[row * PITCH_C + c];
+            r[4 * c + 0] = v.x; r[4 * c + 1] = v.y; r[4 * c + 2] = v.z; r[4 * c + 3] = v.w;
+        }
+    }
+    static VJP_DEVINL void write_row(uint4 *smem, int row, const uint32_t (&r)[RW]) {
+#pragma unroll
+        for (int c = 0; c < CPR; c++)
+            smem[row * PITCH_C + c] = make_uint4(r[4 * c + 0], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+    }
+};
+
+// words <-> scalars
+VJP_DEVINL float word_to(const uint32_t *w, float *) { return __uint_as_float(w[0]); }
+VJP_DEVINL double word_to(const uint32_t *w, double *) {
+    return __hiloint2double((int)w[1], (int)w[0]);
+}
+VJP_DEVINL void to_word(float v, uint32_t *w) { w[0] = __float_as_uint(v); }
+VJP_DEVINL void to_word(double v, uint32_t *w) {
+    w[0] = (uint32_t)__double2loint(v);
+    w[1] = (uint32_t)__double2hiint(v);
+}
+
+}  // namespace vjp
