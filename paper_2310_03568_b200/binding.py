@@ -1,0 +1,281 @@
+"""Thin Python binding of the C ABI in ``include/vjp_b200.h`` (same entry-point names).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+``libvjp_b200.so``.  PyTorch is used for device memory (``torch.empty``, ``data_ptr``) and for the
+current stream, nothing else.  There is no CPU fallback: if the library is missing and cannot be
+built, or a call returns a negative status, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+from . import build as _build
+
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
+_STATUS = {-1: "VJP_ERR_INVALID_ARG", -2: "VJP_ERR_UNSUPPORTED", -3: "VJP_ERR_WORKSPACE", -4: "VJP_ERR_CUDA"}
+
+OP_ADD, OP_MIN, OP_MAX, OP_MUL, OP_LINREC, OP_MATMUL2, OP_MATMUL5, OP_SATADD = range(8)
+OPCODES = {"add": OP_ADD, "min": OP_MIN, "max": OP_MAX, "mul": OP_MUL, "linrec": OP_LINREC,
+           "matmul2": OP_MATMUL2, "matmul5": OP_MATMUL5, "satadd": OP_SATADD}
+F32, F64 = 0, 1
+
+EXPORTS = [
+    "vjp_scan_arity", "vjp_version", "vjp_scan_workspace_bytes", "scan_forward", "vjp_scan",
+    "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_reduce_by_index_workspace_bytes",
+    "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
+    "vjp_reduce_by_index_host", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
+]
+
+
+class VjpError(RuntimeError):
+    pass
+
+
+class _OpStruct(ctypes.Structure):
+    _fields_ = [("code", ctypes.c_int32), ("dtype", ctypes.c_int32), ("param", ctypes.c_double),
+                ("force_general", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+@dataclass(frozen=True)
+class Op:
+    """Operator descriptor (vjp_op_t)."""
+    code: int
+    dtype: int = F32
+    param: float = 0.0
+    force_general: bool = False
+
+    @staticmethod
+    def of(name: str, dtype=torch.float32, S: float = 0.0, force_general: bool = False) -> "Op":
+        return Op(OPCODES[name], F64 if dtype in (torch.float64, F64) else F32, float(S), bool(force_general))
+
+    def c(self) -> _OpStruct:
+        return _OpStruct(self.code, self.dtype, self.param, int(self.force_general), 0)
+
+    @property
+    def torch_dtype(self):
+        return torch.float64 if self.dtype == F64 else torch.float32
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load() -> ctypes.CDLL:
+    """Loads (building first if needed) libvjp_b200.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or os.environ.get("VJP_B200_REBUILD"):
+        path = _build.build()
+    lib = ctypes.CDLL(path)
+    vp, i64, sz, opp = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.POINTER(_OpStruct)
+    sig = {
+        "vjp_scan_arity": (ctypes.c_int, [opp]),
+        "vjp_version": (ctypes.c_char_p, []),
+        "vjp_scan_workspace_bytes": (sz, [opp, i64]),
+        "scan_forward": (ctypes.c_int, [opp, i64, vp, vp, vp, sz, vp]),
+        "vjp_scan": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_scan_host_scratch_bytes": (sz, [opp, i64]),
+        "vjp_scan_host": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_by_index_workspace_bytes": (sz, [opp, i64, i64]),
+        "reduce_by_index_forward": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_by_index": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_by_index_host_scratch_bytes": (sz, [opp, i64, i64]),
+        "vjp_reduce_by_index_host": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)  # AttributeError if the library does not export it
+        fn.restype, fn.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != OK:
+        raise VjpError("%s failed: %s (%d)" % (what, _STATUS.get(rc, "?"), rc))
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype) -> torch.Tensor:
+    if not t.is_cuda:
+        raise VjpError("expected a CUDA tensor (there is no CPU path)")
+    if t.dtype != dtype:
+        raise VjpError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return t.contiguous()
+
+
+def _workspace(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def scan_arity(op: Op) -> int:
+    o = op.c()
+    return load().vjp_scan_arity(ctypes.byref(o))
+
+
+def version() -> str:
+    return load().vjp_version().decode()
+
+
+def _scan_n(op: Op, xs: torch.Tensor) -> int:
+    d = scan_arity(op)
+    if d < 0:
+        raise VjpError("not a scan operator")
+    if xs.numel() % d:
+        raise VjpError("tensor size is not a multiple of the operator arity %d" % d)
+    return xs.numel() // d
+
+
+def vjp_scan_workspace_bytes(op: Op, n: int) -> int:
+    o = op.c()
+    return load().vjp_scan_workspace_bytes(ctypes.byref(o), n)
+
+
+def scan_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
+    """Primal inclusive scan."""
+    xs = _dev(xs, op.torch_dtype)
+    n = _scan_n(op, xs)
+    ys = torch.empty_like(xs) if out is None else out
+    ws = _workspace(vjp_scan_workspace_bytes(op, n), xs.device) if ws is None else ws
+    o = op.c()
+    _check(load().scan_forward(ctypes.byref(o), n, _ptr(xs), _ptr(ys), _ptr(ws), ws.numel(), _stream(stream)),
+           "scan_forward")
+    return ys
+
+
+def vjp_scan(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
+    """xs_bar = J^T ys_bar of the inclusive scan (Fig. 7).  xs may be None for '+'."""
+    ys_bar = _dev(ys_bar, op.torch_dtype)
+    if xs is not None:
+        xs = _dev(xs, op.torch_dtype)
+        if xs.shape != ys_bar.shape:
+            raise VjpError("xs and ys_bar differ in shape")
+    n = _scan_n(op, ys_bar)
+    xs_bar = torch.empty_like(ys_bar) if out is None else out
+    ws = _workspace(vjp_scan_workspace_bytes(op, n), ys_bar.device) if ws is None else ws
+    o = op.c()
+    _check(load().vjp_scan(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
+                           _stream(stream)), "vjp_scan")
+    return xs_bar
+
+
+def vjp_scan_host_scratch_bytes(op: Op, n: int) -> int:
+    o = op.c()
+    return load().vjp_scan_host_scratch_bytes(ctypes.byref(o), n)
+
+
+def vjp_scan_host(op: Op, xs, ys_bar: torch.Tensor, out: torch.Tensor, scratch: torch.Tensor, stream=None):
+    """HOST tensors in and out (pinned for speed); `scratch` is a device uint8 tensor."""
+    n = _scan_n(op, ys_bar)
+    o = op.c()
+    _check(load().vjp_scan_host(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(out), _ptr(scratch),
+                                scratch.numel(), _stream(stream)), "vjp_scan_host")
+    return out
+
+
+def vjp_reduce_by_index_workspace_bytes(op: Op, n: int, num_bins: int) -> int:
+    o = op.c()
+    return load().vjp_reduce_by_index_workspace_bytes(ctypes.byref(o), n, num_bins)
+
+
+def reduce_by_index_forward(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, out=None, ws=None,
+                            stream=None) -> torch.Tensor:
+    """Primal reduce_by_index over a neutral-initialised histogram."""
+    is_, vs = _dev(is_, torch.int64), _dev(vs, op.torch_dtype)
+    n = is_.numel()
+    hist = torch.empty(num_bins, dtype=op.torch_dtype, device=is_.device) if out is None else out
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    o = op.c()
+    _check(load().reduce_by_index_forward(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist),
+                                          _ptr(ws), ws.numel(), _stream(stream)), "reduce_by_index_forward")
+    return hist
+
+
+def vjp_reduce_by_index(op: Op, num_bins: int, is_: torch.Tensor, vs, hist_bar: torch.Tensor, out=None,
+                        ws=None, stream=None) -> torch.Tensor:
+    """vs_bar of reduce_by_index given hist_bar (Fig. 4 for the general rule)."""
+    is_ = _dev(is_, torch.int64)
+    hist_bar = _dev(hist_bar, op.torch_dtype)
+    if vs is not None:
+        vs = _dev(vs, op.torch_dtype)
+    n = is_.numel()
+    vs_bar = torch.empty(n, dtype=op.torch_dtype, device=is_.device) if out is None else out
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    o = op.c()
+    _check(load().vjp_reduce_by_index(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
+                                      _ptr(vs_bar), _ptr(ws), ws.numel(), _stream(stream)),
+           "vjp_reduce_by_index")
+    return vs_bar
+
+
+def vjp_reduce_by_index_host_scratch_bytes(op: Op, n: int, num_bins: int) -> int:
+    o = op.c()
+    return load().vjp_reduce_by_index_host_scratch_bytes(ctypes.byref(o), n, num_bins)
+
+
+def vjp_reduce_by_index_host(op: Op, num_bins: int, is_, vs, hist_bar, out, scratch, stream=None):
+    """HOST tensors in and out (pinned for speed); `scratch` is a device uint8 tensor."""
+    n = is_.numel()
+    o = op.c()
+    _check(load().vjp_reduce_by_index_host(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
+                                           _ptr(out), _ptr(scratch), scratch.numel(), _stream(stream)),
+           "vjp_reduce_by_index_host")
+    return out
+
+
+def rbi_argext(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=None, stream=None):
+    """(arg[w] int64 with n for an empty bin, ext[w]) of the lifted min/max primal (Fig. 5)."""
+    is_, vs = _dev(is_, torch.int64), _dev(vs, torch.float32)
+    n = is_.numel()
+    arg = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
+    ext = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    o = op.c()
+    _check(load().rbi_argext(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(arg), _ptr(ext), _ptr(ws),
+                             ws.numel(), _stream(stream)), "rbi_argext")
+    return arg, ext
+
+
+def rbi_zero_prod(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=None, stream=None):
+    """(zeros[w] int64, prod_nz[w]) of the lifted '*' primal."""
+    is_, vs = _dev(is_, torch.int64), _dev(vs, torch.float32)
+    n = is_.numel()
+    zeros = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
+    prod = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    o = op.c()
+    _check(load().rbi_zero_prod(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(zeros), _ptr(prod),
+                                _ptr(ws), ws.numel(), _stream(stream)), "rbi_zero_prod")
+    return zeros, prod
+
+
+def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
+    """(sorted_keys, perm) of the stable sort by clamped key (Fig. 4)."""
+    is_ = _dev(is_, torch.int64)
+    n = is_.numel()
+    sk = torch.empty(n, dtype=torch.int64, device=is_.device)
+    perm = torch.empty(n, dtype=torch.int64, device=is_.device)
+    if ws is None:
+        ws = _workspace(vjp_reduce_by_index_workspace_bytes(Op(OP_SATADD), n, num_bins), is_.device)
+    _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
+                                _stream(stream)), "rbi_sort_perm")
+    return sk, perm

@@ -1,0 +1,255 @@
+// api.cu -- the C ABI of include/vjp_b200.h: argument validation, workspace accounting and
+// dispatch.  No arithmetic of the method lives here.
+#include <cstring>
+
+#include "internal.h"
+
+using namespace vjp;
+
+namespace {
+
+bool op_ok(const vjp_op_t *op) {
+    return op && op->code >= VJP_OP_ADD && op->code <= VJP_OP_SATADD &&
+           (op->dtype == VJP_F32 || op->dtype == VJP_F64) && op->reserved == 0;
+}
+size_t dtype_bytes(int dtype) { return dtype == VJP_F64 ? 8 : 4; }
+
+bool scan_supported(const vjp_op_t *op) {
+    switch (op->code) {
+    case VJP_OP_ADD:
+    case VJP_OP_MUL: return true;
+    case VJP_OP_LINREC:
+    case VJP_OP_MATMUL2:
+    case VJP_OP_MATMUL5: return op->dtype == VJP_F32;
+    default: return false;
+    }
+}
+// Which reduce-by-index route an operator takes: 0 none, 1 '+', 2 min/max, 3 '*', 4 general.
+int rbi_route(const vjp_op_t *op) {
+    const bool f32 = op->dtype == VJP_F32;
+    switch (op->code) {
+    case VJP_OP_ADD: return op->force_general ? (f32 ? 4 : 0) : 1;
+    case VJP_OP_MIN:
+    case VJP_OP_MAX: return f32 ? (op->force_general ? 4 : 2) : 0;
+    case VJP_OP_MUL: return f32 ? (op->force_general ? 4 : 3) : 0;
+    case VJP_OP_SATADD: return f32 ? 4 : 0;
+    default: return 0;  // LINREC / MATMUL are not commutative
+    }
+}
+const int64_t RBI_MAX_N = 0xfffffffell;  // packed 32-bit positions
+
+cudaStream_t as_stream(void *s) { return static_cast<cudaStream_t>(s); }
+
+}  // namespace
+
+extern "C" {
+
+int vjp_scan_arity(const vjp_op_t *op) {
+    if (!op) return -1;
+    switch (op->code) {
+    case VJP_OP_ADD:
+    case VJP_OP_MUL: return 1;
+    case VJP_OP_LINREC: return 2;
+    case VJP_OP_MATMUL2: return 4;
+    case VJP_OP_MATMUL5: return 25;
+    default: return -1;
+    }
+}
+
+const char *vjp_version(void) { return "vjp_b200 0.1 (sm_100a, CUDA " VJP_STR(CUDART_VERSION) ")"; }
+
+// ------------------------------------------------------------------------------ scan -----
+
+size_t vjp_scan_workspace_bytes(const vjp_op_t *op, int64_t n) {
+    if (!op_ok(op) || !scan_supported(op) || n < 0) return 0;
+    return scan_workspace_bytes(op->code, op->dtype, n);
+}
+
+int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys, void *ws,
+                 size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!xs || !ys || !ws) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < scan_workspace_bytes(op->code, op->dtype, n)) return VJP_ERR_WORKSPACE;
+    return launch_scan_forward(op->code, op->dtype, n, xs, ys, ws, as_stream(stream));
+}
+
+int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar,
+             void *ws, size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!ys_bar || !xs_bar || !ws || (!xs && op->code != VJP_OP_ADD)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < scan_workspace_bytes(op->code, op->dtype, n)) return VJP_ERR_WORKSPACE;
+    return launch_scan_vjp(op->code, op->dtype, n, xs, ys_bar, xs_bar, ws, as_stream(stream));
+}
+
+size_t vjp_scan_host_scratch_bytes(const vjp_op_t *op, int64_t n) {
+    if (!op_ok(op) || !scan_supported(op) || n < 0) return 0;
+    const size_t arr = align_up((size_t)n * vjp_scan_arity(op) * dtype_bytes(op->dtype), 256);
+    return 3 * arr + scan_workspace_bytes(op->code, op->dtype, n);
+}
+
+int vjp_scan_host(const vjp_op_t *op, int64_t n, const void *xs_host, const void *ys_bar_host,
+                  void *xs_bar_host, void *dev_scratch, size_t dev_scratch_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!ys_bar_host || !xs_bar_host || !dev_scratch || (!xs_host && op->code != VJP_OP_ADD))
+        return VJP_ERR_INVALID_ARG;
+    if (dev_scratch_bytes < vjp_scan_host_scratch_bytes(op, n)) return VJP_ERR_WORKSPACE;
+    cudaStream_t s = as_stream(stream);
+    const size_t bytes = (size_t)n * vjp_scan_arity(op) * dtype_bytes(op->dtype);
+    const size_t arr = align_up(bytes, 256);
+    char *d = static_cast<char *>(dev_scratch);
+    char *dx = d, *dy = d + arr, *dout = d + 2 * arr, *ws = d + 3 * arr;
+    if (xs_host && op->code != VJP_OP_ADD &&
+        cudaMemcpyAsync(dx, xs_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    if (cudaMemcpyAsync(dy, ys_bar_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    int rc = launch_scan_vjp(op->code, op->dtype, n, dx, dy, dout, ws, s);
+    if (rc != VJP_OK) return rc;
+    if (cudaMemcpyAsync(xs_bar_host, dout, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    return cuda_status(cudaStreamSynchronize(s));
+}
+
+// ------------------------------------------------------------------- reduce-by-index -----
+
+size_t vjp_reduce_by_index_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t num_bins) {
+    if (!op_ok(op) || n < 0 || num_bins < 0) return 0;
+    switch (rbi_route(op)) {
+    case 1:
+    case 2:
+    case 3: return rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins);
+    case 4: return rbi_general_workspace_bytes(n, num_bins);
+    default: return 0;
+    }
+}
+
+int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                            const void *vs, void *hist, void *ws, size_t ws_bytes, void *stream) {
+    (void)ws_bytes;
+    if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (rbi_route(op) == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if ((num_bins > 0 && !hist) || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    return launch_rbi_forward(op->code, op->dtype, op->param, n, num_bins, is, vs, hist, ws,
+                              as_stream(stream));
+}
+
+int vjp_reduce_by_index(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                        const void *vs, const void *hist_bar, void *vs_bar, void *ws,
+                        size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    const int route = rbi_route(op);
+    if (route == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!is || !vs_bar || (num_bins > 0 && !hist_bar) || (!vs && route != 1)) return VJP_ERR_INVALID_ARG;
+    if (!ws || ws_bytes < vjp_reduce_by_index_workspace_bytes(op, n, num_bins)) return VJP_ERR_WORKSPACE;
+    cudaStream_t s = as_stream(stream);
+    switch (route) {
+    case 1: return launch_rbi_vjp_add(op->dtype, n, num_bins, is, hist_bar, vs_bar, s);
+    case 2:
+        return launch_rbi_minmax(op->code, n, num_bins, is, static_cast<const float *>(vs),
+                                 static_cast<const float *>(hist_bar), static_cast<float *>(vs_bar),
+                                 nullptr, nullptr, ws, s);
+    case 3:
+        return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs),
+                              static_cast<const float *>(hist_bar), static_cast<float *>(vs_bar),
+                              nullptr, nullptr, ws, s);
+    default:
+        return launch_rbi_general_vjp(op->code, op->param, n, num_bins, is,
+                                      static_cast<const float *>(vs),
+                                      static_cast<const float *>(hist_bar),
+                                      static_cast<float *>(vs_bar), ws, s);
+    }
+}
+
+size_t vjp_reduce_by_index_host_scratch_bytes(const vjp_op_t *op, int64_t n, int64_t num_bins) {
+    if (!op_ok(op) || n < 0 || num_bins < 0 || rbi_route(op) == 0) return 0;
+    const size_t e = dtype_bytes(op->dtype);
+    return align_up((size_t)n * 8, 256) + 2 * align_up((size_t)n * e, 256) +
+           align_up((size_t)num_bins * e, 256) + vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
+}
+
+int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
+                             const int64_t *is_host, const void *vs_host,
+                             const void *hist_bar_host, void *vs_bar_host, void *dev_scratch,
+                             size_t dev_scratch_bytes, void *stream) {
+    if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    const int route = rbi_route(op);
+    if (route == 0) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!is_host || !vs_bar_host || !dev_scratch || (num_bins > 0 && !hist_bar_host) ||
+        (!vs_host && route != 1))
+        return VJP_ERR_INVALID_ARG;
+    if (dev_scratch_bytes < vjp_reduce_by_index_host_scratch_bytes(op, n, num_bins))
+        return VJP_ERR_WORKSPACE;
+    cudaStream_t s = as_stream(stream);
+    const size_t e = dtype_bytes(op->dtype);
+    char *d = static_cast<char *>(dev_scratch);
+    char *dis = d;
+    char *dvs = dis + align_up((size_t)n * 8, 256);
+    char *dout = dvs + align_up((size_t)n * e, 256);
+    char *dhb = dout + align_up((size_t)n * e, 256);
+    char *ws = dhb + align_up((size_t)num_bins * e, 256);
+    const size_t ws_bytes = vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
+    if (cudaMemcpyAsync(dis, is_host, (size_t)n * 8, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    if (route != 1 &&
+        cudaMemcpyAsync(dvs, vs_host, (size_t)n * e, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    if (num_bins > 0 &&
+        cudaMemcpyAsync(dhb, hist_bar_host, (size_t)num_bins * e, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    int rc = vjp_reduce_by_index(op, n, num_bins, reinterpret_cast<const int64_t *>(dis), dvs, dhb,
+                                 dout, ws, ws_bytes, stream);
+    if (rc != VJP_OK) return rc;
+    if (cudaMemcpyAsync(vs_bar_host, dout, (size_t)n * e, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    return cuda_status(cudaStreamSynchronize(s));
+}
+
+int rbi_argext(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is, const void *vs,
+               int64_t *arg, void *ext, void *ws, size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if ((op->code != VJP_OP_MIN && op->code != VJP_OP_MAX) || op->dtype != VJP_F32)
+        return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (num_bins == 0) return VJP_OK;
+    if (!arg || !ext || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (!ws || ws_bytes < rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins))
+        return VJP_ERR_WORKSPACE;
+    return launch_rbi_minmax(op->code, n, num_bins, is, static_cast<const float *>(vs), nullptr,
+                             nullptr, arg, static_cast<float *>(ext), ws, as_stream(stream));
+}
+
+int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
+                  const void *vs, int64_t *zeros, void *prod_nz, void *ws, size_t ws_bytes,
+                  void *stream) {
+    if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (op->code != VJP_OP_MUL || op->dtype != VJP_F32) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (num_bins == 0) return VJP_OK;
+    if (!zeros || !prod_nz || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (!ws || ws_bytes < rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins))
+        return VJP_ERR_WORKSPACE;
+    return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs), nullptr, nullptr, zeros,
+                          static_cast<float *>(prod_nz), ws, as_stream(stream));
+}
+
+int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
+                  int64_t *perm, void *ws, size_t ws_bytes, void *stream) {
+    if (n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!is || !sorted_keys || !perm) return VJP_ERR_INVALID_ARG;
+    if (!ws || ws_bytes < rbi_general_workspace_bytes(n, num_bins)) return VJP_ERR_WORKSPACE;
+    return launch_rbi_sort_perm(n, num_bins, is, sorted_keys, perm, ws, as_stream(stream));
+}
+
+}  // extern "C"

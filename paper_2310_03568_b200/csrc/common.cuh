@@ -298,6 +298,59 @@ struct TileStage {
     }
 };
 
+// Rows whose word count is not a multiple of 4 (the 25-word 5x5 matrix): the tile keeps its
+// global (linear) layout in shared memory.  Whole-tile copies still move 16-byte chunks; a
+// thread reads its row with 32-bit accesses, conflict-free when RW is odd.
+template <int NT, int RW>
+struct TileStageLinear {
+    static constexpr int TILE_WORDS = NT * RW;
+    static_assert(TILE_WORDS % 4 == 0, "tile must be a whole number of 16-byte chunks");
+    static constexpr int TILE_CHUNKS = TILE_WORDS / 4;
+    static constexpr int SMEM_BYTES = TILE_WORDS * 4;
+
+    template <int FW>
+    static VJP_DEVINL void load(uint4 *smem, const uint32_t *__restrict__ g, int valid_words,
+                                const uint32_t (&fill)[FW]) {
+        static_assert(RW % FW == 0, "fill pattern must tile a row");
+        const uint4 *g4 = reinterpret_cast<const uint4 *>(g);
+        if (valid_words == TILE_WORDS) {
+#pragma unroll
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) smem[c] = ldg_stream(g4 + c);
+        } else {
+            uint32_t *s = reinterpret_cast<uint32_t *>(smem);
+            for (int wi = threadIdx.x; wi < TILE_WORDS; wi += NT)
+                s[wi] = (wi < valid_words) ? __ldg(g + wi) : fill[wi % FW];
+        }
+    }
+    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words) {
+        uint4 *g4 = reinterpret_cast<uint4 *>(g);
+        if (valid_words == TILE_WORDS) {
+#pragma unroll
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) stg_stream(g4 + c, smem[c]);
+        } else {
+            const uint32_t *s = reinterpret_cast<const uint32_t *>(smem);
+            for (int wi = threadIdx.x; wi < valid_words; wi += NT) g[wi] = s[wi];
+        }
+    }
+    static VJP_DEVINL void read_row(const uint4 *smem, int row, uint32_t (&r)[RW]) {
+        const uint32_t *s = reinterpret_cast<const uint32_t *>(smem) + row * RW;
+#pragma unroll
+        for (int k = 0; k < RW; k++) r[k] = s[k];
+    }
+    static VJP_DEVINL void write_row(uint4 *smem, int row, const uint32_t (&r)[RW]) {
+        uint32_t *s = reinterpret_cast<uint32_t *>(smem) + row * RW;
+#pragma unroll
+        for (int k = 0; k < RW; k++) s[k] = r[k];
+    }
+};
+
+template <int NT, int RW, bool ALIGNED = (RW % 4 == 0)>
+struct StageSelect { using type = TileStage<NT, RW>; };
+template <int NT, int RW>
+struct StageSelect<NT, RW, false> { using type = TileStageLinear<NT, RW>; };
+template <int NT, int RW>
+using Stage = typename StageSelect<NT, RW>::type;
+
 // words <-> scalars
 VJP_DEVINL float word_to(const uint32_t *w, float *) { return __uint_as_float(w[0]); }
 VJP_DEVINL double word_to(const uint32_t *w, double *) {

@@ -1,0 +1,53 @@
+// internal.h -- host-side declarations shared by the translation units of libvjp_b200.so.
+// Each launch_* function validates nothing: api.cu has already checked the arguments and the
+// workspace size.  All pointers are device pointers; every function only enqueues on `stream`
+// and returns a vjp_status_t.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/vjp_b200.h"
+
+#define VJP_STR2(x) #x
+#define VJP_STR(x) VJP_STR2(x)
+
+namespace vjp {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? VJP_OK : VJP_ERR_CUDA; }
+inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
+
+// ------------------------------------------------------------------------------ scans ---
+size_t scan_workspace_bytes(int code, int dtype, int64_t n);
+int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,
+                        cudaStream_t stream);
+int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *ys_bar,
+                    void *xs_bar, void *ws, cudaStream_t stream);
+
+// -------------------------------------------------------------- reduce-by-index (special) -
+size_t rbi_special_workspace_bytes(int code, int dtype, int64_t n, int64_t w);
+int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, const int64_t *is,
+                       const void *vs, void *hist, void *ws, cudaStream_t stream);
+int launch_rbi_vjp_add(int dtype, int64_t n, int64_t w, const int64_t *is, const void *hist_bar,
+                       void *vs_bar, cudaStream_t stream);
+// MIN / MAX: lifted primal into ws, then (arg, ext) and / or the return sweep.
+int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                      const float *hist_bar, float *vs_bar, int64_t *arg, float *ext, void *ws,
+                      cudaStream_t stream);
+// MUL: lifted primal into ws, then (zeros, prod_nz) and / or the return sweep.
+int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
+                   const float *hist_bar, float *vs_bar, int64_t *zeros, float *prod_nz, void *ws,
+                   cudaStream_t stream);
+
+// -------------------------------------------------------------- reduce-by-index (general) -
+size_t rbi_general_workspace_bytes(int64_t n, int64_t w);
+int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
+                           const float *vs, const float *hist_bar, float *vs_bar, void *ws,
+                           cudaStream_t stream);
+int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
+                         int64_t *perm, void *ws, cudaStream_t stream);
+
+}  // namespace vjp

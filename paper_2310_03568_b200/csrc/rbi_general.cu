@@ -1,0 +1,602 @@
+// rbi_general.cu -- the general-case rule for reduce-by-index (Fig. 4, eq. 5):
+//
+//   (sks, siota) = radix sort of (clamped key, iota)            P:L350-351, P:L396   G1
+//   svs          = values carried through the sort as payload   P:L396               G2
+//   segment flags from adjacent sorted keys (never stored)      P:L352-355           G3
+//   ls = forward segmented exclusive scan of svs                P:L356, P:L400       G4
+//   rs = reverse segmented exclusive scan of svs                P:L357-358, P:L402   G5
+//   sv_bar_j = d(l_j (.) x (.) r_j)/dx at svs_j  *  hist_bar[sks_j]   (0 if out of range)  G6
+//   vs_bar[siota_j] = sv_bar_j                                  P:L365-367           G7
+//
+// G1-G2: stable LSD radix sort over the ceil(log2(w+1)) key bits only, each pass = per-tile digit
+// histogram, one exclusive scan over the [digit][tile] table, and a ranking + scatter kernel
+// (warp-level match ranking keeps equal digits in input order).  G4 and G5-G7 are single-pass
+// decoupled-look-back segmented scans whose (status, segment flag, value) triple fits one 64-bit
+// word; G5-G7 are fused into one kernel.  Keys outside [0,w) are clamped to w (Q18): they sort
+// behind every bin, in input order, and receive adjoint 0.
+#include <math_constants.h>
+
+#include "common.cuh"
+#include "internal.h"
+
+namespace vjp {
+
+// ------------------------------------------------------------------ packed look-back ------
+// word = status (bits 62-63) | payload (bits 0-32: value bits 0-31, segment flag bit 32)
+
+constexpr int PK_NT = 256;
+enum : uint64_t { PK_EMPTY = 0, PK_AGG = 1, PK_PREFIX = 2 };
+constexpr uint64_t PK_PAYLOAD = (1ull << 33) - 1;
+
+VJP_DEVINL uint64_t ld_relaxed_u64(const uint64_t *p) {
+    uint64_t v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+VJP_DEVINL void st_relaxed_u64(uint64_t *p, uint64_t v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+VJP_DEVINL uint64_t shfl_u64(uint64_t v, int src) {
+    const uint32_t lo = __shfl_sync(FULL_MASK, (uint32_t)v, src);
+    const uint32_t hi = __shfl_sync(FULL_MASK, (uint32_t)(v >> 32), src);
+    return ((uint64_t)hi << 32) | lo;
+}
+
+// Exclusive scan of one payload per thread in processing order (REVT: thread NT-1 first).
+template <int NT, bool REVT, class F>
+VJP_DEVINL uint64_t block_exclusive_u64(uint64_t local, uint64_t &total, uint64_t ident, F comb,
+                                        uint64_t *scratch /* NT/32 + 1 */) {
+    constexpr int NW = NT / 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int plane = REVT ? 31 - lane : lane;
+    const int pwarp = REVT ? NW - 1 - warp : warp;
+    __syncthreads();
+    uint64_t incl = local;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const uint64_t o = shfl_u64(incl, REVT ? lane + off : lane - off);
+        if (plane >= off) incl = comb(o, incl);
+    }
+    uint64_t ex = shfl_u64(incl, REVT ? lane + 1 : lane - 1);
+    if (plane == 0) ex = ident;
+    if (plane == 31) scratch[pwarp] = incl;
+    __syncthreads();
+    if (warp == 0) {
+        const uint64_t wt = lane < NW ? scratch[lane] : ident;
+        uint64_t wi = wt;
+#pragma unroll
+        for (int off = 1; off < NW; off <<= 1) {
+            const uint64_t o = shfl_u64(wi, lane - off);
+            if (lane >= off) wi = comb(o, wi);
+        }
+        uint64_t wex = shfl_u64(wi, lane - 1);
+        if (lane == 0) wex = ident;
+        __syncwarp();
+        if (lane < NW) scratch[lane] = wex;
+        if (lane == NW - 1) scratch[NW] = wi;
+    }
+    __syncthreads();
+    total = scratch[NW];
+    if (pwarp > 0) ex = comb(scratch[pwarp], ex);
+    return ex;
+}
+
+// Called by warp 0.  Publishes the tile aggregate, folds the predecessors, publishes the inclusive
+// prefix, returns the exclusive prefix of tile p (processing order).
+template <class F>
+VJP_DEVINL uint64_t packed_tile_prefix(uint64_t *status, int p, uint64_t total, uint64_t ident,
+                                       F comb) {
+    const int lane = threadIdx.x & 31;
+    if (p == 0) {
+        if (lane == 0) st_relaxed_u64(status, (PK_PREFIX << 62) | total);
+        return ident;
+    }
+    if (lane == 0) st_relaxed_u64(status + p, (PK_AGG << 62) | total);
+    uint64_t acc = ident;
+    int base = p - 1;
+    while (true) {
+        const int q = base - lane;
+        uint64_t word = (PK_PREFIX << 62) | ident;
+        if (q >= 0) word = ld_relaxed_u64(status + q);
+        while (__any_sync(FULL_MASK, (word >> 62) == PK_EMPTY)) {
+            if ((word >> 62) == PK_EMPTY) {
+                __nanosleep(32);
+                word = ld_relaxed_u64(status + q);
+            }
+        }
+        const unsigned pm = __ballot_sync(FULL_MASK, (word >> 62) == PK_PREFIX);
+        const int first = __ffs(pm) - 1;
+        uint64_t s = (first < 0 || lane <= first) ? (word & PK_PAYLOAD) : ident;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const uint64_t o = shfl_u64(s, lane + off);
+            if (lane + off < 32) s = comb(o, s);
+        }
+        s = shfl_u64(s, 0);
+        acc = comb(s, acc);
+        if (pm != 0) break;
+        base -= 32;
+    }
+    if (lane == 0) st_relaxed_u64(status + p, (PK_PREFIX << 62) | comb(acc, total));
+    return acc;
+}
+
+// ------------------------------------------------------------------ u32 exclusive scan ----
+// of the [digit][tile] histogram table.
+
+struct AddComb {
+    VJP_DEVINL uint64_t operator()(uint64_t a, uint64_t b) const { return (uint32_t)(a + b); }
+};
+constexpr int US_NT = 256, US_IPT = 8;
+
+__global__ void __launch_bounds__(US_NT)
+u32_exclusive_scan_kernel(uint32_t *data, int64_t m, int *ticket, uint64_t *status) {
+    __shared__ uint64_t scratch[US_NT / 32 + 2];
+    __shared__ int s_p;
+    if (threadIdx.x == 0) s_p = atomicAdd(ticket, 1);
+    __syncthreads();
+    const int p = s_p;
+    const int64_t base = (int64_t)p * (US_NT * US_IPT) + threadIdx.x * US_IPT;
+    uint32_t v[US_IPT];
+    uint32_t sum = 0;
+    if (base + US_IPT <= m) {
+        const uint4 a = *reinterpret_cast<const uint4 *>(data + base);
+        const uint4 b = *reinterpret_cast<const uint4 *>(data + base + 4);
+        v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+    } else {
+#pragma unroll
+        for (int j = 0; j < US_IPT; j++) v[j] = (base + j < m) ? data[base + j] : 0u;
+    }
+#pragma unroll
+    for (int j = 0; j < US_IPT; j++) sum += v[j];
+    uint64_t total;
+    uint64_t ex = block_exclusive_u64<US_NT, false>(sum, total, 0ull, AddComb(), scratch);
+    if (threadIdx.x < 32) {
+        const uint64_t pre = packed_tile_prefix(status, p, total, 0ull, AddComb());
+        if (threadIdx.x == 0) scratch[US_NT / 32 + 1] = pre;
+    }
+    __syncthreads();
+    uint32_t run = (uint32_t)(scratch[US_NT / 32 + 1] + ex);
+#pragma unroll
+    for (int j = 0; j < US_IPT; j++) {
+        const uint32_t c = v[j];
+        v[j] = run;
+        run += c;
+    }
+    if (base + US_IPT <= m) {
+        *reinterpret_cast<uint4 *>(data + base) = make_uint4(v[0], v[1], v[2], v[3]);
+        *reinterpret_cast<uint4 *>(data + base + 4) = make_uint4(v[4], v[5], v[6], v[7]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < US_IPT; j++)
+            if (base + j < m) data[base + j] = v[j];
+    }
+}
+
+// ------------------------------------------------------------------ radix sort passes -----
+
+constexpr int SORT_NT = 256;
+constexpr int SORT_IPT = 16;
+constexpr int SORT_TILE = SORT_NT * SORT_IPT;  // 4096 keys; warp w owns keys [512 w, 512 w + 512)
+constexpr int SORT_MAX_RADIX = 256;
+
+// key' = k if 0 <= k < w else w (Q18)
+VJP_DEVINL uint32_t clamp_key(int64_t k, int64_t w) {
+    return (uint64_t)k < (uint64_t)w ? (uint32_t)k : (uint32_t)w;
+}
+
+template <bool FIRST>
+VJP_DEVINL uint32_t sort_load_key(const int64_t *__restrict__ is, const uint32_t *__restrict__ kin,
+                                  int64_t i, int64_t w) {
+    return FIRST ? clamp_key(__ldg(is + i), w) : __ldg(kin + i);
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(SORT_NT)
+sort_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                 const uint32_t *__restrict__ kin, int shift, int radix, int num_tiles,
+                 uint32_t *__restrict__ counts) {
+    __shared__ uint32_t h[SORT_MAX_RADIX];
+    for (int d = threadIdx.x; d < radix; d += SORT_NT) h[d] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+    const uint32_t mask = (uint32_t)radix - 1;
+#pragma unroll 4
+    for (int j = 0; j < SORT_IPT; j++) {
+        const int64_t i = base + j * SORT_NT + threadIdx.x;
+        if (i < n) atomicAdd(&h[(sort_load_key<FIRST>(is, kin, i, w) >> shift) & mask], 1u);
+    }
+    __syncthreads();
+    for (int d = threadIdx.x; d < radix; d += SORT_NT)
+        counts[(size_t)d * num_tiles + blockIdx.x] = h[d];
+}
+
+// Stable ranking + scatter.  In round j, lane l of warp wp holds key number 512 wp + 32 j + l of
+// the tile, so "earlier in the input" = (lower warp, lower round, lower lane): the rank of a key
+// among equal digits is  offset[warp][digit] + (keys of that digit in earlier rounds of the warp)
+// + (lower lanes with that digit in this round).
+template <bool FIRST>
+__global__ void __launch_bounds__(SORT_NT)
+sort_scatter_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                    const float *__restrict__ vs, const uint32_t *__restrict__ kin,
+                    const uint2 *__restrict__ pin, int shift, int radix, int num_tiles,
+                    const uint32_t *__restrict__ offsets, uint32_t *__restrict__ kout,
+                    uint2 *__restrict__ pout) {
+    constexpr int NW = SORT_NT / 32;
+    __shared__ uint32_t cnt[NW][SORT_MAX_RADIX];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int d = threadIdx.x; d < NW * SORT_MAX_RADIX; d += SORT_NT) (&cnt[0][0])[d] = 0;
+    __syncthreads();
+    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + warp * (32 * SORT_IPT);
+    const uint32_t mask = (uint32_t)radix - 1;
+    const unsigned lt = (1u << lane) - 1;
+    uint32_t key[SORT_IPT];
+    uint16_t rank[SORT_IPT];
+#pragma unroll
+    for (int j = 0; j < SORT_IPT; j++) {
+        const int64_t i = wbase + j * 32 + lane;
+        const bool valid = i < n;
+        key[j] = valid ? sort_load_key<FIRST>(is, kin, i, w) : 0u;
+        const unsigned vm = __ballot_sync(FULL_MASK, valid);
+        if (valid) {
+            const uint32_t d = (key[j] >> shift) & mask;
+            const unsigned peers = __match_any_sync(vm, d);
+            const uint32_t before = cnt[warp][d];
+            __syncwarp(vm);
+            if ((peers & lt) == 0) cnt[warp][d] = before + __popc(peers);
+            __syncwarp(vm);
+            rank[j] = (uint16_t)(before + __popc(peers & lt));
+        }
+    }
+    __syncthreads();
+    // per digit: global base of (digit, tile) + exclusive prefix over the warps
+    for (int d = threadIdx.x; d < radix; d += SORT_NT) {
+        uint32_t run = offsets[(size_t)d * num_tiles + blockIdx.x];
+#pragma unroll
+        for (int x = 0; x < NW; x++) {
+            const uint32_t c = cnt[x][d];
+            cnt[x][d] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < SORT_IPT; j++) {
+        const int64_t i = wbase + j * 32 + lane;
+        if (i < n) {
+            const uint32_t d = (key[j] >> shift) & mask;
+            const uint32_t pos = cnt[warp][d] + rank[j];
+            kout[pos] = key[j];
+            pout[pos] = FIRST ? make_uint2((uint32_t)i, vs ? __float_as_uint(__ldg(vs + i)) : 0u)
+                              : __ldg(pin + i);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ operators -------------
+
+enum : int { G_ADD = 0, G_MIN = 1, G_MAX = 2, G_MUL = 3, G_SATADD = 4 };
+
+// The operator, its neutral element, and d/dx of (l (.) x) (.) r at x = v (eq. 5).
+template <int CODE>
+struct GenOp {
+    float S;
+    VJP_DEVINL float neutral() const {
+        return CODE == G_MUL ? 1.f : CODE == G_MIN ? CUDART_INF_F : CODE == G_MAX ? -CUDART_INF_F : 0.f;
+    }
+    VJP_DEVINL float apply(float a, float b) const {
+        switch (CODE) {
+        case G_ADD: return a + b;
+        case G_MUL: return a * b;
+        case G_MIN: return b < a ? b : a;
+        case G_MAX: return b > a ? b : a;
+        default: return fminf(a + b, S);
+        }
+    }
+    // min / max: the accumulated (left) operand wins ties, so among equal extrema the lowest index
+    // gets the adjoint, as with min^L.  satadd: slope 1 strictly below S (Q17).
+    VJP_DEVINL float dfdx(float l, float v, float r) const {
+        switch (CODE) {
+        case G_ADD: return 1.f;
+        case G_MUL: return l * r;
+        case G_MIN: return (v < l && !(r < v)) ? 1.f : 0.f;
+        case G_MAX: return (v > l && !(r > v)) ? 1.f : 0.f;
+        default: {
+            const float s = l + v;
+            return (s < S && s + r < S) ? 1.f : 0.f;
+        }
+        }
+    }
+};
+
+// Segmented-scan combine on payloads (flag << 32 | value bits).  REV: "earlier" holds the HIGHER
+// indices, and the fold keeps index order: value = later (.) earlier.
+template <int CODE, bool REV>
+struct SegComb {
+    GenOp<CODE> op;
+    VJP_DEVINL uint64_t operator()(uint64_t earlier, uint64_t later) const {
+        const float ve = __uint_as_float((uint32_t)earlier), vl = __uint_as_float((uint32_t)later);
+        const bool fl = (later >> 32) & 1;
+        const float v = fl ? vl : (REV ? op.apply(vl, ve) : op.apply(ve, vl));
+        return (((earlier | later) >> 32) & 1) << 32 | __float_as_uint(v);
+    }
+};
+
+// ------------------------------------------------------------------ segmented scans -------
+
+constexpr int SEG_NT = 256;
+constexpr int SEG_IPT = 8;
+constexpr int SEG_TILE = SEG_NT * SEG_IPT;
+
+// G4: ls[j] = fold of the same-key elements before j (neutral at a segment head).
+template <int CODE>
+__global__ void __launch_bounds__(SEG_NT)
+seg_forward_kernel(int64_t n, const uint32_t *__restrict__ keys, const uint2 *__restrict__ pay,
+                   float *__restrict__ ls, GenOp<CODE> op, int *ticket, uint64_t *status) {
+    using KS = Stage<SEG_NT, SEG_IPT>;
+    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
+    extern __shared__ uint4 smem[];
+    uint4 *sk = smem;
+    uint4 *sp = smem + KS::SMEM_BYTES / 16;
+    __shared__ uint64_t scratch[SEG_NT / 32 + 2];
+    __shared__ uint32_t last_key[SEG_NT];
+    __shared__ int s_p;
+    if (threadIdx.x == 0) s_p = atomicAdd(ticket, 1);
+    __syncthreads();
+    const int p = s_p;
+    const int64_t base = (int64_t)p * SEG_TILE;
+    const int valid = (int)min((int64_t)SEG_TILE, n - base);
+    const uint32_t fillk[1] = {0xffffffffu};  // a key no element has: the padding is its own segment
+    const uint32_t fillp[1] = {0u};
+    KS::load(sk, keys + base, valid, fillk);
+    PS::load(sp, reinterpret_cast<const uint32_t *>(pay + base), 2 * valid, fillp);
+    __syncthreads();
+    uint32_t k[SEG_IPT], pw[2 * SEG_IPT];
+    KS::read_row(sk, threadIdx.x, k);
+    PS::read_row(sp, threadIdx.x, pw);
+    last_key[threadIdx.x] = k[SEG_IPT - 1];
+    __syncthreads();
+    uint32_t prev;
+    bool first_head = false;
+    if (threadIdx.x > 0) prev = last_key[threadIdx.x - 1];
+    else if (base > 0) prev = __ldg(keys + base - 1);
+    else { prev = 0; first_head = true; }
+
+    const SegComb<CODE, false> comb{op};
+    const uint64_t ident = __float_as_uint(op.neutral());
+    bool head[SEG_IPT];
+    uint64_t acc = ident;
+#pragma unroll
+    for (int j = 0; j < SEG_IPT; j++) {
+        head[j] = (j == 0) ? (first_head || k[0] != prev) : (k[j] != k[j - 1]);
+        acc = comb(acc, ((uint64_t)head[j] << 32) | pw[2 * j + 1]);
+    }
+    uint64_t total;
+    const uint64_t ex = block_exclusive_u64<SEG_NT, false>(acc, total, ident, comb, scratch);
+    if (threadIdx.x < 32) {
+        const uint64_t pre = packed_tile_prefix(status, p, total, ident, comb);
+        if (threadIdx.x == 0) scratch[SEG_NT / 32 + 1] = pre;
+    }
+    __syncthreads();
+    float run = __uint_as_float((uint32_t)comb(scratch[SEG_NT / 32 + 1], ex));
+    uint32_t out[SEG_IPT];
+#pragma unroll
+    for (int j = 0; j < SEG_IPT; j++) {
+        const float v = __uint_as_float(pw[2 * j + 1]);
+        const float l = head[j] ? op.neutral() : run;
+        out[j] = __float_as_uint(l);
+        run = op.apply(l, v);
+    }
+    __syncthreads();  // every thread has read its key row
+    KS::write_row(sk, threadIdx.x, out);
+    __syncthreads();
+    KS::store(sk, reinterpret_cast<uint32_t *>(ls) + base, valid);
+}
+
+// G5-G7 fused: reverse segmented exclusive scan, per-element derivative, un-permute.
+template <int CODE>
+__global__ void __launch_bounds__(SEG_NT)
+seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
+                       const uint2 *__restrict__ pay, const float *__restrict__ ls,
+                       const float *__restrict__ hist_bar, float *__restrict__ vs_bar,
+                       GenOp<CODE> op, int num_tiles, int *ticket, uint64_t *status) {
+    using KS = Stage<SEG_NT, SEG_IPT>;
+    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
+    extern __shared__ uint4 smem[];
+    uint4 *sk = smem;
+    uint4 *sl = sk + KS::SMEM_BYTES / 16;
+    uint4 *sp = sl + KS::SMEM_BYTES / 16;
+    __shared__ uint64_t scratch[SEG_NT / 32 + 2];
+    __shared__ uint32_t first_key[SEG_NT];
+    __shared__ int s_p;
+    if (threadIdx.x == 0) s_p = atomicAdd(ticket, 1);
+    __syncthreads();
+    const int p = s_p;
+    const int t = num_tiles - 1 - p;
+    const int64_t base = (int64_t)t * SEG_TILE;
+    const int valid = (int)min((int64_t)SEG_TILE, n - base);
+    const uint32_t fillk[1] = {0xffffffffu};
+    const uint32_t fill0[1] = {0u};
+    KS::load(sk, keys + base, valid, fillk);
+    KS::load(sl, reinterpret_cast<const uint32_t *>(ls) + base, valid, fill0);
+    PS::load(sp, reinterpret_cast<const uint32_t *>(pay + base), 2 * valid, fill0);
+    __syncthreads();
+    uint32_t k[SEG_IPT], lw[SEG_IPT], pw[2 * SEG_IPT];
+    KS::read_row(sk, threadIdx.x, k);
+    KS::read_row(sl, threadIdx.x, lw);
+    PS::read_row(sp, threadIdx.x, pw);
+    first_key[threadIdx.x] = k[0];
+    __syncthreads();
+    uint32_t next;
+    bool last_tail = false;
+    if (threadIdx.x < SEG_NT - 1) next = first_key[threadIdx.x + 1];
+    else if (base + SEG_TILE < n) next = __ldg(keys + base + SEG_TILE);
+    else { next = 0; last_tail = true; }
+
+    const SegComb<CODE, true> comb{op};
+    const uint64_t ident = __float_as_uint(op.neutral());
+    bool tail[SEG_IPT];  // segment boundary seen from the right
+    uint64_t acc = ident;
+#pragma unroll
+    for (int j = SEG_IPT - 1; j >= 0; j--) {
+        tail[j] = (j == SEG_IPT - 1) ? (last_tail || k[j] != next) : (k[j] != k[j + 1]);
+        acc = comb(acc, ((uint64_t)tail[j] << 32) | pw[2 * j + 1]);
+    }
+    uint64_t total;
+    const uint64_t ex = block_exclusive_u64<SEG_NT, true>(acc, total, ident, comb, scratch);
+    if (threadIdx.x < 32) {
+        const uint64_t pre = packed_tile_prefix(status, p, total, ident, comb);
+        if (threadIdx.x == 0) scratch[SEG_NT / 32 + 1] = pre;
+    }
+    __syncthreads();
+    float run = __uint_as_float((uint32_t)comb(scratch[SEG_NT / 32 + 1], ex));
+    const int mine = valid - threadIdx.x * SEG_IPT;  // number of real elements in this row
+#pragma unroll
+    for (int j = SEG_IPT - 1; j >= 0; j--) {
+        const float v = __uint_as_float(pw[2 * j + 1]);
+        const float r = tail[j] ? op.neutral() : run;
+        run = op.apply(v, r);
+        if (j < mine) {
+            float g = 0.f;
+            if (k[j] < (uint32_t)w)  // out-of-range keys were clamped to w: adjoint 0
+                g = op.dfdx(__uint_as_float(lw[j]), v, r) * __ldg(hist_bar + k[j]);
+            vs_bar[pw[2 * j]] = g;
+        }
+    }
+}
+
+__global__ void sort_export_kernel(int64_t n, const uint32_t *__restrict__ keys,
+                                   const uint2 *__restrict__ pay, int64_t *sorted_keys,
+                                   int64_t *perm) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        sorted_keys[i] = keys[i];
+        perm[i] = pay[i].x;
+    }
+}
+
+// ------------------------------------------------------------------ host side -------------
+
+struct GenWs {
+    uint32_t *key[2];
+    uint2 *pay[2];
+    float *ls;
+    uint32_t *counts;
+    int *ticket;       // ticket + status words: zeroed before each look-back kernel
+    uint64_t *status;
+    size_t zero_bytes;
+    size_t total;
+};
+
+static int64_t sort_tiles(int64_t n) { return (n + SORT_TILE - 1) / SORT_TILE; }
+static int64_t seg_tiles(int64_t n) { return (n + SEG_TILE - 1) / SEG_TILE; }
+
+static GenWs gen_carve(void *ws, int64_t n) {
+    GenWs g;
+    const size_t nn = (size_t)(n < 1 ? 1 : n);
+    char *p = static_cast<char *>(ws);
+    auto take = [&](size_t bytes) { char *r = p; p += align_up(bytes, 256); return r; };
+    g.key[0] = reinterpret_cast<uint32_t *>(take(nn * 4));
+    g.key[1] = reinterpret_cast<uint32_t *>(take(nn * 4));
+    g.pay[0] = reinterpret_cast<uint2 *>(take(nn * 8));
+    g.pay[1] = reinterpret_cast<uint2 *>(take(nn * 8));
+    g.ls = reinterpret_cast<float *>(take(nn * 4));
+    const size_t m = (size_t)SORT_MAX_RADIX * (size_t)sort_tiles(nn);
+    g.counts = reinterpret_cast<uint32_t *>(take(m * 4));
+    size_t lb_tiles = (m + US_NT * US_IPT - 1) / (US_NT * US_IPT);
+    if ((size_t)seg_tiles(nn) > lb_tiles) lb_tiles = (size_t)seg_tiles(nn);
+    g.zero_bytes = align_up(8 + 8 * lb_tiles, 256);
+    char *z = take(g.zero_bytes);
+    g.ticket = reinterpret_cast<int *>(z);
+    g.status = reinterpret_cast<uint64_t *>(z + 8);
+    g.total = (size_t)(p - static_cast<char *>(ws));
+    return g;
+}
+
+size_t rbi_general_workspace_bytes(int64_t n, int64_t) { return gen_carve(nullptr, n).total; }
+
+// Sorts (clamped key, (index, value)); returns the buffer index holding the result in *out_buf.
+static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, const GenWs &g,
+                    int *out_buf, cudaStream_t stream) {
+    int bits = 0;
+    while (bits < 32 && ((uint64_t)w >> bits) != 0) bits++;  // keys are 0..w
+    if (bits < 1) bits = 1;
+    if (bits > 32) return VJP_ERR_UNSUPPORTED;
+    const int passes = (bits + 7) / 8;
+    const int per = (bits + passes - 1) / passes;
+    const int nt = (int)sort_tiles(n);
+    int shift = 0, src = -1;
+    for (int ps = 0; ps < passes; ps++) {
+        const int b = (bits - shift) < per ? (bits - shift) : per;
+        const int radix = 1 << b;
+        const int dst = ps & 1;
+        const int64_t m = (int64_t)radix * nt;
+        if (ps == 0)
+            sort_hist_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, nullptr, shift, radix, nt, g.counts);
+        else
+            sort_hist_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, g.key[src], shift, radix, nt, g.counts);
+        if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+        const int sb = (int)((m + US_NT * US_IPT - 1) / (US_NT * US_IPT));
+        u32_exclusive_scan_kernel<<<sb, US_NT, 0, stream>>>(g.counts, m, g.ticket, g.status);
+        if (ps == 0)
+            sort_scatter_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, vs, nullptr, nullptr, shift, radix,
+                                                                  nt, g.counts, g.key[dst], g.pay[dst]);
+        else
+            sort_scatter_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, nullptr, g.key[src],
+                                                                   g.pay[src], shift, radix, nt, g.counts,
+                                                                   g.key[dst], g.pay[dst]);
+        src = dst;
+        shift += b;
+    }
+    *out_buf = src;
+    return last_launch_status();
+}
+
+template <int CODE>
+static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                       const float *hist_bar, float *vs_bar, const GenWs &g, cudaStream_t stream) {
+    int buf;
+    int rc = run_sort(n, w, is, vs, g, &buf, stream);
+    if (rc != VJP_OK) return rc;
+    using KS = Stage<SEG_NT, SEG_IPT>;
+    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
+    const GenOp<CODE> op{S};
+    const int nt = (int)seg_tiles(n);
+    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    seg_forward_kernel<CODE><<<nt, SEG_NT, KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+        n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
+    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, 2 * KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+        n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status);
+    return last_launch_status();
+}
+
+int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
+                           const float *vs, const float *hist_bar, float *vs_bar, void *ws,
+                           cudaStream_t stream) {
+    if (n == 0) return VJP_OK;
+    const GenWs g = gen_carve(ws, n);
+    const float S = (float)param;
+    switch (code) {
+    case VJP_OP_ADD: return run_general<G_ADD>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    case VJP_OP_MIN: return run_general<G_MIN>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    case VJP_OP_MAX: return run_general<G_MAX>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    case VJP_OP_MUL: return run_general<G_MUL>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    case VJP_OP_SATADD: return run_general<G_SATADD>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    default: return VJP_ERR_UNSUPPORTED;
+    }
+}
+
+int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
+                         int64_t *perm, void *ws, cudaStream_t stream) {
+    if (n == 0) return VJP_OK;
+    const GenWs g = gen_carve(ws, n);
+    int buf;
+    int rc = run_sort(n, w, is, nullptr, g, &buf, stream);
+    if (rc != VJP_OK) return rc;
+    const int grid = (int)((n + 255) / 256 < 2368 ? (n + 255) / 256 : 2368);
+    sort_export_kernel<<<grid, 256, 0, stream>>>(n, g.key[buf], g.pay[buf], sorted_keys, perm);
+    return last_launch_status();
+}
+
+}  // namespace vjp

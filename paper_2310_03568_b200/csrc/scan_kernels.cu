@@ -1,0 +1,384 @@
+// scan_kernels.cu -- single-pass decoupled-look-back scans (forward and reverse) and the fused
+// reverse kernel of the scan VJP.
+//
+//   scan_lookback_kernel<Op, NT, IPT, REV, MODE>
+//       MODE_SCAN    : out[i] = fold of in[0..i] (REV: of in[i..n-1]) -- the primal inclusive scan
+//                       and, with Op = '+' and REV, the '+' rule of the scan VJP
+//                      (xs_bar = reverse inclusive sum of ys_bar).
+//       MODE_TILEPRE : only the exclusive prefix of every tile is written (fpre[t] = fold of all
+//                      elements before tile t): the forward re-execution the return sweep needs
+//                      (r_{i-1} of P:L613; re-execution instead of a tape).
+//   scan_vjp_reverse_kernel<Op, NT, IPT>
+//       the general rule of Fig. 7 in one kernel: Jacobians formed on the fly
+//       (never stored), reverse linear-recurrence scan with lin_o
+//        in its redundant-block-diagonal form, final map.
+//
+// Tile = NT threads x IPT consecutive elements per thread, staged through shared memory with
+// 128-bit coalesced global accesses.  A tile's processing index comes from an atomic ticket.
+#include "internal.h"
+#include "scan_ops.cuh"
+
+namespace vjp {
+
+enum : int { MODE_SCAN = 0, MODE_TILEPRE = 1 };
+
+template <class S>
+struct LookbackWs {
+    int *ticket;
+    TileStatus<S> st;
+};
+
+constexpr size_t WS_ALIGN = 256;
+
+template <class S>
+static size_t lookback_bytes(int64_t num_tiles) {
+    return align_up(sizeof(int) * (size_t)(num_tiles + 1), WS_ALIGN) +
+           2 * align_up(sizeof(S) * (size_t)num_tiles, WS_ALIGN);
+}
+// Carves ticket + flags (contiguous: one memset) and the two payload arrays out of `base`.
+template <class S>
+static LookbackWs<S> lookback_carve(char *base, int64_t num_tiles, size_t *zero_bytes) {
+    LookbackWs<S> w;
+    w.ticket = reinterpret_cast<int *>(base);
+    w.st.flags = w.ticket + 1;
+    *zero_bytes = align_up(sizeof(int) * (size_t)(num_tiles + 1), WS_ALIGN);
+    char *p = base + *zero_bytes;
+    w.st.agg = reinterpret_cast<S *>(p);
+    p += align_up(sizeof(S) * (size_t)num_tiles, WS_ALIGN);
+    w.st.incl = reinterpret_cast<S *>(p);
+    return w;
+}
+
+// Warp 0 of the block: publish the tile aggregate, look back, publish the inclusive prefix.
+// Returns (in every lane of warp 0) the fold of all tiles processed before tile p.
+template <class M>
+VJP_DEVINL typename M::State tile_prefix_warp0(const TileStatus<typename M::State> &st, int p,
+                                               const typename M::State &total) {
+    using S = typename M::State;
+    const int lane = threadIdx.x & 31;
+    if (p == 0) {
+        if (lane == 0) publish_tile(st, 0, total, true);
+        return M::identity();
+    }
+    if (lane == 0) publish_tile(st, p, total, false);
+    S pre = lookback_warp<M>(
+        st.flags, p, [&](int q) { return load_state_cg(st.agg + q); },
+        [&](int q) { return load_state_cg(st.incl + q); });
+    if (lane == 0) publish_tile(st, p, M::combine(pre, total), true);
+    return pre;
+}
+
+template <class Op, int NT, int IPT, bool REV, int MODE>
+__global__ void __launch_bounds__(NT)
+scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int64_t n,
+                     int num_tiles, LookbackWs<typename Op::Fwd> ws,
+                     typename Op::Fwd *__restrict__ fpre) {
+    using M = FwdMonoid<Op>;
+    using S = typename Op::Fwd;
+    constexpr int EW = Op::EW, RW = IPT * EW, SW = sizeof(S) / 4;
+    using St = Stage<NT, RW>;
+    using BS = BlockScan<M, NT>;
+    extern __shared__ uint4 smem[];
+    uint32_t *scratch = reinterpret_cast<uint32_t *>(smem + St::SMEM_BYTES / 16);
+    uint32_t *bcast = scratch + BS::SMEM_WORDS;
+    __shared__ int s_p;
+
+    if (threadIdx.x == 0) s_p = atomicAdd(ws.ticket, 1);
+    __syncthreads();
+    const int p = s_p;
+    const int t = REV ? num_tiles - 1 - p : p;
+    const int64_t base = (int64_t)t * (NT * IPT);
+    const int valid = (int)min((int64_t)(NT * IPT), n - base);
+
+    uint32_t fill[EW];
+    Op::identity_words(fill);
+    St::load(smem, in + base * EW, valid * EW, fill);
+    __syncthreads();
+    uint32_t r[RW];
+    St::read_row(smem, threadIdx.x, r);
+
+    // thread-local fold in processing order
+    S acc;
+    if (!REV) {
+        acc = Op::from_elem(r);
+#pragma unroll
+        for (int j = 1; j < IPT; j++) acc = Op::combine(acc, Op::from_elem(r + j * EW));
+    } else {
+        acc = Op::from_elem(r + (IPT - 1) * EW);
+#pragma unroll
+        for (int j = IPT - 2; j >= 0; j--) acc = Op::combine(Op::from_elem(r + j * EW), acc);
+    }
+    S total;
+    S ex = BS::template exclusive<REV>(acc, total, scratch);
+
+    if (threadIdx.x < 32) {
+        S pre = tile_prefix_warp0<M>(ws.st, p, total);
+        if (threadIdx.x == 0) store_state_smem(bcast, pre);
+    }
+    __syncthreads();
+    const S pre = load_state_smem<S>(bcast);
+
+    if (MODE == MODE_TILEPRE) {
+        if (threadIdx.x == 0) store_state_cg(fpre + t, pre);
+        return;
+    }
+    // REV is only instantiated for commutative operators ('+'): operand order is immaterial there
+    S run = Op::combine(pre, ex);
+    if (!REV) {
+#pragma unroll
+        for (int j = 0; j < IPT; j++) {
+            run = Op::combine(run, Op::from_elem(r + j * EW));
+            Op::to_elem(run, r + j * EW);
+        }
+    } else {
+#pragma unroll
+        for (int j = IPT - 1; j >= 0; j--) {
+            run = Op::combine(Op::from_elem(r + j * EW), run);
+            Op::to_elem(run, r + j * EW);
+        }
+    }
+    St::write_row(smem, threadIdx.x, r);
+    __syncthreads();
+    St::store(smem, out + base * EW, valid * EW);
+}
+
+// The fused reverse kernel of the scan VJP.  With u_i = rbar_i * X_i^T ("what element i hands to
+// element i-1", see scan_ops.cuh) the return sweep of P:L553-558 reads
+//     rbar_i = ybar_i + u_{i+1},   xbar_i = (d(r_{i-1} (.) x_i)/dx_i)^T rbar_i,   u_n = 0,
+// and element i acts on the incoming u as the affine map z -> (ybar_i + z) * X_i^T.
+template <class Op, int NT, int IPT>
+__global__ void __launch_bounds__(NT)
+scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
+                        uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
+                        const typename Op::Fwd *__restrict__ fpre,
+                        LookbackWs<typename RevMonoid<Op>::State> ws) {
+    using RM = RevMonoid<Op>;
+    using RS = typename RM::State;
+    using FM = FwdMonoid<Op>;
+    using FS = typename Op::Fwd;
+    using Adj = typename Op::Adj;
+    constexpr int EW = Op::EW, RW = IPT * EW;
+    using St = Stage<NT, RW>;
+    using RBS = BlockScan<RM, NT>;
+    using FBS = BlockScan<FM, NT>;
+    constexpr int SCR = RBS::SMEM_WORDS > FBS::SMEM_WORDS ? RBS::SMEM_WORDS : FBS::SMEM_WORDS;
+    extern __shared__ uint4 smem[];
+    uint4 *sx = smem;
+    uint4 *sy = smem + St::SMEM_BYTES / 16;
+    uint32_t *scratch = reinterpret_cast<uint32_t *>(sy + St::SMEM_BYTES / 16);
+    uint32_t *bcast = scratch + SCR;
+    __shared__ int s_p;
+
+    if (threadIdx.x == 0) s_p = atomicAdd(ws.ticket, 1);
+    __syncthreads();
+    const int p = s_p;
+    const int t = num_tiles - 1 - p;
+    const int64_t base = (int64_t)t * (NT * IPT);
+    const int valid = (int)min((int64_t)(NT * IPT), n - base);
+
+    uint32_t fillx[EW];
+    Op::identity_words(fillx);  // identity element: u passes through unchanged
+    const uint32_t filly[1] = {0u};
+    St::load(sx, xs + base * EW, valid * EW, fillx);
+    St::load(sy, ybar + base * EW, valid * EW, filly);
+    __syncthreads();
+    uint32_t rx[RW], ry[RW];
+    St::read_row(sx, threadIdx.x, rx);
+    St::read_row(sy, threadIdx.x, ry);
+
+    // thread-local reduce, walking the thread's elements from the highest index down
+    Adj bacc = Op::adj_zero();
+    FS facc = Op::identity();
+#pragma unroll
+    for (int j = IPT - 1; j >= 0; j--) {
+        const FS xj = Op::from_elem(rx + j * EW);
+        bacc = Op::adj_mul(Op::adj_add(Op::adj_from_elem(ry + j * EW), bacc), Op::lin_of(xj));
+        facc = Op::combine(xj, facc);
+    }
+    RS racc;
+    racc.b = bacc;
+    racc.l = Op::lin_of(facc);  // forward product of the thread's range: the c of lin_o, transposed
+    RS rtotal;
+    const RS rex = RBS::template exclusive<true>(racc, rtotal, scratch);
+    FS ftotal;
+    const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+
+    if (threadIdx.x < 32) {
+        RS pre = tile_prefix_warp0<RM>(ws.st, p, rtotal);
+        if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
+    }
+    __syncthreads();
+    const Adj ztile = load_state_smem<Adj>(bcast);  // u entering the tile from the right
+
+    // forward prefixes r_{i-1} of the thread's elements
+    FS rp[IPT];
+    rp[0] = Op::combine(load_state_cg(fpre + t), fex);
+#pragma unroll
+    for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
+
+    Adj u = Op::adj_add(rex.b, Op::adj_mul(ztile, rex.l));
+#pragma unroll
+    for (int j = IPT - 1; j >= 0; j--) {
+        const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);
+        u = Op::adj_mul(rbar, Op::lin_of(Op::from_elem(rx + j * EW)));
+        Op::xbar(rp[j], rbar, ry + j * EW);
+    }
+    St::write_row(sy, threadIdx.x, ry);
+    __syncthreads();
+    St::store(sy, xbar + base * EW, valid * EW);
+}
+
+// ------------------------------------------------------------------ host side ------------
+
+template <class Op, int NT_, int IPT_, int VNT_, int VIPT_>
+struct ScanCfg {
+    using op = Op;
+    static constexpr int NT = NT_, IPT = IPT_;     // plain scans
+    static constexpr int VNT = VNT_, VIPT = VIPT_; // VJP: forward tile prefixes + fused reverse
+};
+
+template <class Op, int NT, int IPT>
+static size_t scan_smem_bytes() {
+    using St = Stage<NT, IPT * Op::EW>;
+    using BS = BlockScan<FwdMonoid<Op>, NT>;
+    return St::SMEM_BYTES + (BS::SMEM_WORDS + sizeof(typename Op::Fwd) / 4) * 4;
+}
+template <class Op, int NT, int IPT>
+static size_t vjp_smem_bytes() {
+    using St = Stage<NT, IPT * Op::EW>;
+    using RBS = BlockScan<RevMonoid<Op>, NT>;
+    using FBS = BlockScan<FwdMonoid<Op>, NT>;
+    constexpr int SCR = RBS::SMEM_WORDS > FBS::SMEM_WORDS ? RBS::SMEM_WORDS : FBS::SMEM_WORDS;
+    return 2 * St::SMEM_BYTES + (SCR + sizeof(typename Op::Adj) / 4) * 4;
+}
+
+static int64_t tiles_of(int64_t n, int tile) { return (n + tile - 1) / tile; }
+
+template <class Op, int NT, int IPT, bool REV, int MODE>
+static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre, char *ws,
+                    cudaStream_t stream) {
+    using S = typename Op::Fwd;
+    const int64_t nt = tiles_of(n, NT * IPT);
+    size_t zero_bytes;
+    LookbackWs<S> lw = lookback_carve<S>(ws, nt, &zero_bytes);
+    if (cudaMemsetAsync(ws, 0, zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    auto kern = scan_lookback_kernel<Op, NT, IPT, REV, MODE>;
+    const size_t smem = scan_smem_bytes<Op, NT, IPT>();
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(in),
+                                             static_cast<uint32_t *>(out), n, (int)nt, lw, fpre);
+    return last_launch_status();
+}
+
+template <class Cfg>
+static size_t ws_bytes_cfg(int64_t n) {
+    using Op = typename Cfg::op;
+    const int64_t nt = tiles_of(n, Cfg::NT * Cfg::IPT);
+    return lookback_bytes<typename Op::Fwd>(nt);
+}
+template <class Cfg>
+static size_t ws_bytes_vjp_cfg(int64_t n) {
+    using Op = typename Cfg::op;
+    const int64_t nt = tiles_of(n, Cfg::VNT * Cfg::VIPT);
+    return lookback_bytes<typename Op::Fwd>(nt) +
+           lookback_bytes<typename RevMonoid<Op>::State>(nt) +
+           align_up(sizeof(typename Op::Fwd) * (size_t)nt, WS_ALIGN);
+}
+
+template <class Cfg>
+static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, char *ws,
+                   cudaStream_t stream) {
+    using Op = typename Cfg::op;
+    using FS = typename Op::Fwd;
+    using RS = typename RevMonoid<Op>::State;
+    constexpr int NT = Cfg::VNT, IPT = Cfg::VIPT;
+    const int64_t nt = tiles_of(n, NT * IPT);
+    char *ws_fwd = ws;
+    char *ws_rev = ws_fwd + lookback_bytes<FS>(nt);
+    FS *fpre = reinterpret_cast<FS *>(ws_rev + lookback_bytes<RS>(nt));
+    // (A) forward tile prefixes
+    int rc = run_scan<Op, NT, IPT, false, MODE_TILEPRE>(n, xs, nullptr, fpre, ws_fwd, stream);
+    if (rc != VJP_OK) return rc;
+    // (B) fused reverse kernel
+    size_t zero_bytes;
+    LookbackWs<RS> lw = lookback_carve<RS>(ws_rev, nt, &zero_bytes);
+    if (cudaMemsetAsync(ws_rev, 0, zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    auto kern = scan_vjp_reverse_kernel<Op, NT, IPT>;
+    const size_t smem = vjp_smem_bytes<Op, NT, IPT>();
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(xs),
+                                             static_cast<const uint32_t *>(ys_bar),
+                                             static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw);
+    return last_launch_status();
+}
+
+// tile shapes: rows of 16 words (plain scans) / 8 words (VJP: two staged arrays + more live state)
+using CfgAddF32 = ScanCfg<OpAdd<float>, 256, 16, 256, 16>;
+using CfgAddF64 = ScanCfg<OpAdd<double>, 256, 8, 256, 8>;
+using CfgMulF32 = ScanCfg<OpMul<float>, 256, 16, 256, 8>;
+using CfgMulF64 = ScanCfg<OpMul<double>, 256, 8, 256, 4>;
+using CfgLinRec = ScanCfg<OpLinRec<float>, 256, 8, 256, 4>;
+using CfgMat2 = ScanCfg<OpMatMul<2, float, double, double>, 256, 4, 256, 2>;
+using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 1, 128, 1>;
+
+#define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
+    switch (code) {                                                                          \
+    case VJP_OP_ADD: if (dtype == VJP_F32) { F(CfgAddF32) } else { F(CfgAddF64) } break;     \
+    case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;     \
+    case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } else { FAIL } break;          \
+    case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } else { FAIL } break;           \
+    case VJP_OP_MATMUL5: if (dtype == VJP_F32) { F(CfgMat5) } else { FAIL } break;           \
+    default: FAIL                                                                            \
+    }
+
+size_t scan_workspace_bytes(int code, int dtype, int64_t n) {
+    if (n <= 0) return WS_ALIGN;
+    if (code == VJP_OP_ADD)
+        return dtype == VJP_F32 ? ws_bytes_cfg<CfgAddF32>(n) : ws_bytes_cfg<CfgAddF64>(n);
+    size_t a = 0, b = 0;
+#define F(C) a = ws_bytes_cfg<C>(n); b = ws_bytes_vjp_cfg<C>(n);
+    switch (code) {
+    case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
+    case VJP_OP_LINREC: F(CfgLinRec) break;
+    case VJP_OP_MATMUL2: F(CfgMat2) break;
+    case VJP_OP_MATMUL5: F(CfgMat5) break;
+    default: return 0;
+    }
+#undef F
+    return a > b ? a : b;
+}
+
+int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,
+                        cudaStream_t stream) {
+#define F(C) return run_scan<typename C::op, C::NT, C::IPT, false, MODE_SCAN>(n, xs, ys, nullptr, (char *)ws, stream);
+    VJP_SCAN_DISPATCH(code, dtype, F, return VJP_ERR_UNSUPPORTED;)
+#undef F
+    return VJP_ERR_UNSUPPORTED;
+}
+
+int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *ys_bar,
+                    void *xs_bar, void *ws, cudaStream_t stream) {
+    if (code == VJP_OP_ADD) {  // reverse inclusive sum of ys_bar
+        if (dtype == VJP_F32)
+            return run_scan<OpAdd<float>, CfgAddF32::NT, CfgAddF32::IPT, true, MODE_SCAN>(
+                n, ys_bar, xs_bar, nullptr, (char *)ws, stream);
+        return run_scan<OpAdd<double>, CfgAddF64::NT, CfgAddF64::IPT, true, MODE_SCAN>(
+            n, ys_bar, xs_bar, nullptr, (char *)ws, stream);
+    }
+#define F(C) return run_vjp<C>(n, xs, ys_bar, xs_bar, (char *)ws, stream);
+    switch (code) {
+    case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
+    case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } break;
+    case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } break;
+    case VJP_OP_MATMUL5: if (dtype == VJP_F32) { F(CfgMat5) } break;
+    default: break;
+    }
+#undef F
+    return VJP_ERR_UNSUPPORTED;
+}
+
+}  // namespace vjp

@@ -1,0 +1,294 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the f64 CPU oracle, element by
+element on the same seeded inputs.  Sizes span several tiles and a ragged tail for every tile shape
+in use (128 ... 4096 elements) and the edge cases n = 1, 2, tile-1, tile, tile+1.
+
+Bars (BASELINE.json north_star): bit-exact for indices, argmins, zero counts, permutations and for
+the pure copies ('+' gather, min/max scatter); normwise relative error ||d||inf / ||ref||inf
+<= 1e-4 for f32 and <= 1e-10 for f64 (when ||ref||inf = 0 the result must be exactly 0)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2310_03568_b200 import binding as B
+from paper_2310_03568_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float32: 1e-4, torch.float64: 1e-10}
+SIZES = [1, 2, 33, 127, 128, 129, 511, 513, 1023, 1025, 2047, 2049, 4095, 4096, 4097, 12345, 100003]
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def nrel(got, ref):
+    got = np.asarray(got, dtype=np.float64).ravel()
+    ref = np.asarray(ref, dtype=np.float64).ravel()
+    assert got.shape == ref.shape
+    if got.size == 0:
+        return 0.0
+    assert np.all(np.isfinite(got)), "non-finite values in the GPU result"
+    den = np.max(np.abs(ref))
+    err = np.max(np.abs(got - ref))
+    if den == 0.0:
+        return 0.0 if err == 0.0 else np.inf
+    return err / den
+
+
+# ------------------------------------------------------------------------------ scans ----
+
+def scan_inputs(name, n, seed=0):
+    if name == "add_f32":
+        d = W.c3_scan_add(n=n, seed=seed)
+        return B.Op.of("add"), "add", 0, d["xs"], d["ys_bar"]
+    if name == "add_f64":
+        d = W.c3_scan_add(n=n, seed=seed, dtype=np.float64)
+        return B.Op.of("add", torch.float64), "add", 0, d["xs"], d["ys_bar"]
+    if name == "mul_f64":
+        d = W.c3_scan_mul(n=n, seed=seed, zero_rate=1e-3 if n > 5000 else 0.02)
+        return B.Op.of("mul", torch.float64), "mul", 0, d["xs"], d["ys_bar"]
+    if name == "mul_f64_nozero":
+        d = W.c3_scan_mul(n=n, seed=seed, zero_rate=0.0, lo=0.999, hi=1.001)
+        return B.Op.of("mul", torch.float64), "mul", 0, d["xs"], d["ys_bar"]
+    if name == "mul_f32":
+        d = W.c3_scan_mul(n=n, seed=seed, dtype=np.float32, zero_rate=0.0, lo=0.999, hi=1.001)
+        return B.Op.of("mul"), "mul", 0, d["xs"], d["ys_bar"]
+    if name == "linrec":
+        d = W.c3_scan_linrec(n=n, seed=seed)
+        return B.Op.of("linrec"), "linrec", 0, d["xs"], d["ys_bar"]
+    if name in ("matmul2", "matmul5"):
+        q = int(name[-1])
+        d = W.c4_scan_matmul(q, n=n, seed=seed)
+        return B.Op.of(name), "matmul", q, d["xs"], d["ys_bar"]
+    raise ValueError(name)
+
+
+SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "linrec", "matmul2", "matmul5"]
+
+
+@pytest.mark.parametrize("n", SIZES)
+@pytest.mark.parametrize("name", SCAN_OPS)
+def test_scan_vjp_matches_oracle(name, n):
+    op, oname, q, xs, ys_bar = scan_inputs(name, n)
+    got = B.vjp_scan(op, dev(xs), dev(ys_bar)).cpu().numpy()
+    ref = oracle.vjp_scan(oname, xs, ys_bar, q=q)
+    assert nrel(got, ref) <= TOL[op.torch_dtype]
+
+
+@pytest.mark.parametrize("n", [1, 129, 4097, 100003])
+@pytest.mark.parametrize("name", SCAN_OPS)
+def test_scan_forward_matches_oracle(name, n):
+    op, oname, q, xs, _ = scan_inputs(name, n)
+    got = B.scan_forward(op, dev(xs)).cpu().numpy()
+    ref = oracle.scan_forward(oname, xs, q=q)
+    if oname == "linrec":  # the A component underflows: compare the two components separately
+        got, ref = got.reshape(-1, 2)[:, 1], ref.reshape(-1, 2)[:, 1]
+    assert nrel(got, ref) <= TOL[op.torch_dtype]
+
+
+def test_scan_add_vjp_needs_no_xs_and_repeats_bit_exactly():
+    d = W.c3_scan_add(n=300001, seed=3)
+    op = B.Op.of("add")
+    yb = dev(d["ys_bar"])
+    a = B.vjp_scan(op, None, yb)
+    ref = oracle.vjp_scan("add", d["xs"], d["ys_bar"])
+    assert nrel(a.cpu().numpy(), ref) <= 1e-4
+    for _ in range(3):  # tile order varies from run to run; the association order may, the bar may not
+        b = B.vjp_scan(op, None, yb)
+        assert nrel(b.cpu().numpy(), ref) <= 1e-4
+
+
+def test_scan_mul_zeros_at_the_ends_and_everywhere():
+    op = B.Op.of("mul", torch.float64)
+    rng = np.random.default_rng(5)
+    for n in (5, 1000, 5000):
+        for pattern in ("first", "last", "all", "alternate"):
+            xs = 0.5 + rng.random(n)
+            if pattern == "first":
+                xs[0] = 0.0
+            elif pattern == "last":
+                xs[-1] = 0.0
+            elif pattern == "all":
+                xs[:] = 0.0
+            else:
+                xs[::2] = 0.0
+            yb = rng.standard_normal(n)
+            got = B.vjp_scan(op, dev(xs), dev(yb)).cpu().numpy()
+            assert nrel(got, oracle.vjp_scan("mul", xs, yb)) <= 1e-10
+
+
+def test_scan_rejects_bad_arguments():
+    op = B.Op.of("satadd")
+    x = torch.zeros(8, device="cuda")
+    with pytest.raises(B.VjpError):
+        B.vjp_scan(op, x, x)
+    with pytest.raises(B.VjpError):
+        B.vjp_scan(B.Op.of("mul"), None, x)  # xs is required unless op is '+'
+    with pytest.raises(B.VjpError):
+        B.vjp_scan(B.Op.of("add"), None, x, ws=torch.empty(8, dtype=torch.uint8, device="cuda"))
+    assert B.vjp_scan(B.Op.of("add"), None, x[:0]).numel() == 0
+
+
+# ------------------------------------------------------------------- reduce-by-index -----
+
+RBI_SHAPES = [(1, 1), (5, 3), (1000, 1), (4097, 7), (100003, 1024), (100003, 20000), (1 << 18, 70000)]
+
+
+def keys_with_oob(rng, n, w):
+    return rng.integers(-max(1, w // 16), w + max(1, w // 16), size=n, dtype=np.int64)
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+def test_rbi_add_vjp_is_a_bit_exact_gather(n, w, dtype):
+    rng = np.random.default_rng([n, w])
+    is_ = keys_with_oob(rng, n, w)
+    npdt = np.float32 if dtype == torch.float32 else np.float64
+    hb = rng.standard_normal(w).astype(npdt)
+    got = B.vjp_reduce_by_index(B.Op.of("add", dtype), w, dev(is_), None, dev(hb)).cpu().numpy()
+    ref = oracle.vjp_rbi_add(w, is_, hb)
+    assert np.array_equal(got.astype(np.float64), ref)
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+@pytest.mark.parametrize("opname", ["add", "min", "max", "mul", "satadd"])
+def test_rbi_forward_matches_oracle(opname, n, w):
+    rng = np.random.default_rng([n, w, 1])
+    is_ = keys_with_oob(rng, n, w)
+    if opname == "mul":
+        vs = (0.9 + 0.2 * rng.random(n)).astype(np.float32)
+    elif opname == "satadd":
+        vs = rng.random(n, dtype=np.float32)
+    else:
+        vs = rng.standard_normal(n, dtype=np.float32)
+    S = max(1.0, 0.5 * n / w) + 0.123
+    got = B.reduce_by_index_forward(B.Op.of(opname, S=S), w, dev(is_), dev(vs)).cpu().numpy()
+    ref = oracle.reduce_by_index_forward(opname, w, is_, vs, S=S)
+    if opname in ("min", "max"):
+        assert np.array_equal(got.astype(np.float64), ref)
+    else:
+        fin = np.isfinite(ref)
+        assert np.array_equal(np.isfinite(got), fin)
+        assert nrel(got[fin], ref[fin]) <= 1e-4
+
+
+def minmax_inputs(n, w, dist, seed=0):
+    d = W.c2_rbi_min(n=n, w=w, dist=dist, seed=seed)
+    return d["is_"], d["vs"], d["hist_bar"]
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+@pytest.mark.parametrize("dist", ["uniform", "zipf"])
+@pytest.mark.parametrize("opname", ["min", "max"])
+def test_rbi_minmax_vjp_bit_exact(opname, dist, n, w):
+    is_, vs, hb = minmax_inputs(n, w, dist)
+    if opname == "max":
+        vs = -vs
+    is_ = is_.copy()
+    is_[::97] = -1 - (is_[::97] % 5)  # some out-of-range keys, negative included
+    is_[5::101] = w + is_[5::101] % 3
+    op = B.Op.of(opname)
+    arg, ext = B.rbi_argext(op, w, dev(is_), dev(vs))
+    got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+    ref, rarg, rext = oracle.vjp_rbi_minmax(opname, w, is_, vs, hb)
+    assert np.array_equal(arg.cpu().numpy(), rarg)
+    assert np.array_equal(ext.cpu().numpy().astype(np.float64), rext)
+    assert np.array_equal(got.astype(np.float64), ref)
+
+
+def test_rbi_min_signed_zero_is_a_tie_and_infinities_are_values():
+    # -0.0 == +0.0 under the paper's "<" (Q6): the lower index wins whatever the sign bit
+    is_ = np.array([0, 0, 1, 1, 2, 2, 2], dtype=np.int64)
+    vs = np.array([0.0, -0.0, -0.0, 0.0, np.inf, np.inf, -np.inf], dtype=np.float32)
+    hb = np.array([1.0, 2.0, 3.0, 4.0], dtype=np.float32)
+    for opname in ("min", "max"):
+        op = B.Op.of(opname)
+        arg, _ = B.rbi_argext(op, 4, dev(is_), dev(vs))
+        _, rarg, _ = oracle.vjp_rbi_minmax(opname, 4, is_, vs, hb)
+        assert arg.cpu().numpy().tolist() == rarg.tolist()
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+@pytest.mark.parametrize("dist", ["uniform", "zipf"])
+def test_rbi_mul_vjp(dist, n, w):
+    # zero rate chosen so that bins with 0, 1 and >= 2 zeros all occur
+    d = W.c2_rbi_mul(n=n, w=w, dist=dist, zero_rate=min(0.3, 0.7 * w / n))
+    is_, vs, hb = d["is_"].copy(), d["vs"], d["hist_bar"]
+    is_[::89] = -3
+    op = B.Op.of("mul")
+    zeros, prod = B.rbi_zero_prod(op, w, dev(is_), dev(vs))
+    got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+    ref, rz, rp = oracle.vjp_rbi_mul(w, is_, vs, hb)
+    assert np.array_equal(zeros.cpu().numpy(), rz)
+    gp = prod.cpu().numpy().astype(np.float64)
+    ok = rp > 1e-30  # hot Zipf bins underflow; compare the representable ones element-wise
+    assert np.all(np.abs(gp[ok] - rp[ok]) <= 1e-4 * np.abs(rp[ok]))
+    assert nrel(got, ref) <= 1e-4
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+def test_rbi_sort_perm_bit_exact(n, w):
+    rng = np.random.default_rng([n, w, 2])
+    is_ = keys_with_oob(rng, n, w)
+    sk, perm = B.rbi_sort_perm(w, dev(is_))
+    rsk, rperm = oracle.rbi_sort_perm(w, is_)
+    assert np.array_equal(sk.cpu().numpy(), rsk)
+    assert np.array_equal(perm.cpu().numpy(), rperm)
+
+
+@pytest.mark.parametrize("n,w", RBI_SHAPES)
+def test_rbi_general_satadd(n, w):
+    d = W.c5_rbi_satadd(n=n, w=w)
+    is_ = d["is_"].copy()
+    is_[::53] = w + 2
+    # re-establish the margin around the kink after the keys changed
+    tot = np.bincount(is_[is_ < w], weights=d["vs"][is_ < w].astype(np.float64), minlength=w)
+    S = float(d["S"])
+    if np.any(np.abs(tot - S) < 2.0 ** -6):
+        S += 2.0 ** -4
+    assert not np.any(np.abs(tot - S) < 2.0 ** -7)
+    got = B.vjp_reduce_by_index(B.Op.of("satadd", S=S), w, dev(is_), dev(d["vs"]), dev(d["hist_bar"]))
+    ref = oracle.vjp_rbi_general("satadd", w, is_, d["vs"], d["hist_bar"], S=S)
+    assert np.array_equal(got.cpu().numpy().astype(np.float64), ref)  # every adjoint is a copy or 0
+
+
+@pytest.mark.parametrize("n,w", [(5, 3), (4097, 7), (100003, 1024), (100003, 20000)])
+@pytest.mark.parametrize("opname", ["add", "min", "max", "mul"])
+def test_general_rule_with_specialisable_operators(opname, n, w):
+    """the specialised rules are instances of eq. 5; force_general must agree."""
+    if opname == "mul":
+        d = W.c2_rbi_mul(n=n, w=w, zero_rate=min(0.3, 0.7 * w / n))
+    else:
+        d = W.c2_rbi_min(n=n, w=w)
+    is_, vs, hb = d["is_"], d["vs"], d["hist_bar"]
+    op = B.Op.of(opname, force_general=True)
+    got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+    ref = oracle.vjp_rbi_general(opname, w, is_, vs, hb)
+    if opname == "mul":
+        assert nrel(got, ref) <= 1e-4
+    else:
+        assert np.array_equal(got.astype(np.float64), ref)
+
+
+def test_rbi_rejects_bad_arguments_and_handles_empty_input():
+    is_ = torch.zeros(4, dtype=torch.int64, device="cuda")
+    v = torch.ones(4, device="cuda")
+    with pytest.raises(B.VjpError):
+        B.vjp_reduce_by_index(B.Op.of("linrec"), 2, is_, v, v[:2])
+    with pytest.raises(B.VjpError):
+        B.vjp_reduce_by_index(B.Op.of("min", torch.float64), 2, is_, v.double(), v[:2].double())
+    with pytest.raises(B.VjpError):
+        B.vjp_reduce_by_index(B.Op.of("mul"), 2, is_, None, v[:2])
+    for name in ("add", "min", "mul", "satadd"):
+        op = B.Op.of(name, S=1.0)
+        assert B.vjp_reduce_by_index(op, 2, is_[:0], v[:0], v[:2]).numel() == 0
+        h = B.reduce_by_index_forward(op, 3, is_[:0], v[:0]).cpu().numpy()
+        assert h.tolist() == [{"add": 0.0, "min": np.inf, "mul": 1.0, "satadd": 0.0}[name]] * 3
+    # every key out of range: all adjoints are exactly 0
+    bad = torch.full((1000,), -7, dtype=torch.int64, device="cuda")
+    vv = torch.rand(1000, device="cuda")
+    for name in ("add", "min", "max", "mul", "satadd"):
+        out = B.vjp_reduce_by_index(B.Op.of(name, S=1.0), 5, bad, vv, torch.ones(5, device="cuda"))
+        assert torch.count_nonzero(out).item() == 0
