@@ -1,0 +1,227 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the VJP hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--configs all|none]
+
+Workload (config.workload): BASELINE.json configs[1] -- reduce-by-index VJP, ops = min and '*', f32,
+n = 2^24, bins 2^10 and 2^16, keys uniform and Zipf(1.1): 8 cells.  One STEP = the VJP call of all 8
+cells on one batch of seeded synthetic input.  value = elements processed per second, whole job.
+The other four configs (and the primal timings for the AD overhead) are measured once per run on
+rank 0 at N = 1 and reported in "per_config"; they are not part of the timed steps.
+
+Multi-GPU: the path shards by independent problems (no data-path collective): every rank runs the
+same workload on its own seed; value = all ranks' elements / max-over-ranks time; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "vjp_throughput"
+UNIT = "Gelem/s"
+WORKLOAD = ("c2: reduce-by-index VJP, ops min and *, f32, n=2^24, w in {2^10, 2^16}, keys uniform and "
+            "Zipf(1.1) -- 8 cells per step")
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--configs", default="all", choices=["all", "none"],
+                    help="also measure every BASELINE config once (rank 0, N=1)")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink n (quick checks only; invalid as a result)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def log(msg):
+    sys.stderr.write("[bench %6.1fs] %s\n" % (time.time() - T0, msg))
+    sys.stderr.flush()
+
+
+T0 = time.time()
+
+
+def gen_cells(n, seed):
+    from paper_2310_03568_b200 import benchlib as L
+    return [L.gen_c2_cell(op, w, dist, n, seed=seed) for op, w, dist in L.C2_CELLS]
+
+
+# ------------------------------------------------------------------ reference arm (oracle) --
+
+def oracle_step(cells):
+    import oracle
+    for d in cells:
+        if d["op"] == "min":
+            oracle.vjp_rbi_minmax("min", d["w"], d["is_"], d["vs"], d["hist_bar"])
+        else:
+            oracle.vjp_rbi_mul(d["w"], d["is_"], d["vs"], d["hist_bar"])
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    n = max(1024, int((1 << 24) * args.scale))
+    cells = gen_cells(n, 0)
+    for _ in range(min(args.warmup, 1)):
+        oracle_step(cells)
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(cells)
+    dt = (time.perf_counter() - t) / args.steps
+    value = len(cells) * n / dt / 1e9
+    sample = "every step = the full workload (8 cells, n=%d each), oracle/vjp_oracle.c single-threaded f64" % n
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded numpy PCG64)",
+        "config": {"workload": WORKLOAD},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------ our arm ------------------
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2310_03568_b200 import benchlib as L
+    from paper_2310_03568_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.load()
+    peak, peak_kind = L.measured_peak()
+    n = max(1024, int((1 << 24) * args.scale))
+    if rank == 0:
+        log("generating the 8 cells of config 2 (n=%d)" % n)
+    cells = gen_cells(n, rank)
+    cases = [L.RbiCase(B.Op.of(d["op"]), d, with_host=True) for d in cells]
+    elems_per_step = sum(c.n for c in cases)
+
+    def step():
+        for c in cases:
+            c.vjp()
+
+    def step_host():
+        for c in cases:
+            c.vjp_host()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        """K steps between barrier+synchronize, device time by CUDA events, max over ranks (ms/step)."""
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        a.record()
+        for _ in range(steps):
+            fn()
+        b.record()
+        barrier()
+        ms = torch.tensor([a.elapsed_time(b) / steps], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = L.ClockSampler(local) if rank == 0 else None
+    l0 = B.launch_count()
+    ms_step = timed(step, args.steps)
+    launches = (B.launch_count() - l0) // args.steps
+    clocks = sampler.stop() if sampler else None
+    value = world * elems_per_step / (ms_step * 1e-3) / 1e9
+
+    # end to end: host buffers, H2D + kernels + D2H inside the timed region (the *_host entry points)
+    step_host()
+    ms_e2e = timed(step_host, args.steps)
+    e2e = {"value": world * elems_per_step / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
+           "h2d_bytes_per_step": sum(c.h2d_bytes() for c in cases),
+           "d2h_bytes_per_step": sum(c.d2h_bytes() for c in cases), "ms_per_step": ms_e2e}
+
+    # per-kernel durations of the same steps, CUDA events around every launch (library instrumentation)
+    psteps = min(args.steps, 5)
+    B.profile_enable(True)
+    for _ in range(psteps):
+        step()
+    torch.cuda.synchronize()
+    prof = B.profile_read()
+    B.profile_enable(False)
+    kernels, tot = [], sum(ms for ms, _ in prof.values())
+    for name, (ms, cnt) in sorted(prof.items(), key=lambda kv: -kv[1][0]):
+        bpe = L.kernel_bytes_per_elem(name)
+        avg = ms / cnt
+        kernels.append({"kernel": name, "launches_per_step": cnt // psteps, "avg_ms": round(avg, 4),
+                        "share_of_step": round(ms / tot, 3),
+                        "alg_gbs": round(bpe * n / (avg * 1e-3) / 1e9, 1) if bpe else None})
+    dom = kernels[0]
+    traffic = None
+    try:  # dram bytes per launch of the dominant kernel from the committed ncu capture, if there is one
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(dom["kernel"])
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["alg_gbs"], "peak": peak,
+                "peak_kind": peak_kind + " (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured" else "fallback",
+                "unit": "GB/s", "frac": round(dom["alg_gbs"] / peak, 3), "frac_of_8tbs": round(dom["alg_gbs"] / 8000.0, 3),
+                "alg_bytes_per_launch": L.kernel_bytes_per_elem(dom["kernel"]) * n, "traffic": traffic}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic (seeded numpy PCG64, recipe in DESIGN.md)",
+        "config": {"workload": WORKLOAD, "n": n, "cells": len(cases),
+                   "l2": "inputs larger than L2 (192 MB of keys+values per cell, 8 cells back to back)"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "kernels": kernels,
+    }
+    if rank == 0 and world == 1:
+        if args.configs == "all":
+            del cases, cells
+            torch.cuda.empty_cache()
+            line["per_config"] = L.measure_all_configs(reps=max(5, args.steps), peak_gbs=peak, scale=args.scale, log=log)
+        if not args.no_cpu_baseline:
+            log("cpu baseline (oracle)")
+            import oracle
+            oracle.build()
+            ocells = gen_cells(n, 0)
+            t = time.perf_counter()
+            oracle_step(ocells)
+            dt = time.perf_counter() - t
+            line["cpu_baseline"] = {"value": len(ocells) * n / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "host_cores": os.cpu_count(), "seconds": round(dt, 2),
+                                    "sample": "one full step (8 cells, n=%d each), oracle/vjp_oracle.c, single thread, f64" % n}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse()
+    sys.exit(run_reference(a) if a.impl == "reference" else run_ours(a))

@@ -156,6 +156,23 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
                   int64_t *perm, void *ws, size_t ws_bytes, void *stream);
 
+/* ------------------------------------------------------------------ instrumentation ----- */
+
+/* The library's kernels are numbered 0 .. vjp_kernel_count()-1; vjp_kernel_name gives the kernel's
+ * name (static storage; NULL if out of range).  vjp_launch_count(kid) is the number of launches of
+ * kernel kid since the library was loaded, kid < 0 the total over all kernels (cudaMemsetAsync
+ * calls are not kernels of this library and are not counted). */
+int vjp_kernel_count(void);
+const char *vjp_kernel_name(int kid);
+int64_t vjp_launch_count(int kid);
+
+/* While enabled, every kernel launch is bracketed by CUDA events on its stream (at most 8192
+ * launches are recorded; enabling clears the record).  vjp_profile_read synchronises on the
+ * recorded events and returns the summed duration and the number of recorded launches of kernel
+ * kid.  Not thread-safe; meant for bench.py's per-kernel roofline, off by default. */
+void vjp_profile_enable(int on);
+int vjp_profile_read(int kid, double *total_ms, int64_t *launches);
+
 #ifdef __cplusplus
 }
 #endif

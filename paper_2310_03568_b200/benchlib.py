@@ -1,0 +1,253 @@
+"""Measurement helpers for bench.py: CUDA-event timing, clock sampling, the algorithmic byte
+counts of SURVEY.md section 8(d) / DESIGN.md, and the per-config measurements (VJP time, primal
+time, AD overhead, achieved GB/s).  No arithmetic of the method and no oracle import here."""
+from __future__ import annotations
+
+import json
+import os
+import statistics
+import subprocess
+import threading
+
+import numpy as np
+import torch
+
+from . import binding as B
+from . import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+NORTH_STAR_PEAK_GBS = 8000.0   # "~8 TB/s" of BASELINE.json:north_star, reported beside the measured peak
+FALLBACK_PEAK_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def measured_peak():
+    """(GB/s, 'measured' | 'fallback') from MEASURED_PEAKS.json (driver-written)."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_PEAK_GBS, "fallback"
+
+
+# Algorithmic bytes per element of each kernel (what the method itself must move once; look-back
+# words, w-sized tables and L2-resident histograms excluded).  Keyed by the library's kernel name.
+def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
+    table = {
+        "rbi_vjp_add_kernel": 8 + elem_bytes,        # is + write vs_bar
+        "rbi_minmax_lifted_kernel": 8 + 4 + 4,       # is + vs + zero-fill of vs_bar
+        "rbi_mul_lifted_kernel": 8 + 4,              # is + vs (per pass over the input)
+        "rbi_mul_sweep_kernel": 8 + 4 + 4,           # is + vs + write vs_bar
+        "rbi_forward_kernel": 8 + elem_bytes,
+        "scan_lookback_kernel<MODE_SCAN>": 2 * elem_bytes,
+        "scan_lookback_kernel<MODE_TILEPRE>": elem_bytes,
+        "scan_vjp_reverse_kernel": 3 * elem_bytes,
+        "sort_hist_kernel": 8,                       # first pass reads int64 keys (4 on later passes)
+        "sort_scatter_kernel": 24,                   # read 12, write 12
+        "seg_forward_kernel": 12 + 4,
+        "seg_reverse_vjp_kernel": 16 + 4,
+    }
+    return float(table.get(name, 0.0))
+
+
+def event_time_ms(fn, reps: int, warmup: int = 3):
+    """Per-call device times (ms) of fn() on the current stream, CUDA events, after warm-up."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    out = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        b.synchronize()
+        out.append(a.elapsed_time(b))
+    return out
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons while a timed region runs."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int = 0, period_ms: int = 100):
+        self.lines = []
+        self.proc = None
+        self.thread = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.QUERY, "--format=csv,noheader,nounits",
+                 "-lms", str(period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def to_dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def to_pinned(a):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    return t.pin_memory()
+
+
+# ------------------------------------------------------------------ workloads ------------
+
+C2_CELLS = [(op, w, dist) for op in ("min", "mul") for w in (1 << 10, 1 << 16) for dist in ("uniform", "zipf")]
+VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (roofline table)
+    "c1_rbi_add": 12, "c2_rbi_min": 16, "c2_rbi_mul": 28, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 32,
+    "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
+}
+PRIMAL_BYTES_PER_ELEM = {
+    "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
+    "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
+}
+
+
+def gen_c2_cell(op, w, dist, n, seed=0):
+    d = (W.c2_rbi_min if op == "min" else W.c2_rbi_mul)(n=n, w=w, dist=dist, seed=seed)
+    d["op"], d["dist"] = op, dist
+    return d
+
+
+class RbiCase:
+    """One reduce-by-index VJP problem resident on the device, with preallocated output/workspace."""
+
+    def __init__(self, op: B.Op, d, with_host: bool = False):
+        self.op, self.n, self.w = op, int(d["n"]), int(d["w"])
+        self.is_, self.vs, self.hb = to_dev(d["is_"]), to_dev(d["vs"]), to_dev(d["hist_bar"])
+        self.out = torch.empty(self.n, dtype=op.torch_dtype, device="cuda")
+        self.hist = torch.empty(self.w, dtype=op.torch_dtype, device="cuda")
+        self.ws = torch.empty(max(256, B.vjp_reduce_by_index_workspace_bytes(op, self.n, self.w)),
+                              dtype=torch.uint8, device="cuda")
+        self.host = None
+        if with_host:
+            self.host = dict(is_=to_pinned(d["is_"]), vs=to_pinned(d["vs"]), hb=to_pinned(d["hist_bar"]),
+                             out=torch.empty(self.n, dtype=op.torch_dtype).pin_memory())
+            self.scratch = torch.empty(B.vjp_reduce_by_index_host_scratch_bytes(op, self.n, self.w),
+                                       dtype=torch.uint8, device="cuda")
+
+    def vjp(self):
+        return B.vjp_reduce_by_index(self.op, self.w, self.is_, self.vs, self.hb, out=self.out, ws=self.ws)
+
+    def primal(self):
+        return B.reduce_by_index_forward(self.op, self.w, self.is_, self.vs, out=self.hist, ws=self.ws)
+
+    def vjp_host(self):
+        h = self.host
+        return B.vjp_reduce_by_index_host(self.op, self.w, h["is_"], h["vs"], h["hb"], h["out"], self.scratch)
+
+    def h2d_bytes(self):
+        h = self.host
+        return h["is_"].numel() * 8 + h["vs"].numel() * h["vs"].element_size() + h["hb"].numel() * h["hb"].element_size()
+
+    def d2h_bytes(self):
+        return self.host["out"].numel() * self.host["out"].element_size()
+
+
+class ScanCase:
+    def __init__(self, op: B.Op, d):
+        self.op, self.n = op, int(d["n"])
+        self.xs, self.yb = to_dev(d["xs"]), to_dev(d["ys_bar"])
+        self.out = torch.empty_like(self.yb)
+        self.ws = torch.empty(max(256, B.vjp_scan_workspace_bytes(op, self.n)), dtype=torch.uint8, device="cuda")
+
+    def vjp(self):
+        return B.vjp_scan(self.op, self.xs, self.yb, out=self.out, ws=self.ws)
+
+    def primal(self):
+        return B.scan_forward(self.op, self.xs, out=self.out, ws=self.ws)
+
+
+def measure_case(key, label, case, reps, peak_gbs):
+    """VJP and primal timings of one case (median over reps, CUDA events)."""
+    tv = statistics.median(event_time_ms(case.vjp, reps))
+    tp = statistics.median(event_time_ms(case.primal, reps))
+    n = case.n
+    vb, pb = VJP_BYTES_PER_ELEM[key] * n, PRIMAL_BYTES_PER_ELEM[key] * n
+    gbs = vb / (tv * 1e-3) / 1e9
+    return {
+        "case": label, "n": n, "vjp_ms": round(tv, 4), "primal_ms": round(tp, 4),
+        "vjp_gelem_s": round(n / (tv * 1e-3) / 1e9, 3),
+        "ad_overhead": round((tp + tv) / tp, 3),            # BASELINE.json: (primal + VJP) / primal
+        "vjp_over_primal": round(tv / tp, 3),               # the VJP call alone (it re-executes the forward part)
+        "vjp_alg_gbs": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak_gbs, 3),
+        "frac_of_8tbs": round(gbs / NORTH_STAR_PEAK_GBS, 3),
+        "primal_alg_gbs": round(pb / (tp * 1e-3) / 1e9, 1),
+    }
+
+
+def measure_all_configs(reps, peak_gbs, scale=1.0, log=None):
+    """Every BASELINE config at full size (scale < 1 shrinks n, for quick checks), one at a time."""
+    rows = []
+
+    def say(msg):
+        if log:
+            log(msg)
+
+    def sz(n):
+        return max(1024, int(n * scale))
+
+    say("config 1")
+    d = W.c1_rbi_add(n=sz(W.FULL["c1"]["n"]))
+    rows.append(measure_case("c1_rbi_add", "c1 rbi + f32 w=1024 (L2-resident, latency-bound)",
+                             RbiCase(B.Op.of("add"), d), reps, peak_gbs))
+    d = W.c1_rbi_add(n=sz(1 << 26))
+    rows.append(measure_case("c1_rbi_add", "c1 twin rbi + f32 w=1024 n=2^26 (bandwidth)",
+                             RbiCase(B.Op.of("add"), d), reps, peak_gbs))
+    for op, w, dist in C2_CELLS:
+        say("config 2 %s w=%d %s" % (op, w, dist))
+        d = gen_c2_cell(op, w, dist, sz(W.FULL["c2"]["n"]))
+        rows.append(measure_case("c2_rbi_" + op, "c2 rbi %s f32 w=%d %s" % (op, w, dist),
+                                 RbiCase(B.Op.of(op), d), reps, peak_gbs))
+    n3 = sz(W.FULL["c3"]["n"])
+    say("config 3")
+    rows.append(measure_case("c3_scan_add_f32", "c3 scan + f32", ScanCase(B.Op.of("add"), W.c3_scan_add(n=n3)),
+                             reps, peak_gbs))
+    rows.append(measure_case("c3_scan_mul_f64", "c3 scan * f64",
+                             ScanCase(B.Op.of("mul", torch.float64), W.c3_scan_mul(n=n3)), reps, peak_gbs))
+    rows.append(measure_case("c3_scan_linrec_f32", "c3 scan linrec f32x2",
+                             ScanCase(B.Op.of("linrec"), W.c3_scan_linrec(n=n3)), reps, peak_gbs))
+    say("config 4")
+    rows.append(measure_case("c4_scan_matmul2", "c4 scan matmul 2x2 f32",
+                             ScanCase(B.Op.of("matmul2"), W.c4_scan_matmul(2, n=sz(W.FULL["c4"]["n2"]))), reps, peak_gbs))
+    rows.append(measure_case("c4_scan_matmul5", "c4 scan matmul 5x5 f32",
+                             ScanCase(B.Op.of("matmul5"), W.c4_scan_matmul(5, n=sz(W.FULL["c4"]["n5"]))), reps, peak_gbs))
+    say("config 5")
+    d = W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"]))
+    rows.append(measure_case("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
+                             RbiCase(B.Op.of("satadd", S=d["S"]), d), reps, peak_gbs))
+    return rows

@@ -28,6 +28,7 @@ EXPORTS = [
     "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_reduce_by_index_workspace_bytes",
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
     "vjp_reduce_by_index_host", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
+    "vjp_kernel_count", "vjp_kernel_name", "vjp_launch_count", "vjp_profile_enable", "vjp_profile_read",
 ]
 
 
@@ -93,6 +94,12 @@ def load() -> ctypes.CDLL:
         "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_kernel_count": (ctypes.c_int, []),
+        "vjp_kernel_name": (ctypes.c_char_p, [ctypes.c_int]),
+        "vjp_launch_count": (i64, [ctypes.c_int]),
+        "vjp_profile_enable": (None, [ctypes.c_int]),
+        "vjp_profile_read": (ctypes.c_int, [ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                            ctypes.POINTER(ctypes.c_int64)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)  # AttributeError if the library does not export it
@@ -279,3 +286,31 @@ def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm
+
+
+# ------------------------------------------------------------------ instrumentation ------
+
+def kernel_names():
+    lib = load()
+    return [lib.vjp_kernel_name(i).decode() for i in range(lib.vjp_kernel_count())]
+
+
+def launch_count(kid: int = -1) -> int:
+    """Launches of kernel `kid` (all kernels if negative) since the library was loaded."""
+    return int(load().vjp_launch_count(kid))
+
+
+def profile_enable(on: bool) -> None:
+    load().vjp_profile_enable(1 if on else 0)
+
+
+def profile_read():
+    """{kernel name: (total ms, recorded launches)} for the kernels recorded since profile_enable(True)."""
+    lib = load()
+    out = {}
+    for i, name in enumerate(kernel_names()):
+        ms, cnt = ctypes.c_double(0.0), ctypes.c_int64(0)
+        _check(lib.vjp_profile_read(i, ctypes.byref(ms), ctypes.byref(cnt)), "vjp_profile_read")
+        if cnt.value:
+            out[name] = (ms.value, cnt.value)
+    return out

@@ -42,7 +42,72 @@ cudaStream_t as_stream(void *s) { return static_cast<cudaStream_t>(s); }
 
 }  // namespace
 
+// ------------------------------------------------------------------ instrumentation ------
+namespace vjp {
+namespace {
+const char *const KERNEL_NAMES[K_COUNT] = {
+    "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEPRE>", "scan_vjp_reverse_kernel",
+    "rbi_fill_kernel", "rbi_forward_kernel", "rbi_decode_kernel", "rbi_vjp_add_kernel",
+    "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_mul_lifted_kernel",
+    "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
+    "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
+    "seg_reverse_vjp_kernel", "sort_export_kernel"};
+constexpr int PROF_MAX = 8192;
+struct ProfRec { int kid; cudaEvent_t a, b; };
+long long g_launches[K_COUNT];
+bool g_prof_on = false;
+ProfRec g_rec[PROF_MAX];
+int g_nrec = 0, g_nalloc = 0;
+}  // namespace
+
+void prof_begin(int kid, cudaStream_t s) {
+    __atomic_add_fetch(&g_launches[kid], 1, __ATOMIC_RELAXED);
+    if (!g_prof_on || g_nrec >= PROF_MAX) return;
+    if (g_nrec >= g_nalloc) {
+        if (cudaEventCreate(&g_rec[g_nalloc].a) != cudaSuccess) return;
+        if (cudaEventCreate(&g_rec[g_nalloc].b) != cudaSuccess) return;
+        g_nalloc++;
+    }
+    g_rec[g_nrec].kid = kid;
+    cudaEventRecord(g_rec[g_nrec].a, s);
+}
+void prof_end(int kid, cudaStream_t s) {
+    if (!g_prof_on || g_nrec >= g_nalloc || g_nrec >= PROF_MAX || g_rec[g_nrec].kid != kid) return;
+    cudaEventRecord(g_rec[g_nrec].b, s);
+    g_nrec++;
+}
+}  // namespace vjp
+
 extern "C" {
+
+int vjp_kernel_count(void) { return K_COUNT; }
+const char *vjp_kernel_name(int kid) { return (kid >= 0 && kid < K_COUNT) ? KERNEL_NAMES[kid] : nullptr; }
+int64_t vjp_launch_count(int kid) {
+    if (kid >= 0 && kid < K_COUNT) return g_launches[kid];
+    long long t = 0;
+    for (int i = 0; i < K_COUNT; i++) t += g_launches[i];
+    return t;
+}
+void vjp_profile_enable(int on) {
+    g_prof_on = on != 0;
+    g_nrec = 0;
+}
+int vjp_profile_read(int kid, double *total_ms, int64_t *launches) {
+    if (kid < 0 || kid >= K_COUNT || !total_ms || !launches) return VJP_ERR_INVALID_ARG;
+    double t = 0.0;
+    int64_t c = 0;
+    for (int i = 0; i < g_nrec; i++) {
+        if (g_rec[i].kid != kid) continue;
+        if (cudaEventSynchronize(g_rec[i].b) != cudaSuccess) return VJP_ERR_CUDA;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, g_rec[i].a, g_rec[i].b) != cudaSuccess) return VJP_ERR_CUDA;
+        t += ms;
+        c++;
+    }
+    *total_ms = t;
+    *launches = c;
+    return VJP_OK;
+}
 
 int vjp_scan_arity(const vjp_op_t *op) {
     if (!op) return -1;

@@ -20,6 +20,26 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? VJP_OK : VJP_ERR_CUDA; }
 inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 
+// ------------------------------------------------------------------ instrumentation ------
+// Every kernel launch of the library goes through a LaunchScope: it counts the launch and, while
+// profiling is enabled (vjp_profile_enable), brackets it with CUDA events on the launching stream.
+enum KernelId : int {
+    K_SCAN_LOOKBACK = 0, K_SCAN_TILEPRE, K_SCAN_VJP_REVERSE,
+    K_RBI_FILL, K_RBI_FORWARD, K_RBI_DECODE, K_RBI_GATHER,
+    K_MINMAX_LIFTED, K_MINMAX_FINISH, K_MUL_LIFTED, K_MUL_FINISH, K_MUL_SWEEP,
+    K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
+    K_COUNT
+};
+void prof_begin(int kid, cudaStream_t s);
+void prof_end(int kid, cudaStream_t s);
+struct LaunchScope {
+    int k;
+    cudaStream_t s;
+    LaunchScope(int kid, cudaStream_t st) : k(kid), s(st) { prof_begin(k, s); }
+    ~LaunchScope() { prof_end(k, s); }
+};
+#define VJP_LAUNCH(kid, stream) if (::vjp::LaunchScope vjp_ls_{kid, stream}; true)
+
 // ------------------------------------------------------------------------------ scans ---
 size_t scan_workspace_bytes(int code, int dtype, int64_t n);
 int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,

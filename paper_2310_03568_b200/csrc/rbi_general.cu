@@ -532,17 +532,17 @@ static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, co
         const int dst = ps & 1;
         const int64_t m = (int64_t)radix * nt;
         if (ps == 0)
-            sort_hist_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, nullptr, shift, radix, nt, g.counts);
+            VJP_LAUNCH(K_SORT_HIST, stream) sort_hist_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, nullptr, shift, radix, nt, g.counts);
         else
-            sort_hist_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, g.key[src], shift, radix, nt, g.counts);
+            VJP_LAUNCH(K_SORT_HIST, stream) sort_hist_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, g.key[src], shift, radix, nt, g.counts);
         if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
         const int sb = (int)((m + US_NT * US_IPT - 1) / (US_NT * US_IPT));
-        u32_exclusive_scan_kernel<<<sb, US_NT, 0, stream>>>(g.counts, m, g.ticket, g.status);
+        VJP_LAUNCH(K_U32_SCAN, stream) u32_exclusive_scan_kernel<<<sb, US_NT, 0, stream>>>(g.counts, m, g.ticket, g.status);
         if (ps == 0)
-            sort_scatter_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, vs, nullptr, nullptr, shift, radix,
+            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<true><<<nt, SORT_NT, 0, stream>>>(n, w, is, vs, nullptr, nullptr, shift, radix,
                                                                   nt, g.counts, g.key[dst], g.pay[dst]);
         else
-            sort_scatter_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, nullptr, g.key[src],
+            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<false><<<nt, SORT_NT, 0, stream>>>(n, w, nullptr, nullptr, g.key[src],
                                                                    g.pay[src], shift, radix, nt, g.counts,
                                                                    g.key[dst], g.pay[dst]);
         src = dst;
@@ -563,10 +563,10 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
     const GenOp<CODE> op{S};
     const int nt = (int)seg_tiles(n);
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    seg_forward_kernel<CODE><<<nt, SEG_NT, KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+    VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
         n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, 2 * KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+    VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, 2 * KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
         n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status);
     return last_launch_status();
 }
@@ -595,7 +595,7 @@ int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorte
     int rc = run_sort(n, w, is, nullptr, g, &buf, stream);
     if (rc != VJP_OK) return rc;
     const int grid = (int)((n + 255) / 256 < 2368 ? (n + 255) / 256 : 2368);
-    sort_export_kernel<<<grid, 256, 0, stream>>>(n, g.key[buf], g.pay[buf], sorted_keys, perm);
+    VJP_LAUNCH(K_SORT_EXPORT, stream) sort_export_kernel<<<grid, 256, 0, stream>>>(n, g.key[buf], g.pay[buf], sorted_keys, perm);
     return last_launch_status();
 }
 

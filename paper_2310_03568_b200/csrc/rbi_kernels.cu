@@ -244,17 +244,17 @@ static int run_forward(int64_t n, int64_t w, const int64_t *is, const void *vs, 
     C *tab = static_cast<C *>(hist);
     if (w == 0) return VJP_OK;
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
-    rbi_fill_kernel<ACC, T><<<fb, 256, 0, stream>>>(tab, w, S);
+    VJP_LAUNCH(K_RBI_FILL, stream) rbi_fill_kernel<ACC, T><<<fb, 256, 0, stream>>>(tab, w, S);
     if (n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         if ((size_t)w * sizeof(C) <= RBI_SMEM_TABLE_MAX)
-            rbi_forward_kernel<ACC, T, true><<<grid, RBI_NT, (size_t)w * sizeof(C), stream>>>(
+            VJP_LAUNCH(K_RBI_FORWARD, stream) rbi_forward_kernel<ACC, T, true><<<grid, RBI_NT, (size_t)w * sizeof(C), stream>>>(
                 n, w, is, static_cast<const T *>(vs), tab, S);
         else
-            rbi_forward_kernel<ACC, T, false><<<grid, RBI_NT, 0, stream>>>(
+            VJP_LAUNCH(K_RBI_FORWARD, stream) rbi_forward_kernel<ACC, T, false><<<grid, RBI_NT, 0, stream>>>(
                 n, w, is, static_cast<const T *>(vs), tab, S);
     }
-    if (ACC == ACC_MIN || ACC == ACC_MAX) rbi_decode_kernel<ACC, T><<<fb, 256, 0, stream>>>(tab, w);
+    if (ACC == ACC_MIN || ACC == ACC_MAX) VJP_LAUNCH(K_RBI_DECODE, stream) rbi_decode_kernel<ACC, T><<<fb, 256, 0, stream>>>(tab, w);
     return last_launch_status();
 }
 
@@ -307,10 +307,10 @@ static int run_vjp_add(int64_t n, int64_t w, const int64_t *is, const void *hist
     const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
     const size_t bytes = (size_t)w * sizeof(T);
     if (bytes <= GATHER_SMEM_MAX / 2) {
-        rbi_vjp_add_kernel<T, true><<<grid, RBI_NT, bytes, stream>>>(
+        VJP_LAUNCH(K_RBI_GATHER, stream) rbi_vjp_add_kernel<T, true><<<grid, RBI_NT, bytes, stream>>>(
             n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar));
     } else {
-        rbi_vjp_add_kernel<T, false><<<grid, RBI_NT, 0, stream>>>(
+        VJP_LAUNCH(K_RBI_GATHER, stream) rbi_vjp_add_kernel<T, false><<<grid, RBI_NT, 0, stream>>>(
             n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar));
     }
     return last_launch_status();
@@ -333,7 +333,8 @@ constexpr unsigned long long EMPTY_KEY = ~0ull;
 template <bool IS_MAX, bool SMEM>
 __global__ void __launch_bounds__(RBI_NT)
 rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
-                         const float *__restrict__ vs, unsigned long long *tab) {
+                         const float *__restrict__ vs, unsigned long long *tab,
+                         float *__restrict__ vs_bar /* zero-filled here if not NULL */) {
     extern __shared__ uint4 smem_raw[];
     unsigned long long *sh = reinterpret_cast<unsigned long long *>(smem_raw);
     if (SMEM) {
@@ -346,6 +347,10 @@ rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         float v[4];
         const int cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
+        if (vs_bar) {
+            const float z[4] = {0.f, 0.f, 0.f, 0.f};
+            store_vals4(vs_bar, q * 4, cnt, z);
+        }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             if (!in_range(k[j], w)) continue;
@@ -396,10 +401,12 @@ static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
                       const float *hist_bar, float *vs_bar, int64_t *arg, float *ext, void *ws,
                       cudaStream_t stream) {
     unsigned long long *tab = static_cast<unsigned long long *>(ws);
-    if (vs_bar && n > 0 &&
-        cudaMemsetAsync(vs_bar, 0, (size_t)n * sizeof(float), stream) != cudaSuccess)
-        return VJP_ERR_CUDA;
-    if (w == 0) return VJP_OK;
+    if (w == 0) {  // no bins: every adjoint is 0
+        if (vs_bar && n > 0 &&
+            cudaMemsetAsync(vs_bar, 0, (size_t)n * sizeof(float), stream) != cudaSuccess)
+            return VJP_ERR_CUDA;
+        return VJP_OK;
+    }
     if (cudaMemsetAsync(tab, 0xff, (size_t)w * 8, stream) != cudaSuccess) return VJP_ERR_CUDA;
     if (n > 0) {
         const size_t bytes = (size_t)w * 8;
@@ -410,14 +417,14 @@ static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
                                      (int)MINMAX_SMEM_MAX) != cudaSuccess)
                 return VJP_ERR_CUDA;
             const int per_sm = bytes <= 16 * 1024 ? RBI_CTAS_PER_SM : (bytes <= 32 * 1024 ? 3 : 2);
-            kern<<<grid_for(n, RBI_NT, per_sm), RBI_NT, bytes, stream>>>(n, w, is, vs, tab);
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, RBI_NT, per_sm), RBI_NT, bytes, stream>>>(n, w, is, vs, tab, vs_bar);
         } else {
-            rbi_minmax_lifted_kernel<IS_MAX, false>
-                <<<grid_for(n, RBI_NT, RBI_CTAS_PER_SM), RBI_NT, 0, stream>>>(n, w, is, vs, tab);
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) rbi_minmax_lifted_kernel<IS_MAX, false>
+                <<<grid_for(n, RBI_NT, RBI_CTAS_PER_SM), RBI_NT, 0, stream>>>(n, w, is, vs, tab, vs_bar);
         }
     }
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
-    rbi_minmax_finish_kernel<IS_MAX><<<fb, 256, 0, stream>>>(n, w, tab, hist_bar, vs_bar, arg, ext);
+    VJP_LAUNCH(K_MINMAX_FINISH, stream) rbi_minmax_finish_kernel<IS_MAX><<<fb, 256, 0, stream>>>(n, w, tab, hist_bar, vs_bar, arg, ext);
     return last_launch_status();
 }
 
@@ -561,17 +568,17 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
         cudaFuncSetAttribute(rbi_mul_lifted_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(MUL_PART * sizeof(float))) != cudaSuccess)
         return VJP_ERR_CUDA;
-    rbi_mul_lifted_kernel<<<G, MUL_NT, smem, stream>>>(n, w, part_bins, is, vs, m.part, m.zeros);
+    VJP_LAUNCH(K_MUL_LIFTED, stream) rbi_mul_lifted_kernel<<<G, MUL_NT, smem, stream>>>(n, w, part_bins, is, vs, m.part, m.zeros);
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
-    rbi_mul_finish_kernel<<<fb, 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
+    VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fb, 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
                                                   vs_bar ? m.coef : nullptr);
     if (vs_bar && n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         const size_t bytes = (size_t)w * sizeof(float2);
         if (bytes <= GATHER_SMEM_MAX / 2)
-            rbi_mul_sweep_kernel<true><<<grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar);
+            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<true><<<grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar);
         else
-            rbi_mul_sweep_kernel<false><<<grid, RBI_NT, 0, stream>>>(n, w, is, vs, m.coef, vs_bar);
+            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<false><<<grid, RBI_NT, 0, stream>>>(n, w, is, vs, m.coef, vs_bar);
     }
     return last_launch_status();
 }

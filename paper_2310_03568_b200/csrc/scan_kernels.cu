@@ -267,6 +267,7 @@ static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
+    VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : K_SCAN_TILEPRE, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(in),
                                              static_cast<uint32_t *>(out), n, (int)nt, lw, fpre);
     return last_launch_status();
@@ -310,6 +311,7 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
+    VJP_LAUNCH(K_SCAN_VJP_REVERSE, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(xs),
                                              static_cast<const uint32_t *>(ys_bar),
                                              static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw);
