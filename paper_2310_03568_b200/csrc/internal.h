@@ -38,7 +38,8 @@ struct LaunchScope {
     LaunchScope(int kid, cudaStream_t st) : k(kid), s(st) { prof_begin(k, s); }
     ~LaunchScope() { prof_end(k, s); }
 };
-#define VJP_LAUNCH(kid, stream) if (::vjp::LaunchScope vjp_ls_{kid, stream}; true)
+// else-safe: "if (c) VJP_LAUNCH(..) a<<<>>>(); else VJP_LAUNCH(..) b<<<>>>();" pairs up as written
+#define VJP_LAUNCH(kid, stream) if (::vjp::LaunchScope vjp_ls_{kid, stream}; false) {} else
 
 // ------------------------------------------------------------------------------ scans ---
 size_t scan_workspace_bytes(int code, int dtype, int64_t n);
