@@ -210,44 +210,80 @@ def measure_case(key, label, case, reps, peak_gbs):
     }
 
 
-def measure_all_configs(reps, peak_gbs, scale=1.0, log=None):
-    """Every BASELINE config at full size (scale < 1 shrinks n, for quick checks), one at a time."""
-    rows = []
-
-    def say(msg):
-        if log:
-            log(msg)
-
+def case_table(scale=1.0):
+    """(key, label, factory) of every measured case: the five BASELINE configs at full size
+    (scale < 1 shrinks n, for quick checks) plus the config-1 bandwidth twin."""
     def sz(n):
         return max(1024, int(n * scale))
 
-    say("config 1")
-    d = W.c1_rbi_add(n=sz(W.FULL["c1"]["n"]))
-    rows.append(measure_case("c1_rbi_add", "c1 rbi + f32 w=1024 (L2-resident, latency-bound)",
-                             RbiCase(B.Op.of("add"), d), reps, peak_gbs))
-    d = W.c1_rbi_add(n=sz(1 << 26))
-    rows.append(measure_case("c1_rbi_add", "c1 twin rbi + f32 w=1024 n=2^26 (bandwidth)",
-                             RbiCase(B.Op.of("add"), d), reps, peak_gbs))
+    def rbi(opname, gen, **kw):
+        def make():
+            d = gen()
+            return RbiCase(B.Op.of(opname, **({"S": d["S"]} if opname == "satadd" else {})), d)
+        return make
+
+    def scan(opname, gen, dtype=None):
+        def make():
+            return ScanCase(B.Op.of(opname, dtype) if dtype is not None else B.Op.of(opname), gen())
+        return make
+
+    t = [
+        ("c1_rbi_add", "c1 rbi + f32 w=1024 (L2-resident, latency-bound)",
+         rbi("add", lambda: W.c1_rbi_add(n=sz(W.FULL["c1"]["n"])))),
+        ("c1_rbi_add", "c1 twin rbi + f32 w=1024 n=2^26 (bandwidth)",
+         rbi("add", lambda: W.c1_rbi_add(n=sz(1 << 26)))),
+    ]
     for op, w, dist in C2_CELLS:
-        say("config 2 %s w=%d %s" % (op, w, dist))
-        d = gen_c2_cell(op, w, dist, sz(W.FULL["c2"]["n"]))
-        rows.append(measure_case("c2_rbi_" + op, "c2 rbi %s f32 w=%d %s" % (op, w, dist),
-                                 RbiCase(B.Op.of(op), d), reps, peak_gbs))
+        t.append(("c2_rbi_" + op, "c2 rbi %s f32 w=%d %s" % (op, w, dist),
+                  rbi(op, lambda op=op, w=w, dist=dist: gen_c2_cell(op, w, dist, sz(W.FULL["c2"]["n"])))))
     n3 = sz(W.FULL["c3"]["n"])
-    say("config 3")
-    rows.append(measure_case("c3_scan_add_f32", "c3 scan + f32", ScanCase(B.Op.of("add"), W.c3_scan_add(n=n3)),
-                             reps, peak_gbs))
-    rows.append(measure_case("c3_scan_mul_f64", "c3 scan * f64",
-                             ScanCase(B.Op.of("mul", torch.float64), W.c3_scan_mul(n=n3)), reps, peak_gbs))
-    rows.append(measure_case("c3_scan_linrec_f32", "c3 scan linrec f32x2",
-                             ScanCase(B.Op.of("linrec"), W.c3_scan_linrec(n=n3)), reps, peak_gbs))
-    say("config 4")
-    rows.append(measure_case("c4_scan_matmul2", "c4 scan matmul 2x2 f32",
-                             ScanCase(B.Op.of("matmul2"), W.c4_scan_matmul(2, n=sz(W.FULL["c4"]["n2"]))), reps, peak_gbs))
-    rows.append(measure_case("c4_scan_matmul5", "c4 scan matmul 5x5 f32",
-                             ScanCase(B.Op.of("matmul5"), W.c4_scan_matmul(5, n=sz(W.FULL["c4"]["n5"]))), reps, peak_gbs))
-    say("config 5")
-    d = W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"]))
-    rows.append(measure_case("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
-                             RbiCase(B.Op.of("satadd", S=d["S"]), d), reps, peak_gbs))
+    t += [
+        ("c3_scan_add_f32", "c3 scan + f32", scan("add", lambda: W.c3_scan_add(n=n3))),
+        ("c3_scan_mul_f64", "c3 scan * f64", scan("mul", lambda: W.c3_scan_mul(n=n3), torch.float64)),
+        ("c3_scan_linrec_f32", "c3 scan linrec f32x2", scan("linrec", lambda: W.c3_scan_linrec(n=n3))),
+        ("c4_scan_matmul2", "c4 scan matmul 2x2 f32",
+         scan("matmul2", lambda: W.c4_scan_matmul(2, n=sz(W.FULL["c4"]["n2"])))),
+        ("c4_scan_matmul5", "c4 scan matmul 5x5 f32",
+         scan("matmul5", lambda: W.c4_scan_matmul(5, n=sz(W.FULL["c4"]["n5"])))),
+        ("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
+         rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])))),
+    ]
+    return t
+
+
+def measure_all_configs(reps, peak_gbs, scale=1.0, log=None, only=None):
+    """Every case of case_table(), one at a time; `only` = substrings of the labels to keep."""
+    rows = []
+    for key, label, make in case_table(scale):
+        if only and not any(s in label for s in only):
+            continue
+        if log:
+            log(label)
+        case = make()
+        rows.append(measure_case(key, label, case, reps, peak_gbs))
+        del case
+        torch.cuda.empty_cache()
     return rows
+
+
+def main(argv=None):
+    """python -m paper_2310_03568_b200.benchlib --cases 'scan +,matmul' [--reps R] [--scale S]
+    times the named cases only (one JSON row per line): the command the ncu captures under
+    profiles/ were taken with."""
+    import argparse
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--cases", default="")
+    ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--scale", type=float, default=1.0)
+    a = ap.parse_args(argv)
+    if not torch.cuda.is_available():
+        raise SystemExit("needs a CUDA device: there is no CPU path")
+    B.load()
+    peak, _ = measured_peak()
+    only = [s for s in a.cases.split(",") if s] or None
+    for row in measure_all_configs(a.reps, peak, a.scale, only=only):
+        print(json.dumps(row), flush=True)
+
+
+if __name__ == "__main__":
+    main()
