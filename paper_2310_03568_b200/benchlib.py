@@ -35,7 +35,7 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
     table = {
         "rbi_vjp_add_kernel": 8 + elem_bytes,        # is + write vs_bar
         "rbi_minmax_lifted_kernel": 8 + 4 + 4,       # is + vs + zero-fill of vs_bar
-        "rbi_mul_lifted_kernel": 8 + 4,              # is + vs (per pass over the input)
+        "rbi_cached_kernel": 8 + 4,                  # is + vs
         "rbi_mul_sweep_kernel": 8 + 4 + 4,           # is + vs + write vs_bar
         "rbi_forward_kernel": 8 + elem_bytes,
         "scan_lookback_kernel<MODE_SCAN>": 2 * elem_bytes,

@@ -47,9 +47,9 @@ namespace vjp {
 namespace {
 const char *const KERNEL_NAMES[K_COUNT] = {
     "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEPRE>", "scan_vjp_reverse_kernel",
-    "rbi_fill_kernel", "rbi_forward_kernel", "rbi_decode_kernel", "rbi_vjp_add_kernel",
-    "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_mul_lifted_kernel",
-    "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
+    "rbi_fill_kernel", "rbi_forward_kernel", "rbi_vjp_add_kernel",
+    "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_cached_kernel",
+    "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel"};
 constexpr int PROF_MAX = 8192;
@@ -185,22 +185,27 @@ int vjp_scan_host(const vjp_op_t *op, int64_t n, const void *xs_host, const void
 
 size_t vjp_reduce_by_index_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t num_bins) {
     if (!op_ok(op) || n < 0 || num_bins < 0) return 0;
+    size_t need;
     switch (rbi_route(op)) {
     case 1:
     case 2:
-    case 3: return rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins);
-    case 4: return rbi_general_workspace_bytes(n, num_bins);
+    case 3: need = rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins); break;
+    case 4: need = rbi_general_workspace_bytes(n, num_bins); break;
     default: return 0;
     }
+    const size_t fwd = rbi_forward_workspace_bytes(op->code, n, num_bins);  // one query serves both calls
+    return need > fwd ? need : fwd;
 }
 
 int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
                             const void *vs, void *hist, void *ws, size_t ws_bytes, void *stream) {
-    (void)ws_bytes;
     if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
     if (rbi_route(op) == 0) return VJP_ERR_UNSUPPORTED;
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if ((num_bins > 0 && !hist) || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (num_bins > 0 && op->code != VJP_OP_ADD &&
+        (!ws || ws_bytes < rbi_forward_workspace_bytes(op->code, n, num_bins)))
+        return VJP_ERR_WORKSPACE;
     return launch_rbi_forward(op->code, op->dtype, op->param, n, num_bins, is, vs, hist, ws,
                               as_stream(stream));
 }

@@ -25,8 +25,8 @@ inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 // profiling is enabled (vjp_profile_enable), brackets it with CUDA events on the launching stream.
 enum KernelId : int {
     K_SCAN_LOOKBACK = 0, K_SCAN_TILEPRE, K_SCAN_VJP_REVERSE,
-    K_RBI_FILL, K_RBI_FORWARD, K_RBI_DECODE, K_RBI_GATHER,
-    K_MINMAX_LIFTED, K_MINMAX_FINISH, K_MUL_LIFTED, K_MUL_FINISH, K_MUL_SWEEP,
+    K_RBI_FILL, K_RBI_FORWARD, K_RBI_GATHER,
+    K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_ACC, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_COUNT
 };
@@ -50,6 +50,8 @@ int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *
 
 // -------------------------------------------------------------- reduce-by-index (special) -
 size_t rbi_special_workspace_bytes(int code, int dtype, int64_t n, int64_t w);
+size_t rbi_forward_workspace_bytes(int code, int64_t n, int64_t w);
+bool rbi_cached_supported(int64_t w);  // '*' / satadd tables: at most 8 passes over the input
 int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, const int64_t *is,
                        const void *vs, void *hist, void *ws, cudaStream_t stream);
 int launch_rbi_vjp_add(int dtype, int64_t n, int64_t w, const int64_t *is, const void *hist_bar,

@@ -125,59 +125,6 @@ struct Cell<ACC_ADD, T> {
     static VJP_DEVINL void upd(C *c, C v, float) { atomicAdd(c, v); }
     static VJP_DEVINL T dec(C c) { return c; }
 };
-template <>
-struct Cell<ACC_MIN, float> {
-    using C = uint32_t;
-    static VJP_DEVINL C neutral(float) { return ext_key<false>(CUDART_INF_F); }
-    static VJP_DEVINL C enc(float v) { return ext_key<false>(v); }
-    static VJP_DEVINL void upd(C *c, C v, float) {
-        if (v < *(volatile C *)c) atomicMin(c, v);
-    }
-    static VJP_DEVINL float dec(C c) { return ext_value<false>(c); }
-};
-template <>
-struct Cell<ACC_MAX, float> {
-    using C = uint32_t;
-    static VJP_DEVINL C neutral(float) { return ext_key<true>(-CUDART_INF_F); }
-    static VJP_DEVINL C enc(float v) { return ext_key<true>(v); }
-    static VJP_DEVINL void upd(C *c, C v, float) {
-        if (v < *(volatile C *)c) atomicMin(c, v);
-    }
-    static VJP_DEVINL float dec(C c) { return ext_value<true>(c); }
-};
-// No hardware atomic multiply (the paper's "atomicMul-class update"): compare-and-swap.
-VJP_DEVINL void atomic_mul_f32(float *c, float v) {
-    unsigned *a = reinterpret_cast<unsigned *>(c);
-    unsigned old = *(volatile unsigned *)a, assumed;
-    do {
-        assumed = old;
-        old = atomicCAS(a, assumed, __float_as_uint(__uint_as_float(assumed) * v));
-    } while (old != assumed);
-}
-template <>
-struct Cell<ACC_MUL, float> {
-    using C = float;
-    static VJP_DEVINL C neutral(float) { return 1.f; }
-    static VJP_DEVINL C enc(float v) { return v; }
-    static VJP_DEVINL void upd(C *c, C v, float) { atomic_mul_f32(c, v); }
-    static VJP_DEVINL float dec(C c) { return c; }
-};
-template <>
-struct Cell<ACC_SATADD, float> {  // min(a + b, S), Q16
-    using C = float;
-    static VJP_DEVINL C neutral(float) { return 0.f; }
-    static VJP_DEVINL C enc(float v) { return v; }
-    static VJP_DEVINL void upd(C *c, C v, float S) {
-        unsigned *a = reinterpret_cast<unsigned *>(c);
-        unsigned old = *(volatile unsigned *)a, assumed;
-        do {
-            assumed = old;
-            old = atomicCAS(a, assumed, __float_as_uint(fminf(__uint_as_float(assumed) + v, S)));
-        } while (old != assumed);
-    }
-    static VJP_DEVINL float dec(C c) { return c; }
-};
-
 template <int ACC, class T>
 __global__ void rbi_fill_kernel(typename Cell<ACC, T>::C *tab, int64_t w, float S) {
     for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
@@ -224,23 +171,12 @@ rbi_forward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const T
     }
 }
 
-template <int ACC, class T>
-__global__ void rbi_decode_kernel(typename Cell<ACC, T>::C *tab, int64_t w) {
-    using CL = Cell<ACC, T>;
-    for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
-         k += (int64_t)gridDim.x * blockDim.x) {
-        const T v = CL::dec(tab[k]);
-        reinterpret_cast<T *>(tab)[k] = v;
-    }
-}
-
 constexpr size_t RBI_SMEM_TABLE_MAX = 32 * 1024;  // private histogram up to this size per CTA
 
 template <int ACC, class T>
 static int run_forward(int64_t n, int64_t w, const int64_t *is, const void *vs, void *hist,
                        float S, cudaStream_t stream) {
     using C = typename Cell<ACC, T>::C;
-    static_assert(sizeof(C) == sizeof(T), "cells are decoded in place");
     C *tab = static_cast<C *>(hist);
     if (w == 0) return VJP_OK;
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
@@ -254,12 +190,15 @@ static int run_forward(int64_t n, int64_t w, const int64_t *is, const void *vs, 
             VJP_LAUNCH(K_RBI_FORWARD, stream) rbi_forward_kernel<ACC, T, false><<<grid, RBI_NT, 0, stream>>>(
                 n, w, is, static_cast<const T *>(vs), tab, S);
     }
-    if (ACC == ACC_MIN || ACC == ACC_MAX) VJP_LAUNCH(K_RBI_DECODE, stream) rbi_decode_kernel<ACC, T><<<fb, 256, 0, stream>>>(tab, w);
     return last_launch_status();
 }
 
+// '*' and satadd have no hardware atomic: cached accumulation (defined further down)
+static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                                float *hist, void *ws, float S, cudaStream_t stream);
+
 int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, const int64_t *is,
-                       const void *vs, void *hist, void *, cudaStream_t stream) {
+                       const void *vs, void *hist, void *ws, cudaStream_t stream) {
     const float S = (float)param;
     if (dtype == VJP_F64) {
         if (code == VJP_OP_ADD) return run_forward<ACC_ADD, double>(n, w, is, vs, hist, S, stream);
@@ -267,10 +206,14 @@ int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, 
     }
     switch (code) {
     case VJP_OP_ADD: return run_forward<ACC_ADD, float>(n, w, is, vs, hist, S, stream);
-    case VJP_OP_MIN: return run_forward<ACC_MIN, float>(n, w, is, vs, hist, S, stream);
-    case VJP_OP_MAX: return run_forward<ACC_MAX, float>(n, w, is, vs, hist, S, stream);
-    case VJP_OP_MUL: return run_forward<ACC_MUL, float>(n, w, is, vs, hist, S, stream);
-    case VJP_OP_SATADD: return run_forward<ACC_SATADD, float>(n, w, is, vs, hist, S, stream);
+    case VJP_OP_MIN:  // the packed-key kernels of the lifted operator, value part only
+    case VJP_OP_MAX:
+        return launch_rbi_minmax(code, n, w, is, static_cast<const float *>(vs), nullptr, nullptr, nullptr,
+                                 static_cast<float *>(hist), ws, stream);
+    case VJP_OP_MUL:
+    case VJP_OP_SATADD:
+        return launch_cached_primal(code, n, w, is, static_cast<const float *>(vs),
+                                    static_cast<float *>(hist), ws, S, stream);
     default: return VJP_ERR_UNSUPPORTED;
     }
 }
@@ -375,6 +318,64 @@ rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
+// Histograms too large for a private shared-memory copy (w > 8192): the packed keys live in global
+// memory (L2) and every CTA keeps a FILTER in shared memory: per slot the top 16 bits of the best
+// (ordered) value key this CTA has seen for the slot's bin.  A bin's minimum only ever decreases, so
+// any value once observed is an upper bound of the current one, and an element whose 16-bit prefix
+// is strictly above the filter cannot win: it is dropped without touching L2.  Racing plain stores
+// can only leave a weaker (larger) bound behind.  Without the filter every element of a hot bin
+// reads the same L2 sector, which a single L2 slice serialises (profiles/r1a: 0.9 ms at Zipf keys).
+// TAGGED = false: w <= 65536, slot = bin, 2-byte entries.  TAGGED = true: 32768 slots of
+// (bin >> 15) << 16 | prefix; a slot that holds another bin does not filter.
+constexpr int MMF_NT = 1024;
+constexpr size_t MMF_SMEM = 128 * 1024;
+
+template <bool IS_MAX, bool TAGGED>
+__global__ void __launch_bounds__(MMF_NT, 1)
+rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                           const float *__restrict__ vs, unsigned long long *tab,
+                           float *__restrict__ vs_bar) {
+    extern __shared__ uint4 smem_raw[];
+    uint16_t *f16 = reinterpret_cast<uint16_t *>(smem_raw);  // [65536]
+    uint32_t *f32 = reinterpret_cast<uint32_t *>(smem_raw);  // [32768]
+    for (int k = threadIdx.x; k < (int)(MMF_SMEM / 16); k += MMF_NT)
+        smem_raw[k] = make_uint4(~0u, ~0u, ~0u, ~0u);
+    __syncthreads();
+    const int64_t stride = (int64_t)gridDim.x * MMF_NT;
+    for (int64_t q = blockIdx.x * (int64_t)MMF_NT + threadIdx.x; q * 4 < n; q += stride) {
+        int64_t k[4];
+        float v[4];
+        const int cnt = load_keys4(is, q * 4, n, k);
+        load_vals4(vs, q * 4, cnt, v);
+        if (vs_bar) {
+            const float z[4] = {0.f, 0.f, 0.f, 0.f};
+            store_vals4(vs_bar, q * 4, cnt, z);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            if (!in_range(k[j], w)) continue;
+            const uint32_t vk = ext_key<IS_MAX>(v[j]);
+            const uint32_t p16 = vk >> 16;
+            const uint32_t b = (uint32_t)k[j];
+            if (TAGGED) {
+                const uint32_t e = f32[b & 32767u];
+                if ((e >> 16) == (b >> 15) && p16 > (e & 0xffffu)) continue;
+            } else {
+                if (p16 > f16[b]) continue;
+            }
+            const unsigned long long key = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
+            unsigned long long cur = __ldcg(tab + k[j]);
+            if (key < cur) {
+                cur = atomicMin(tab + k[j], key);
+                if (key < cur) cur = key;
+            }
+            const uint32_t c16 = (uint32_t)(cur >> 48);
+            if (TAGGED) f32[b & 32767u] = ((b >> 15) << 16) | c16;
+            else f16[b] = (uint16_t)c16;
+        }
+    }
+}
+
 // arg / ext of every bin (an empty bin is (n, +-inf)) and the scatter of the return sweep
 // (P:L438-441).  vs_bar has been zeroed before.
 template <bool IS_MAX>
@@ -418,9 +419,16 @@ static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
                 return VJP_ERR_CUDA;
             const int per_sm = bytes <= 16 * 1024 ? RBI_CTAS_PER_SM : (bytes <= 32 * 1024 ? 3 : 2);
             VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, RBI_NT, per_sm), RBI_NT, bytes, stream>>>(n, w, is, vs, tab, vs_bar);
+        } else if (w <= 65536) {
+            auto kern = rbi_minmax_filtered_kernel<IS_MAX, false>;
+            if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
+                return VJP_ERR_CUDA;
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
         } else {
-            VJP_LAUNCH(K_MINMAX_LIFTED, stream) rbi_minmax_lifted_kernel<IS_MAX, false>
-                <<<grid_for(n, RBI_NT, RBI_CTAS_PER_SM), RBI_NT, 0, stream>>>(n, w, is, vs, tab, vs_bar);
+            auto kern = rbi_minmax_filtered_kernel<IS_MAX, true>;
+            if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
+                return VJP_ERR_CUDA;
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
         }
     }
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
@@ -435,46 +443,302 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
                               : run_minmax<false>(n, w, is, vs, hist_bar, vs_bar, arg, ext, ws, stream);
 }
 
-// ------------------------------------------------------------------ '*' VJP ---------------
+
+
+// ------------------------------------------------- cached accumulation ('*', satadd) -------
 //
-// Lifted primal: per bin (zero count, product of the non-zeros).  Each CTA owns a private
-// table of products in shared memory covering a partition of at most MUL_PART bins; a histogram
-// larger than that takes several passes over the input.  CTA g writes its table to
-// part[g][.]; a second kernel folds the G tables per bin in a fixed order.  Zeros are rare events
-// counted with integer atomics in global memory (exact, Q8).
+// Operators with no hardware atomic (the paper's "atomicMul-class update").  One
+// shared-memory atomicCAS per element is not affordable: ATOMS costs 2 cycles per lane on the SM's
+// LSU pipe, 64x a plain LDS/STS, and a CAS loop on a hot bin retries without bound (profiles/r1a:
+// 5 ms at Zipf keys).  match.any is no way out either: it issues about once per 30 cycles per SM
+// (profiles/r1b).  So every WARP owns a private direct-mapped write-back cache of (bin, partial
+// result) entries in shared memory that it updates with plain loads and stores only:
+//   1. the lanes of a warp arbitrate per slot through a claim byte: every pending lane stores its
+//      lane id, the warp syncs, the lane that reads its own id back owns the slot for this round
+//      and does a plain read-modify-write; the others retry.  Rounds = the largest number of lanes
+//      on one slot (1-2 for uniform keys, ~6 when one bin holds 18 % of the elements);
+//   2. hit: combine in place.  Miss: a 2-bit hit counter guards the resident entry -- a cold bin
+//      arriving at a hot slot decrements it and BYPASSES; only an entry whose counter has run out
+//      is evicted (Misra-Gries style), so hot bins stay resident whatever the key distribution;
+//   3. evictions / bypasses go to the CTA's table in shared memory with a CAS loop (cold bins only:
+//      little contention); a histogram larger than that table takes several passes over the input,
+//      one bin partition per pass.
+// With w <= CS_SLOTS a slot IS a bin: no tags, no evictions, no atomics at all.  CTA g writes its
+// result to part[g][.]; a second kernel folds the G tables per bin in a fixed order (deterministic).
 
-constexpr int MUL_NT = 1024;
-constexpr int MUL_PART = 48 * 1024;  // bins per pass (192 KB of f32 products)
+constexpr int CS_SLOTS = 1024, CS_WARPS = 8, CS_NT = CS_WARPS * 32, CS_CTAS_PER_SM = 5;   // w <= 1024
+constexpr int CB_SLOTS = 256, CB_WARPS = 32, CB_NT = CB_WARPS * 32;                       // w  > 1024
+constexpr int CB_PART = 36864;  // bins per pass: 144 KB of f32 next to 72 KB of warp caches
+constexpr int CB_MAX_PASSES = 8;
+constexpr uint32_t CB_EMPTY = 0xffffffffu;  // tag word = (bin / CB_SLOTS) << 2 | hit counter
 
-__global__ void __launch_bounds__(MUL_NT)
-rbi_mul_lifted_kernel(int64_t n, int64_t w, int part_bins, const int64_t *__restrict__ is,
-                      const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros) {
+template <int ACC>
+struct CachedOp;
+template <>
+struct CachedOp<ACC_MUL> {
+    static VJP_DEVINL float neutral() { return 1.f; }
+    static VJP_DEVINL float comb(float a, float b, float) { return a * b; }
+};
+template <>
+struct CachedOp<ACC_SATADD> {
+    static VJP_DEVINL float neutral() { return 0.f; }
+    static VJP_DEVINL float comb(float a, float b, float S) { return fminf(a + b, S); }
+};
+
+template <int ACC>
+VJP_DEVINL void smem_combine(float *cell, float v, float S) {
+    unsigned *a = reinterpret_cast<unsigned *>(cell);
+    unsigned old = *(volatile unsigned *)a, assumed;
+    do {
+        assumed = old;
+        old = atomicCAS(a, assumed, __float_as_uint(CachedOp<ACC>::comb(__uint_as_float(assumed), v, S)));
+    } while (old != assumed);
+}
+
+// w <= CS_SLOTS.  32 elements, one per lane; lanes with act hold (bin b, value x).
+template <int ACC>
+VJP_DEVINL void claim_update_small(bool act, uint32_t b, float x, float *vl, uint8_t *cl, float S,
+                                   int lane) {
+    bool pend = act;
+    while (__any_sync(FULL_MASK, pend)) {
+        if (pend) cl[b] = (uint8_t)lane;
+        __syncwarp();
+        if (pend && cl[b] == lane) {
+            vl[b] = CachedOp<ACC>::comb(vl[b], x, S);
+            pend = false;
+        }
+        __syncwarp();
+    }
+}
+
+// w > CS_SLOTS.  Returns true if (eb, evv) must go to the CTA table.
+template <int ACC>
+VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint32_t *tg, uint8_t *cl,
+                                 float S, int lane, uint32_t &eb, float &evv) {
+    bool pend = act, ev = false;
+    const uint32_t slot = b & (CB_SLOTS - 1), hi = b / CB_SLOTS;
+    while (__any_sync(FULL_MASK, pend)) {
+        if (pend) cl[slot] = (uint8_t)lane;
+        __syncwarp();
+        if (pend && cl[slot] == lane) {
+            pend = false;
+            const uint32_t t = tg[slot];
+            if (t != CB_EMPTY && (t >> 2) == hi) {             // hit
+                vl[slot] = CachedOp<ACC>::comb(vl[slot], x, S);
+                if ((t & 3u) != 3u) tg[slot] = t + 1;
+            } else if (t == CB_EMPTY || (t & 3u) == 0u) {       // install (evicting)
+                if (t != CB_EMPTY) {
+                    ev = true;
+                    eb = (t >> 2) * CB_SLOTS + slot;
+                    evv = vl[slot];
+                }
+                tg[slot] = hi << 2;
+                vl[slot] = x;
+            } else {                                            // guarded: bypass
+                tg[slot] = t - 1;
+                ev = true;
+                eb = b;
+                evv = x;
+            }
+        }
+        __syncwarp();
+    }
+    return ev;
+}
+
+// COUNT_ZEROS: the lifted '*' of the VJP: zeros are counted (integer atomics, exact) and
+// kept out of the product.  Otherwise: the plain primal histogram of the operator.
+template <int ACC, bool COUNT_ZEROS>
+__global__ void __launch_bounds__(CS_NT, CS_CTAS_PER_SM)
+rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                        const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
+                        float S) {
+    using OP = CachedOp<ACC>;
     extern __shared__ uint4 smem_raw[];
-    float *sh = reinterpret_cast<float *>(smem_raw);
-    const int64_t stride = (int64_t)gridDim.x * MUL_NT;
-    for (int64_t lo = 0; lo < w; lo += part_bins) {
-        const int nb = (int)min((int64_t)part_bins, w - lo);
-        for (int k = threadIdx.x; k < nb; k += MUL_NT) sh[k] = 1.f;
+    float *vals = reinterpret_cast<float *>(smem_raw);                       // [CS_WARPS][CS_SLOTS]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(vals + CS_WARPS * CS_SLOTS);  // [CS_WARPS][CS_SLOTS]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *vl = vals + warp * CS_SLOTS;
+    uint8_t *cl = claim + warp * CS_SLOTS;
+    for (int s = lane; s < CS_SLOTS; s += 32) vl[s] = OP::neutral();
+    __syncwarp();
+    const int64_t nquads = (n + 3) / 4;
+    const int64_t stride = (int64_t)gridDim.x * CS_NT;
+    int64_t qw = blockIdx.x * (int64_t)CS_NT + warp * 32;  // warp-uniform: the warp never diverges here
+    int64_t k[4] = {-1, -1, -1, -1};
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    if (qw < nquads) {
+        const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
+        load_vals4(vs, (qw + lane) * 4, cnt, v);
+    }
+    while (qw < nquads) {
+        int64_t kn[4] = {-1, -1, -1, -1};
+        float vn[4] = {0.f, 0.f, 0.f, 0.f};
+        const int64_t qn = qw + stride;
+        if (qn < nquads) {  // next iteration's loads fly while this one is processed
+            const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
+            load_vals4(vs, (qn + lane) * 4, cnt, vn);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            bool act = in_range(k[j], w);
+            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
+                atomicAdd(zeros + k[j], 1u);
+                act = false;
+            }
+            claim_update_small<ACC>(act, (uint32_t)k[j], v[j], vl, cl, S, lane);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            k[j] = kn[j];
+            v[j] = vn[j];
+        }
+        qw = qn;
+    }
+    __syncthreads();
+    for (int s = threadIdx.x; s < (int)w; s += CS_NT) {
+        float acc = vals[s];
+#pragma unroll
+        for (int wp = 1; wp < CS_WARPS; wp++) acc = OP::comb(acc, vals[wp * CS_SLOTS + s], S);
+        part[(size_t)blockIdx.x * (size_t)w + s] = acc;
+    }
+}
+
+template <int ACC, bool COUNT_ZEROS>
+__global__ void __launch_bounds__(CB_NT, 1)
+rbi_cached_big_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                      const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
+                      float S) {
+    using OP = CachedOp<ACC>;
+    extern __shared__ uint4 smem_raw[];
+    float *table = reinterpret_cast<float *>(smem_raw);                        // [CB_PART]
+    float *vals = table + CB_PART;                                             // [CB_WARPS][CB_SLOTS]
+    uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);  // [CB_WARPS][CB_SLOTS]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(tags + CB_WARPS * CB_SLOTS);   // [CB_WARPS][CB_SLOTS]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *vl = vals + warp * CB_SLOTS;
+    uint32_t *tg = tags + warp * CB_SLOTS;
+    uint8_t *cl = claim + warp * CB_SLOTS;
+    const int64_t nquads = (n + 3) / 4;
+    const int64_t stride = (int64_t)gridDim.x * CB_NT;
+    for (int64_t lo = 0; lo < w; lo += CB_PART) {
+        const int nb = (int)min((int64_t)CB_PART, w - lo);
+        for (int i = threadIdx.x; i < nb; i += CB_NT) table[i] = OP::neutral();
+        for (int s = lane; s < CB_SLOTS; s += 32) {
+            vl[s] = OP::neutral();
+            tg[s] = CB_EMPTY;
+        }
         __syncthreads();
-        for (int64_t q = blockIdx.x * (int64_t)MUL_NT + threadIdx.x; q * 4 < n; q += stride) {
-            int64_t k[4];
-            float v[4];
-            const int cnt = load_keys4(is, q * 4, n, k);
-            load_vals4(vs, q * 4, cnt, v);
+        int64_t qw = blockIdx.x * (int64_t)CB_NT + warp * 32;
+        int64_t k[4] = {-1, -1, -1, -1};
+        float v[4] = {0.f, 0.f, 0.f, 0.f};
+        if (qw < nquads) {
+            const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
+            load_vals4(vs, (qw + lane) * 4, cnt, v);
+        }
+        while (qw < nquads) {
+            int64_t kn[4] = {-1, -1, -1, -1};
+            float vn[4] = {0.f, 0.f, 0.f, 0.f};
+            const int64_t qn = qw + stride;
+            if (qn < nquads) {
+                const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
+                load_vals4(vs, (qn + lane) * 4, cnt, vn);
+            }
 #pragma unroll
             for (int j = 0; j < 4; j++) {
-                const int64_t b = k[j] - lo;
-                if ((uint64_t)b >= (uint64_t)nb) continue;  // other partition, or out of range
-                if (v[j] == 0.f) atomicAdd(zeros + k[j], 1u);  // IEEE equality: +-0 only (Q7)
-                else atomic_mul_f32(sh + b, v[j]);
+                const int64_t rel = k[j] - lo;  // other partition, or out of range: not this pass
+                bool act = (uint64_t)rel < (uint64_t)nb;
+                if (COUNT_ZEROS && act && v[j] == 0.f) {
+                    atomicAdd(zeros + k[j], 1u);
+                    act = false;
+                }
+                uint32_t eb = 0;
+                float evv = 0.f;
+                if (claim_update_big<ACC>(act, (uint32_t)rel, v[j], vl, tg, cl, S, lane, eb, evv))
+                    smem_combine<ACC>(table + eb, evv, S);
             }
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                k[j] = kn[j];
+                v[j] = vn[j];
+            }
+            qw = qn;
+        }
+        __syncwarp();
+        for (int s = lane; s < CB_SLOTS; s += 32) {  // write the warp's cache back
+            const uint32_t t = tg[s];
+            if (t != CB_EMPTY) smem_combine<ACC>(table + (t >> 2) * CB_SLOTS + s, vl[s], S);
         }
         __syncthreads();
         float *dst = part + (size_t)blockIdx.x * (size_t)w + lo;
-        for (int k = threadIdx.x; k < nb; k += MUL_NT) dst[k] = sh[k];
+        for (int i = threadIdx.x; i < nb; i += CB_NT) dst[i] = table[i];
         __syncthreads();
     }
 }
+
+// out[k] = fold over the G partial tables, fixed order.
+template <int ACC>
+__global__ void rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part,
+                                       float *__restrict__ out, float S) {
+    for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
+         k += (int64_t)gridDim.x * blockDim.x) {
+        float p = CachedOp<ACC>::neutral();
+        for (int g = 0; g < G; g++) p = CachedOp<ACC>::comb(p, part[(size_t)g * (size_t)w + k], S);
+        out[k] = p;
+    }
+}
+
+constexpr size_t CS_SMEM = (size_t)CS_WARPS * CS_SLOTS * 5;
+constexpr size_t CB_SMEM = (size_t)CB_PART * 4 + (size_t)CB_WARPS * CB_SLOTS * 9;
+
+static int cached_grid(int64_t n, int64_t w) {
+    return w <= CS_SLOTS ? grid_for(n < 1 ? 1 : n, CS_NT, CS_CTAS_PER_SM) : grid_for(n < 1 ? 1 : n, CB_NT, 1);
+}
+static size_t cached_part_bytes(int64_t n, int64_t w) {
+    return align_up((size_t)cached_grid(n, w) * (size_t)(w < 1 ? 1 : w) * 4, 256);
+}
+bool rbi_cached_supported(int64_t w) { return w <= (int64_t)CB_PART * CB_MAX_PASSES; }
+
+// Accumulates into part[G][w]; returns G in *G_out.
+template <int ACC, bool COUNT_ZEROS>
+static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, float *part,
+                      unsigned *zeros, float S, int *G_out, cudaStream_t stream) {
+    const int G = cached_grid(n, w);
+    *G_out = G;
+    if (w <= CS_SLOTS) {
+        auto kern = rbi_cached_small_kernel<ACC, COUNT_ZEROS>;
+        VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CS_NT, CS_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
+    } else {
+        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS>;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CB_SMEM) != cudaSuccess)
+            return VJP_ERR_CUDA;
+        VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CB_NT, CB_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
+    }
+    return last_launch_status();
+}
+
+static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                                float *hist, void *ws, float S, cudaStream_t stream) {
+    if (w == 0) return VJP_OK;
+    if (!rbi_cached_supported(w)) return VJP_ERR_UNSUPPORTED;
+    float *part = static_cast<float *>(ws);
+    int G = 0;
+    const int rc = code == VJP_OP_MUL
+                       ? run_cached<ACC_MUL, false>(n, w, is, vs, part, nullptr, S, &G, stream)
+                       : run_cached<ACC_SATADD, false>(n, w, is, vs, part, nullptr, S, &G, stream);
+    if (rc != VJP_OK) return rc;
+    const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
+    if (code == VJP_OP_MUL)
+        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL><<<fb, 256, 0, stream>>>(w, G, part, hist, S);
+    else
+        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD><<<fb, 256, 0, stream>>>(w, G, part, hist, S);
+    return last_launch_status();
+}
+
+// ------------------------------------------------------------------ '*' VJP ---------------
+//
+// Lifted primal: per bin (zero count, product of the non-zeros) by the cached accumulation
+// above, then the return sweep.
 
 // Per bin: fold the G partial products (fixed order: deterministic), expose (zeros, prod_nz), and
 // prepare the return sweep's coefficient c_k = prod_nz_k * hist_bar_k with the zero count clamped
@@ -526,14 +790,6 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
-static int mul_grid(int64_t n, int64_t w, int *part_bins, size_t *smem) {
-    *part_bins = (int)(w < MUL_PART ? (w < 1 ? 1 : w) : MUL_PART);
-    *smem = (size_t)*part_bins * sizeof(float);
-    int per_sm = 1;
-    if (*smem <= 24 * 1024) per_sm = 2;  // 2 x 1024 threads fill an SM
-    return grid_for(n, MUL_NT, per_sm);
-}
-
 struct MulWs {
     unsigned *zeros;
     float2 *coef;
@@ -559,16 +815,12 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
             return VJP_ERR_CUDA;
         return VJP_OK;
     }
+    if (!rbi_cached_supported(w)) return VJP_ERR_UNSUPPORTED;
     MulWs m = mul_carve(ws, w);
-    int part_bins;
-    size_t smem;
-    const int G = mul_grid(n, w, &part_bins, &smem);
     if (cudaMemsetAsync(m.zeros, 0, (size_t)w * 4, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    if (smem > 48 * 1024 &&
-        cudaFuncSetAttribute(rbi_mul_lifted_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(MUL_PART * sizeof(float))) != cudaSuccess)
-        return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_MUL_LIFTED, stream) rbi_mul_lifted_kernel<<<G, MUL_NT, smem, stream>>>(n, w, part_bins, is, vs, m.part, m.zeros);
+    int G = 0;
+    const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream);
+    if (rc != VJP_OK) return rc;
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
     VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fb, 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
                                                   vs_bar ? m.coef : nullptr);
@@ -583,20 +835,21 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     return last_launch_status();
 }
 
+// Workspace of the specialised rules; covers reduce_by_index_forward of the same operator too.
 size_t rbi_special_workspace_bytes(int code, int, int64_t n, int64_t w) {
     if (w < 1) w = 1;
     switch (code) {
     case VJP_OP_MIN:
     case VJP_OP_MAX: return align_up((size_t)w * 8, 256);
-    case VJP_OP_MUL: {
-        int part_bins;
-        size_t smem;
-        const int G = mul_grid(n < 1 ? 1 : n, w, &part_bins, &smem);
-        return align_up((size_t)w * 4, 256) + align_up((size_t)w * 8, 256) +
-               align_up((size_t)G * (size_t)w * 4, 256);
-    }
+    case VJP_OP_MUL:
+        return align_up((size_t)w * 4, 256) + align_up((size_t)w * 8, 256) + cached_part_bytes(n, w);
     default: return 256;
     }
+}
+size_t rbi_forward_workspace_bytes(int code, int64_t n, int64_t w) {
+    if (code == VJP_OP_MUL || code == VJP_OP_SATADD) return cached_part_bytes(n, w);
+    if (code == VJP_OP_MIN || code == VJP_OP_MAX) return align_up((size_t)(w < 1 ? 1 : w) * 8, 256);
+    return 256;
 }
 
 }  // namespace vjp
