@@ -159,55 +159,78 @@ struct BlockScan {
 
 // ------------------------------------------------------------------ decoupled look-back -
 //
-// Tile status of processing-order tile p: flags[p] in {EMPTY, AGG, PREFIX}; agg[p] / incl[p]
-// hold the tile aggregate / the inclusive prefix through tile p.  Writers publish the payload
-// with L2 stores, then release-store the flag; readers acquire-load the flag, then read the
-// payload with L2 loads.  Tiles take their processing index from an atomic ticket, so every
-// predecessor of a running tile is itself running or finished (forward progress).
+// Tile status of processing-order tile p: one slot of WP 64-bit words, each word = (flag << 32) |
+// one 32-bit word of the payload, flag in {0 = empty, TILE_AGG, TILE_PREFIX}.  A 64-bit store is
+// single-copy atomic, so every word carries its own validity: a reader that finds the same non-zero
+// flag in all words of a slot has a consistent payload -- no fence, no acquire / release, plain
+// relaxed loads and stores through L2 (the first version published payload -> __threadfence ->
+// st.release and polled with ld.acquire: two MEMBARs per publish and a CCTL.IVALL per poll made the
+// look-back 2/3 of a tile's lifetime, profiles/r1a).  The aggregate and, later, the inclusive prefix
+// of a tile go to the SAME slot; a reader that catches the overwrite half-way sees mixed flags and
+// polls again.  Tiles take their processing index from an atomic ticket, so every predecessor of a
+// running tile is itself running or finished (forward progress).
 
-enum : int { TILE_EMPTY = 0, TILE_AGG = 1, TILE_PREFIX = 2 };
+enum : uint32_t { TILE_EMPTY = 0, TILE_AGG = 1, TILE_PREFIX = 2 };
 
-template <class S>
-struct TileStatus {
-    int *flags;  // [num_tiles], zeroed before the launch
-    S *agg;      // [num_tiles]
-    S *incl;     // [num_tiles]
-};
-
-template <class S>
-VJP_DEVINL void publish_tile(const TileStatus<S> &st, int p, const S &value, bool is_prefix) {
-    store_state_cg((is_prefix ? st.incl : st.agg) + p, value);
-    __threadfence();
-    st_release_s32(st.flags + p, is_prefix ? TILE_PREFIX : TILE_AGG);
+VJP_DEVINL void st_relaxed_u64(uint64_t *p, uint64_t v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+VJP_DEVINL void ld_relaxed_v2u64(const uint64_t *p, uint64_t &a, uint64_t &b) {
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
 }
 
+template <class S>
+struct TileSlots {
+    static constexpr int W = sizeof(S) / 4;
+    static constexpr int WP = (W + 1) & ~1;  // 64-bit words per slot (16-byte aligned slots)
+    uint64_t *slots;                         // [num_tiles][WP], zeroed before the launch
+
+    // Called by all lanes of one warp; `words` (shared memory) holds the payload.
+    VJP_DEVINL void publish(int p, const uint32_t *words, uint32_t flag) const {
+        uint64_t *slot = slots + (size_t)p * WP;
+        for (int i = threadIdx.x & 31; i < WP; i += 32)
+            st_relaxed_u64(slot + i, ((uint64_t)flag << 32) | (i < W ? words[i] : 0u));
+    }
+    // Returns the slot's flag (0 if empty or inconsistent) and its payload.
+    VJP_DEVINL uint32_t load(int q, S &out) const {
+        const uint64_t *slot = slots + (size_t)q * WP;
+        uint32_t *o = reinterpret_cast<uint32_t *>(&out);
+        uint32_t f_and = ~0u, f_or = 0u;
+#pragma unroll
+        for (int i = 0; i < WP; i += 2) {
+            uint64_t a, b;
+            ld_relaxed_v2u64(slot + i, a, b);
+            o[i] = (uint32_t)a;
+            if (i + 1 < W) o[i + 1] = (uint32_t)b;
+            f_and &= (uint32_t)(a >> 32) & (uint32_t)(b >> 32);
+            f_or |= (uint32_t)(a >> 32) | (uint32_t)(b >> 32);
+        }
+        return f_and == f_or ? f_or : 0u;
+    }
+};
+
 // Called by ALL 32 lanes of one warp.  Returns (in every lane) the fold of tiles 0..p-1 in
-// processing order.  `LoadAgg(q)` / `LoadIncl(q)` fetch the payloads of tile q.
-template <class M, class LoadAgg, class LoadIncl>
-VJP_DEVINL typename M::State lookback_warp(const int *flags, int p, LoadAgg load_agg,
-                                           LoadIncl load_incl) {
+// processing order.
+template <class M>
+VJP_DEVINL typename M::State lookback_warp(const TileSlots<typename M::State> &ts, int p) {
     using S = typename M::State;
     const int lane = threadIdx.x & 31;
     S acc = M::identity();
     int base = p - 1;
     while (true) {
         const int q = base - lane;
-        int f = TILE_PREFIX;  // tiles before the first one: an identity prefix
-        if (q >= 0) {
-            f = ld_acquire_s32(flags + q);
-        }
+        uint32_t f = TILE_PREFIX;  // tiles before the first one: an identity prefix
+        S s = M::identity();
+        if (q >= 0) f = ts.load(q, s);
         while (__any_sync(FULL_MASK, f == TILE_EMPTY)) {
             if (f == TILE_EMPTY) {
-                __nanosleep(32);
-                f = ld_acquire_s32(flags + q);
+                __nanosleep(20);
+                f = ts.load(q, s);
             }
         }
         const unsigned pm = __ballot_sync(FULL_MASK, f == TILE_PREFIX);
         const int first = __ffs(pm) - 1;  // nearest tile with a full prefix; -1 if none
-        S s = M::identity();
-        if (first < 0 || lane <= first) {
-            if (q >= 0) s = (f == TILE_PREFIX) ? load_incl(q) : load_agg(q);
-        }
+        if (first >= 0 && lane > first) s = M::identity();
         // ordered fold over the window: higher lanes are earlier tiles
 #pragma unroll
         for (int off = 1; off < 32; off <<= 1) {

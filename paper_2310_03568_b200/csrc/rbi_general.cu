@@ -33,9 +33,6 @@ VJP_DEVINL uint64_t ld_relaxed_u64(const uint64_t *p) {
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
-VJP_DEVINL void st_relaxed_u64(uint64_t *p, uint64_t v) {
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
 VJP_DEVINL uint64_t shfl_u64(uint64_t v, int src) {
     const uint32_t lo = __shfl_sync(FULL_MASK, (uint32_t)v, src);
     const uint32_t hi = __shfl_sync(FULL_MASK, (uint32_t)(v >> 32), src);

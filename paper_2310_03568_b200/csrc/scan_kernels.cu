@@ -25,46 +25,42 @@ enum : int { MODE_SCAN = 0, MODE_TILEPRE = 1 };
 template <class S>
 struct LookbackWs {
     int *ticket;
-    TileStatus<S> st;
+    TileSlots<S> ts;
 };
 
 constexpr size_t WS_ALIGN = 256;
 
+// ticket word (padded to WS_ALIGN) + the slots: one contiguous region, zeroed by one memset
 template <class S>
 static size_t lookback_bytes(int64_t num_tiles) {
-    return align_up(sizeof(int) * (size_t)(num_tiles + 1), WS_ALIGN) +
-           2 * align_up(sizeof(S) * (size_t)num_tiles, WS_ALIGN);
+    return WS_ALIGN + align_up(sizeof(uint64_t) * TileSlots<S>::WP * (size_t)num_tiles, WS_ALIGN);
 }
-// Carves ticket + flags (contiguous: one memset) and the two payload arrays out of `base`.
 template <class S>
 static LookbackWs<S> lookback_carve(char *base, int64_t num_tiles, size_t *zero_bytes) {
     LookbackWs<S> w;
     w.ticket = reinterpret_cast<int *>(base);
-    w.st.flags = w.ticket + 1;
-    *zero_bytes = align_up(sizeof(int) * (size_t)(num_tiles + 1), WS_ALIGN);
-    char *p = base + *zero_bytes;
-    w.st.agg = reinterpret_cast<S *>(p);
-    p += align_up(sizeof(S) * (size_t)num_tiles, WS_ALIGN);
-    w.st.incl = reinterpret_cast<S *>(p);
+    w.ts.slots = reinterpret_cast<uint64_t *>(base + WS_ALIGN);
+    *zero_bytes = lookback_bytes<S>(num_tiles);
     return w;
 }
 
 // Warp 0 of the block: publish the tile aggregate, look back, publish the inclusive prefix.
 // Returns (in every lane of warp 0) the fold of all tiles processed before tile p.
+// `words`: sizeof(State) bytes of shared memory.
 template <class M>
-VJP_DEVINL typename M::State tile_prefix_warp0(const TileStatus<typename M::State> &st, int p,
-                                               const typename M::State &total) {
+VJP_DEVINL typename M::State tile_prefix_warp0(const TileSlots<typename M::State> &ts, int p,
+                                               const typename M::State &total, uint32_t *words) {
     using S = typename M::State;
     const int lane = threadIdx.x & 31;
-    if (p == 0) {
-        if (lane == 0) publish_tile(st, 0, total, true);
-        return M::identity();
-    }
-    if (lane == 0) publish_tile(st, p, total, false);
-    S pre = lookback_warp<M>(
-        st.flags, p, [&](int q) { return load_state_cg(st.agg + q); },
-        [&](int q) { return load_state_cg(st.incl + q); });
-    if (lane == 0) publish_tile(st, p, M::combine(pre, total), true);
+    if (lane == 0) store_state_smem(words, total);
+    __syncwarp();
+    ts.publish(p, words, p == 0 ? TILE_PREFIX : TILE_AGG);
+    if (p == 0) return M::identity();
+    const S pre = lookback_warp<M>(ts, p);
+    __syncwarp();
+    if (lane == 0) store_state_smem(words, M::combine(pre, total));
+    __syncwarp();
+    ts.publish(p, words, TILE_PREFIX);
     return pre;
 }
 
@@ -112,7 +108,8 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     S ex = BS::template exclusive<REV>(acc, total, scratch);
 
     if (threadIdx.x < 32) {
-        S pre = tile_prefix_warp0<M>(ws.st, p, total);
+        S pre = tile_prefix_warp0<M>(ws.ts, p, total, bcast);
+        __syncwarp();
         if (threadIdx.x == 0) store_state_smem(bcast, pre);
     }
     __syncthreads();
@@ -204,7 +201,8 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
 
     if (threadIdx.x < 32) {
-        RS pre = tile_prefix_warp0<RM>(ws.st, p, rtotal);
+        RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
+        __syncwarp();
         if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
     }
     __syncthreads();
@@ -249,7 +247,7 @@ static size_t vjp_smem_bytes() {
     using RBS = BlockScan<RevMonoid<Op>, NT>;
     using FBS = BlockScan<FwdMonoid<Op>, NT>;
     constexpr int SCR = RBS::SMEM_WORDS > FBS::SMEM_WORDS ? RBS::SMEM_WORDS : FBS::SMEM_WORDS;
-    return 2 * St::SMEM_BYTES + (SCR + sizeof(typename Op::Adj) / 4) * 4;
+    return 2 * St::SMEM_BYTES + (SCR + sizeof(typename RevMonoid<Op>::State) / 4) * 4;
 }
 
 static int64_t tiles_of(int64_t n, int tile) { return (n + tile - 1) / tile; }
