@@ -33,7 +33,7 @@ constexpr size_t WS_ALIGN = 256;
 // ticket word (padded to WS_ALIGN) + the slots: one contiguous region, zeroed by one memset
 template <class S>
 static size_t lookback_bytes(int64_t num_tiles) {
-    return WS_ALIGN + align_up(sizeof(uint64_t) * TileSlots<S>::WP * (size_t)num_tiles, WS_ALIGN);
+    return WS_ALIGN + align_up(sizeof(uint64_t) * TileSlots<S>::STRIDE * (size_t)num_tiles, WS_ALIGN);
 }
 template <class S>
 static LookbackWs<S> lookback_carve(char *base, int64_t num_tiles, size_t *zero_bytes) {
@@ -317,12 +317,12 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
 }
 
 // tile shapes: rows of 16 words (plain scans) / 8 words (VJP: two staged arrays + more live state)
-using CfgAddF32 = ScanCfg<OpAdd<float>, 256, 16, 256, 16>;
-using CfgAddF64 = ScanCfg<OpAdd<double>, 256, 8, 256, 8>;
-using CfgMulF32 = ScanCfg<OpMul<float>, 256, 16, 256, 8>;
-using CfgMulF64 = ScanCfg<OpMul<double>, 256, 8, 256, 4>;
-using CfgLinRec = ScanCfg<OpLinRec<float>, 256, 8, 256, 4>;
-using CfgMat2 = ScanCfg<OpMatMul<2, float, double, double>, 256, 4, 256, 2>;
+using CfgAddF32 = ScanCfg<OpAdd<float>, 512, 32, 512, 32>;
+using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
+using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
+using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 512, 8>;
+using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 512, 8>;
+using CfgMat2 = ScanCfg<OpMatMul<2, float, double, double>, 512, 8, 512, 4>;
 using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 1, 128, 1>;
 
 #define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
