@@ -90,8 +90,14 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     Op::identity_words(fill);
     St::load(smem, in + base * EW, valid * EW, fill);
     __syncthreads();
-    uint32_t r[RW];
-    St::read_row(smem, threadIdx.x, r);
+    // WIDE elements (the 25-word 5x5 matrix) stay in shared memory and are read element by element;
+    // narrow ones are held in registers as a whole row.
+    constexpr bool WIDE = EW > 8;
+    static_assert(!WIDE || RW % 4 != 0, "wide elements use the linear tile layout");
+    uint32_t rr[WIDE ? 1 : RW];
+    uint32_t *r = rr;
+    if constexpr (WIDE) r = reinterpret_cast<uint32_t *>(smem) + threadIdx.x * RW;
+    else St::read_row(smem, threadIdx.x, rr);
 
     // thread-local fold in processing order
     S acc;
@@ -134,7 +140,7 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
             Op::to_elem(run, r + j * EW);
         }
     }
-    St::write_row(smem, threadIdx.x, r);
+    if constexpr (!WIDE) St::write_row(smem, threadIdx.x, rr);
     __syncthreads();
     St::store(smem, out + base * EW, valid * EW);
 }
@@ -179,9 +185,17 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     St::load(sx, xs + base * EW, valid * EW, fillx);
     St::load(sy, ybar + base * EW, valid * EW, filly);
     __syncthreads();
-    uint32_t rx[RW], ry[RW];
-    St::read_row(sx, threadIdx.x, rx);
-    St::read_row(sy, threadIdx.x, ry);
+    constexpr bool WIDE = EW > 8;
+    static_assert(!WIDE || RW % 4 != 0, "wide elements use the linear tile layout");
+    uint32_t rrx[WIDE ? 1 : RW], rry[WIDE ? 1 : RW];
+    uint32_t *rx = rrx, *ry = rry;
+    if constexpr (WIDE) {
+        rx = reinterpret_cast<uint32_t *>(sx) + threadIdx.x * RW;
+        ry = reinterpret_cast<uint32_t *>(sy) + threadIdx.x * RW;
+    } else {
+        St::read_row(sx, threadIdx.x, rrx);
+        St::read_row(sy, threadIdx.x, rry);
+    }
 
     // thread-local reduce, walking the thread's elements from the highest index down
     Adj bacc = Op::adj_zero();
@@ -208,20 +222,37 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     __syncthreads();
     const Adj ztile = load_state_smem<Adj>(bcast);  // u entering the tile from the right
 
-    // forward prefixes r_{i-1} of the thread's elements
-    FS rp[IPT];
-    rp[0] = Op::combine(load_state_cg(fpre + t), fex);
-#pragma unroll
-    for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
-
     Adj u = Op::adj_add(rex.b, Op::adj_mul(ztile, rex.l));
+    if constexpr (WIDE) {
+        // descending: rbar_j replaces ybar_j in shared memory; ascending: the forward prefix runs
+        // along and xbar_j replaces rbar_j (keeps one prefix in registers instead of IPT)
+#pragma unroll 1
+        for (int j = IPT - 1; j >= 0; j--) {
+            const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);
+            u = Op::adj_mul(rbar, Op::lin_of(Op::from_elem(rx + j * EW)));
+            Op::adj_to_elem(rbar, ry + j * EW);
+        }
+        FS rp = Op::combine(load_state_cg(fpre + t), fex);
+#pragma unroll 1
+        for (int j = 0; j < IPT; j++) {
+            const Adj rbar = Op::adj_from_elem(ry + j * EW);
+            Op::xbar(rp, rbar, ry + j * EW);
+            if (j + 1 < IPT) rp = Op::combine(rp, Op::from_elem(rx + j * EW));
+        }
+    } else {
+        // forward prefixes r_{i-1} of the thread's elements
+        FS rp[IPT];
+        rp[0] = Op::combine(load_state_cg(fpre + t), fex);
 #pragma unroll
-    for (int j = IPT - 1; j >= 0; j--) {
-        const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);
-        u = Op::adj_mul(rbar, Op::lin_of(Op::from_elem(rx + j * EW)));
-        Op::xbar(rp[j], rbar, ry + j * EW);
+        for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
+#pragma unroll
+        for (int j = IPT - 1; j >= 0; j--) {
+            const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);
+            u = Op::adj_mul(rbar, Op::lin_of(Op::from_elem(rx + j * EW)));
+            Op::xbar(rp[j], rbar, ry + j * EW);
+        }
+        St::write_row(sy, threadIdx.x, rry);
     }
-    St::write_row(sy, threadIdx.x, ry);
     __syncthreads();
     St::store(sy, xbar + base * EW, valid * EW);
 }
@@ -323,7 +354,7 @@ using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 512, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 512, 8>;
 using CfgMat2 = ScanCfg<OpMatMul<2, float, double, double>, 512, 8, 512, 4>;
-using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 1, 128, 1>;
+using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 128, 3>;
 
 #define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
     switch (code) {                                                                          \

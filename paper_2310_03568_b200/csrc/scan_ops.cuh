@@ -172,6 +172,10 @@ struct OpMatMul {
         for (int i = 0; i < D; i++) a.m[i] = (AA)word_to(w + i * WordsOf<T>::value, (T *)nullptr);
         return a;
     }
+    static VJP_DEVINL void adj_to_elem(const Adj &a, uint32_t *w) {
+#pragma unroll
+        for (int i = 0; i < D; i++) to_word((T)a.m[i], w + i * WordsOf<T>::value);
+    }
     static VJP_DEVINL Adj adj_add(const Adj &x, const Adj &y) {
         Adj a;
 #pragma unroll
