@@ -33,7 +33,7 @@ WORKLOAD = ("c2: reduce-by-index VJP, ops min and *, f32, n=2^24, w in {2^10, 2^
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--configs", default="all", choices=["all", "none"],
@@ -143,10 +143,7 @@ def run_ours(args):
             fn()
         b.record()
         barrier()
-        ms = torch.tensor([a.elapsed_time(b) / steps], device="cuda", dtype=torch.float64)
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return L.max_over_ranks(a.elapsed_time(b) / steps, device="cuda")
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -155,12 +152,12 @@ def run_ours(args):
     ms_step = timed(step, args.steps)
     launches = (B.launch_count() - l0) // args.steps
     clocks = sampler.stop() if sampler else None
-    value = world * elems_per_step / (ms_step * 1e-3) / 1e9
+    value = L.whole_job_throughput(elems_per_step, world, ms_step)
 
     # end to end: host buffers, H2D + kernels + D2H inside the timed region (the *_host entry points)
     step_host()
     ms_e2e = timed(step_host, args.steps)
-    e2e = {"value": world * elems_per_step / (ms_e2e * 1e-3) / 1e9, "unit": UNIT,
+    e2e = {"value": L.whole_job_throughput(elems_per_step, world, ms_e2e), "unit": UNIT,
            "h2d_bytes_per_step": sum(c.h2d_bytes() for c in cases),
            "d2h_bytes_per_step": sum(c.d2h_bytes() for c in cases), "ms_per_step": ms_e2e}
 

@@ -66,53 +66,80 @@ def event_time_ms(fn, reps: int, warmup: int = 3):
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons while a timed region runs."""
-    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-             "clocks_event_reasons.sw_power_cap")
+    """Samples SM clocks and throttle reasons while a timed region runs: NVML in a thread (a few ms
+    per sample: the timed region of the default run is well under a second), nvidia-smi as fallback."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
-    def __init__(self, index: int = 0, period_ms: int = 100):
-        self.lines = []
-        self.proc = None
+    def __init__(self, index: int = 0, period_ms: float = 5.0):
+        self.sm, self.mask, self.power = [], 0, []
+        self.max_mhz = None
+        self._stop = threading.Event()
         self.thread = None
+        self.source = "none"
         try:
-            self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.QUERY, "--format=csv,noheader,nounits",
-                 "-lms", str(period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.period = period_ms / 1e3
+            self.source = "nvml"
             self.thread = threading.Thread(target=self._pump, daemon=True)
             self.thread.start()
         except Exception:
-            self.proc = None
+            self.nv = None
+
+    def _sample(self):
+        nv = self.nv
+        self.sm.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+        try:
+            self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        try:
+            self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1e3)
+        except Exception:
+            pass
 
     def _pump(self):
-        for line in self.proc.stdout:
-            self.lines.append(line.strip())
+        while not self._stop.is_set():
+            try:
+                self._sample()
+            except Exception:
+                break
+            self._stop.wait(self.period)
 
     def stop(self):
-        if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ln in self.lines:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 7:
-                continue
+        if self.thread is not None:
+            self._stop.set()
+            self.thread.join(timeout=2)
+        if not self.sm:  # NVML unavailable: one nvidia-smi query
             try:
-                sm.append(float(f[0]))
-                mx.append(float(f[1]))
-            except ValueError:
-                continue
-            for nm, val in zip(names, f[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": statistics.median(sm) if sm else None,
-                "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                out = subprocess.run(["nvidia-smi", "--query-gpu=clocks.sm,clocks.max.sm", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=20).stdout.split("\n")[0].split(",")
+                self.sm, self.max_mhz, self.source = [float(out[0])], float(out[1]), "nvidia-smi (after the region)"
+            except Exception:
+                pass
+        reasons = sorted(name for bit, name in self.REASONS.items() if self.mask & bit)
+        return {"sm_mhz": statistics.median(self.sm) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(self.sm), "source": self.source,
+                "power_w_max": max(self.power) if self.power else None}
+
+
+def max_over_ranks(ms: float, device="cpu") -> float:
+    """The slowest rank's time (the only cross-rank step of the bench: the path itself shards by
+    independent problems and has no collective).  No-op without an initialised process group."""
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_throughput(elems_per_rank: int, world: int, ms_max: float) -> float:
+    """Gelem/s of the whole job: every rank's elements over the slowest rank's time (weak scaling)."""
+    return world * elems_per_rank / (ms_max * 1e-3) / 1e9
 
 
 def to_dev(a):
