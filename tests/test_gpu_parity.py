@@ -16,7 +16,9 @@ from paper_2310_03568_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL = {torch.float32: 1e-4, torch.float64: 1e-10}
-SIZES = [1, 2, 33, 127, 128, 129, 511, 513, 1023, 1025, 2047, 2049, 4095, 4096, 4097, 12345, 100003]
+# tile shapes in use: 384 / 640 (5x5), 2048 ... 16384 elements
+SIZES = [1, 2, 33, 127, 128, 129, 383, 384, 385, 511, 513, 639, 640, 641, 1023, 1025, 2047, 2049, 4095, 4096, 4097,
+         8191, 8192, 8193, 12345, 16383, 16384, 16385, 32769, 100003, 300007]
 
 
 def dev(a):
@@ -71,6 +73,10 @@ SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "linre
 @pytest.mark.parametrize("n", SIZES)
 @pytest.mark.parametrize("name", SCAN_OPS)
 def test_scan_vjp_matches_oracle(name, n):
+    if name == "mul_f32" and n > 100003:
+        # a chain of 3e5 unit-gain f32 products carries eps*sqrt(n)-sized rounding of its own, at the 1e-4
+        # bar whatever the association order (Q27); BASELINE runs scan '*' in f64
+        pytest.skip("f32 product chain longer than the f32 tolerance allows")
     op, oname, q, xs, ys_bar = scan_inputs(name, n)
     got = B.vjp_scan(op, dev(xs), dev(ys_bar)).cpu().numpy()
     ref = oracle.vjp_scan(oname, xs, ys_bar, q=q)
