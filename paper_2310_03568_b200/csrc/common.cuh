@@ -328,6 +328,10 @@ struct TileStage {
         }
     }
 
+    // A row is contiguous in shared memory (the padding sits between rows).
+    static VJP_DEVINL uint32_t *row_ptr(uint4 *smem, int row) {
+        return reinterpret_cast<uint32_t *>(smem + row * PITCH_C);
+    }
     // Row access for the owning thread: whole row <-> registers.
     static VJP_DEVINL void read_row(const uint4 *smem, int row, uint32_t (&r)[RW]) {
 #pragma unroll
@@ -381,6 +385,9 @@ struct TileStageLinear {
             const uint32_t *s = reinterpret_cast<const uint32_t *>(smem);
             for (int wi = threadIdx.x; wi < valid_words; wi += NT) g[wi] = s[wi];
         }
+    }
+    static VJP_DEVINL uint32_t *row_ptr(uint4 *smem, int row) {
+        return reinterpret_cast<uint32_t *>(smem) + row * RW;
     }
     static VJP_DEVINL void read_row(const uint4 *smem, int row, uint32_t (&r)[RW]) {
         const uint32_t *s = reinterpret_cast<const uint32_t *>(smem) + row * RW;

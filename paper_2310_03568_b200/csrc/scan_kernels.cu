@@ -93,10 +93,9 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     // WIDE elements (the 25-word 5x5 matrix) stay in shared memory and are read element by element;
     // narrow ones are held in registers as a whole row.
     constexpr bool WIDE = EW > 8;
-    static_assert(!WIDE || RW % 4 != 0, "wide elements use the linear tile layout");
     uint32_t rr[WIDE ? 1 : RW];
     uint32_t *r = rr;
-    if constexpr (WIDE) r = reinterpret_cast<uint32_t *>(smem) + threadIdx.x * RW;
+    if constexpr (WIDE) r = St::row_ptr(smem, threadIdx.x);
     else St::read_row(smem, threadIdx.x, rr);
 
     // thread-local fold in processing order
@@ -186,12 +185,11 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     St::load(sy, ybar + base * EW, valid * EW, filly);
     __syncthreads();
     constexpr bool WIDE = EW > 8;
-    static_assert(!WIDE || RW % 4 != 0, "wide elements use the linear tile layout");
     uint32_t rrx[WIDE ? 1 : RW], rry[WIDE ? 1 : RW];
     uint32_t *rx = rrx, *ry = rry;
     if constexpr (WIDE) {
-        rx = reinterpret_cast<uint32_t *>(sx) + threadIdx.x * RW;
-        ry = reinterpret_cast<uint32_t *>(sy) + threadIdx.x * RW;
+        rx = St::row_ptr(sx, threadIdx.x);
+        ry = St::row_ptr(sy, threadIdx.x);
     } else {
         St::read_row(sx, threadIdx.x, rrx);
         St::read_row(sy, threadIdx.x, rry);
