@@ -278,7 +278,7 @@ def case_table(scale=1.0):
     return t
 
 
-def measure_all_configs(reps, peak_gbs, scale=1.0, log=None, only=None):
+def measure_all_configs(reps, peak_gbs, scale=1.0, log=None, only=None, kernels=False):
     """Every case of case_table(), one at a time; `only` = substrings of the labels to keep."""
     rows = []
     for key, label, make in case_table(scale):
@@ -287,7 +287,17 @@ def measure_all_configs(reps, peak_gbs, scale=1.0, log=None, only=None):
         if log:
             log(label)
         case = make()
-        rows.append(measure_case(key, label, case, reps, peak_gbs))
+        row = measure_case(key, label, case, reps, peak_gbs)
+        if kernels:  # per-kernel CUDA-event times of the VJP call (library instrumentation)
+            B.profile_enable(True)
+            for _ in range(3):
+                case.vjp()
+            torch.cuda.synchronize()
+            prof = B.profile_read()
+            B.profile_enable(False)
+            row["vjp_kernels_ms"] = {k: round(ms / cnt, 4) for k, (ms, cnt) in prof.items()}
+            row["vjp_kernel_launches"] = {k: cnt // 3 for k, (ms, cnt) in prof.items()}
+        rows.append(row)
         del case
         torch.cuda.empty_cache()
     return rows
@@ -302,13 +312,14 @@ def main(argv=None):
     ap.add_argument("--cases", default="")
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--scale", type=float, default=1.0)
+    ap.add_argument("--kernels", action="store_true", help="add the per-kernel times of the VJP call")
     a = ap.parse_args(argv)
     if not torch.cuda.is_available():
         raise SystemExit("needs a CUDA device: there is no CPU path")
     B.load()
     peak, _ = measured_peak()
     only = [s for s in a.cases.split(",") if s] or None
-    for row in measure_all_configs(a.reps, peak, a.scale, only=only):
+    for row in measure_all_configs(a.reps, peak, a.scale, only=only, kernels=a.kernels):
         print(json.dumps(row), flush=True)
 
 

@@ -134,7 +134,10 @@ struct BlockScan {
         const int pwarp = REVT ? NW - 1 - warp : warp;
         __syncthreads();  // scratch may still be read by a previous call
         S incl = local;
-#pragma unroll
+        // wide states (25- and 50-word 5x5 states): keep the loop rolled -- fully unrolled, the 5x5
+        // VJP kernel was 11 400 instructions (182 KB), more than the instruction cache holds, and
+        // ran at 0.17 IPC with "no instruction" stalls (profiles/r1f)
+#pragma unroll(SW > 16 ? 1 : 5)
         for (int off = 1; off < 32; off <<= 1) {
             S o = shfl_state(incl, REVT ? lane + off : lane - off);
             if (plane >= off) incl = M::combine(o, incl);
@@ -148,7 +151,7 @@ struct BlockScan {
             // lane l holds the total of processing-warp l; Kogge-Stone over NW lanes
             S wt = (lane < NW) ? load_state_smem<S>(scratch + lane * SW) : M::identity();
             S wi = wt;
-#pragma unroll
+#pragma unroll(SW > 16 ? 1 : 5)
             for (int off = 1; off < NW; off <<= 1) {
                 S o = shfl_state(wi, lane - off);
                 if (lane >= off) wi = M::combine(o, wi);
@@ -247,7 +250,7 @@ VJP_DEVINL typename M::State lookback_warp(const TileSlots<typename M::State> &t
         const int first = __ffs(pm) - 1;  // nearest tile with a full prefix; -1 if none
         if (first >= 0 && lane > first) s = M::identity();
         // ordered fold over the window: higher lanes are earlier tiles
-#pragma unroll
+#pragma unroll(sizeof(S) > 64 ? 1 : 5)
         for (int off = 1; off < 32; off <<= 1) {
             S o = shfl_state(s, lane + off);
             if (lane + off < 32) s = M::combine(o, s);

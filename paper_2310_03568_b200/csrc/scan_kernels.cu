@@ -198,7 +198,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     // thread-local reduce, walking the thread's elements from the highest index down
     Adj bacc = Op::adj_zero();
     FS facc = Op::identity();
-#pragma unroll
+#pragma unroll(WIDE ? 1 : IPT)
     for (int j = IPT - 1; j >= 0; j--) {
         const FS xj = Op::from_elem(rx + j * EW);
         bacc = Op::adj_mul(Op::adj_add(Op::adj_from_elem(ry + j * EW), bacc), Op::lin_of(xj));
