@@ -676,16 +676,38 @@ rbi_cached_big_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
-// out[k] = fold over the G partial tables, fixed order.
+// Fold of the G per-CTA tables for 32 consecutive bins by a CTA of 256 threads: thread (x, y) folds
+// part[g][k0 + x] for g = y, y + 8, ... (coalesced across x, 8 independent chains per bin), then the
+// 8 chains are combined in a fixed order through shared memory (deterministic).  Returns the result
+// in the threads with y == 0.  One thread per bin walking all G tables was latency-bound (10 % of
+// the bench step in the launch list of profiles/r1g).
+constexpr int FOLD_NT = 256;
 template <int ACC>
-__global__ void rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part,
-                                       float *__restrict__ out, float S) {
-    for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
-         k += (int64_t)gridDim.x * blockDim.x) {
-        float p = CachedOp<ACC>::neutral();
-        for (int g = 0; g < G; g++) p = CachedOp<ACC>::comb(p, part[(size_t)g * (size_t)w + k], S);
-        out[k] = p;
+VJP_DEVINL float fold_partials(int64_t w, int G, const float *__restrict__ part, int64_t k, float S) {
+    __shared__ float sm[8][32];
+    const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
+    float p = CachedOp<ACC>::neutral();
+    if (k < w) {
+#pragma unroll 4
+        for (int g = y; g < G; g += 8) p = CachedOp<ACC>::comb(p, __ldg(part + (size_t)g * (size_t)w + k), S);
     }
+    sm[y][x] = p;
+    __syncthreads();
+    if (y == 0) {
+#pragma unroll
+        for (int i = 1; i < 8; i++) p = CachedOp<ACC>::comb(p, sm[i][x], S);
+    }
+    return p;
+}
+static int fold_grid(int64_t w) { return (int)((w + 31) / 32); }
+
+// out[k] = fold over the G partial tables.
+template <int ACC>
+__global__ void __launch_bounds__(FOLD_NT)
+rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part, float *__restrict__ out, float S) {
+    const int64_t k = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
+    const float p = fold_partials<ACC>(w, G, part, k, S);
+    if (threadIdx.x < 32 && k < w) out[k] = p;
 }
 
 constexpr size_t CS_SMEM = (size_t)CS_WARPS * CS_SLOTS * 5;
@@ -729,9 +751,9 @@ static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *i
     if (rc != VJP_OK) return rc;
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
     if (code == VJP_OP_MUL)
-        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL><<<fb, 256, 0, stream>>>(w, G, part, hist, S);
+        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL><<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, part, hist, S);
     else
-        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD><<<fb, 256, 0, stream>>>(w, G, part, hist, S);
+        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD><<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, part, hist, S);
     return last_launch_status();
 }
 
@@ -743,14 +765,13 @@ static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *i
 // Per bin: fold the G partial products (fixed order: deterministic), expose (zeros, prod_nz), and
 // prepare the return sweep's coefficient c_k = prod_nz_k * hist_bar_k with the zero count clamped
 // to {0, 1, 2}.
-__global__ void rbi_mul_finish_kernel(int64_t w, int G, const float *__restrict__ part,
-                                      const unsigned *__restrict__ zeros_u,
-                                      const float *__restrict__ hist_bar, int64_t *zeros,
-                                      float *prod_nz, float2 *coef) {
-    for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
-         k += (int64_t)gridDim.x * blockDim.x) {
-        float p = 1.f;
-        for (int g = 0; g < G; g++) p *= part[(size_t)g * (size_t)w + k];
+__global__ void __launch_bounds__(FOLD_NT)
+rbi_mul_finish_kernel(int64_t w, int G, const float *__restrict__ part,
+                      const unsigned *__restrict__ zeros_u, const float *__restrict__ hist_bar,
+                      int64_t *zeros, float *prod_nz, float2 *coef) {
+    const int64_t k = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
+    const float p = fold_partials<ACC_MUL>(w, G, part, k, 0.f);
+    if (threadIdx.x < 32 && k < w) {
         const unsigned z = zeros_u[k];
         if (zeros) zeros[k] = (int64_t)z;
         if (prod_nz) prod_nz[k] = p;
@@ -822,7 +843,7 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream);
     if (rc != VJP_OK) return rc;
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
-    VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fb, 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
+    VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
                                                   vs_bar ? m.coef : nullptr);
     if (vs_bar && n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
