@@ -115,8 +115,8 @@ size_t vjp_reduce_by_index_workspace_bytes(const vjp_op_t *op, int64_t n, int64_
 /* Primal reduce_by_index over a neutral-initialised histogram (P:L332-336 after the rewrite of
  * there is no hist_0 argument).  hist[num_bins] is fully written.
  * Supported: ADD (f32, f64), MIN, MAX, MUL, SATADD (f32).  ADD needs no workspace (ws may be NULL);
- * the others return VJP_ERR_WORKSPACE if ws is too small.  MUL and SATADD keep per-CTA tables of at
- * most 8 x 36864 bins: a larger num_bins returns VJP_ERR_UNSUPPORTED. */
+ * the others return VJP_ERR_WORKSPACE if ws is too small.  MUL and SATADD keep shared-memory tables of
+ * 73728 bins per pass over the input, at most 8 passes: a larger num_bins returns VJP_ERR_UNSUPPORTED. */
 int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
                             const void *vs, void *hist, void *ws, size_t ws_bytes, void *stream);
 
@@ -125,7 +125,7 @@ int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, con
  *   MIN/MAX:  lifted primal (index, value) per bin, lowest index on ties (Fig. 5),
  *             then vs_bar = 0 and vs_bar[arg[k]] = hist_bar[k].  Bit-exact copy.
  *   MUL:      lifted primal (zero count, product of non-zeros) (Fig. 3),
- *             then the three-way map of P:L208-219 / P:L243-246.  num_bins <= 8 x 36864, else
+ *             then the three-way map of P:L208-219 / P:L243-246.  num_bins <= 8 x 73728, else
  *             VJP_ERR_UNSUPPORTED (force_general handles any num_bins).
  *   SATADD or force_general: stable radix sort by clamped bin, forward and reverse segmented
  *             exclusive scans, per-element derivative of l (.) x (.) r, un-permute
