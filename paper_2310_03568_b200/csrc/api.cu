@@ -46,7 +46,8 @@ cudaStream_t as_stream(void *s) { return static_cast<cudaStream_t>(s); }
 namespace vjp {
 namespace {
 const char *const KERNEL_NAMES[K_COUNT] = {
-    "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEPRE>", "scan_vjp_reverse_kernel",
+    "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEAGG>",
+    "tile_exscan_kernel", "scan_vjp_reverse_kernel",
     "rbi_fill_kernel", "rbi_forward_kernel", "rbi_vjp_add_kernel",
     "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_cached_kernel",
     "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",

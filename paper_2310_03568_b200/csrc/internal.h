@@ -24,7 +24,7 @@ inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 // Every kernel launch of the library goes through a LaunchScope: it counts the launch and, while
 // profiling is enabled (vjp_profile_enable), brackets it with CUDA events on the launching stream.
 enum KernelId : int {
-    K_SCAN_LOOKBACK = 0, K_SCAN_TILEPRE, K_SCAN_VJP_REVERSE,
+    K_SCAN_LOOKBACK = 0, K_SCAN_TILEAGG, K_SCAN_TILEPRE, K_SCAN_VJP_REVERSE,
     K_RBI_FILL, K_RBI_FORWARD, K_RBI_GATHER,
     K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_ACC, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,

@@ -5,9 +5,12 @@
 //       MODE_SCAN    : out[i] = fold of in[0..i] (REV: of in[i..n-1]) -- the primal inclusive scan
 //                       and, with Op = '+' and REV, the '+' rule of the scan VJP
 //                      (xs_bar = reverse inclusive sum of ys_bar).
-//       MODE_TILEPRE : only the exclusive prefix of every tile is written (fpre[t] = fold of all
-//                      elements before tile t): the forward re-execution the return sweep needs
-//                      (r_{i-1} of P:L613; re-execution instead of a tape).
+//       MODE_TILEAGG : only the aggregate of every tile is written (no look-back: a streaming
+//                      reduction); tile_exscan_kernel turns the aggregates into exclusive tile
+//                      prefixes fpre[t] = fold of all elements before tile t: the forward
+//                      re-execution the return sweep needs (r_{i-1} of P:L613; re-execution
+//                      instead of a tape).  MODE_TILEPRE (prefixes by look-back) is kept
+//                      for reference; the VJP no longer uses it.
 //   scan_vjp_reverse_kernel<Op, NT, IPT>
 //       the general rule of Fig. 7 in one kernel: Jacobians formed on the fly
 //       (never stored), reverse linear-recurrence scan with lin_o
@@ -15,12 +18,14 @@
 //
 // Tile = NT threads x IPT consecutive elements per thread, staged through shared memory with
 // 128-bit coalesced global accesses.  A tile's processing index comes from an atomic ticket.
+#include <cooperative_groups.h>
+
 #include "internal.h"
 #include "scan_ops.cuh"
 
 namespace vjp {
 
-enum : int { MODE_SCAN = 0, MODE_TILEPRE = 1 };
+enum : int { MODE_SCAN = 0, MODE_TILEPRE = 1, MODE_TILEAGG = 2 };
 
 template <class S>
 struct LookbackWs {
@@ -79,9 +84,11 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     uint32_t *bcast = scratch + BS::SMEM_WORDS;
     __shared__ int s_p;
 
-    if (threadIdx.x == 0) s_p = atomicAdd(ws.ticket, 1);
-    __syncthreads();
-    const int p = s_p;
+    if (MODE != MODE_TILEAGG) {
+        if (threadIdx.x == 0) s_p = atomicAdd(ws.ticket, 1);
+        __syncthreads();
+    }
+    const int p = MODE == MODE_TILEAGG ? (int)blockIdx.x : s_p;
     const int t = REV ? num_tiles - 1 - p : p;
     const int64_t base = (int64_t)t * (NT * IPT);
     const int valid = (int)min((int64_t)(NT * IPT), n - base);
@@ -111,6 +118,10 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     }
     S total;
     S ex = BS::template exclusive<REV>(acc, total, scratch);
+    if (MODE == MODE_TILEAGG) {  // aggregate only: no dependency on other tiles, pure streaming
+        if (threadIdx.x == 0) store_state_cg(fpre + t, total);
+        return;
+    }
 
     if (threadIdx.x < 32) {
         S pre = tile_prefix_warp0<M>(ws.ts, p, total, bcast);
@@ -142,6 +153,46 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     if constexpr (!WIDE) St::write_row(smem, threadIdx.x, rr);
     __syncthreads();
     St::store(smem, out + base * EW, valid * EW);
+}
+
+// In-place exclusive scan of the per-tile aggregates (a few thousand states) by ONE thread-block
+// cluster: every CTA scans its contiguous share, the CTA totals are exchanged through distributed
+// shared memory, one cluster barrier.  Together with MODE_TILEAGG this replaces the look-back in the
+// forward re-execution of the VJP, which writes no per-element output and so gains nothing from being
+// single-pass: the aggregate kernel is a pure streaming reduction (linrec: 107 us vs 161 us for the
+// look-back version), the cluster scan takes a few microseconds (a single CTA took 68 - 435 us).
+constexpr int XCL = 8;  // portable cluster size
+template <class Op, int NT>
+__global__ void __launch_bounds__(NT)
+tile_exscan_kernel(int num_tiles, typename Op::Fwd *__restrict__ fpre) {
+    namespace cg = cooperative_groups;
+    using M = FwdMonoid<Op>;
+    using S = typename Op::Fwd;
+    using BS = BlockScan<M, NT>;
+    constexpr int SW = sizeof(S) / 4;
+    __shared__ uint32_t scratch[BS::SMEM_WORDS];
+    __shared__ uint32_t tot[XCL][SW];
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
+    const int per = (num_tiles + XCL * NT - 1) / (XCL * NT);
+    const int lo = min((rank * NT + (int)threadIdx.x) * per, num_tiles), hi = min(lo + per, num_tiles);
+    S acc = Op::identity();
+    for (int i = lo; i < hi; i++) acc = Op::combine(acc, load_state_cg(fpre + i));
+    S total;
+    const S ex = BS::template exclusive<false>(acc, total, scratch);
+    if (threadIdx.x < XCL) {  // thread r delivers this CTA's total to CTA r
+        uint32_t *dst = cluster.map_shared_rank(&tot[0][0], threadIdx.x) + rank * SW;
+        store_state_smem(dst, total);
+    }
+    cluster.sync();
+    S run = Op::identity();
+    for (int r = 0; r < rank; r++) run = Op::combine(run, load_state_smem<S>(&tot[r][0]));
+    run = Op::combine(run, ex);
+    for (int i = lo; i < hi; i++) {
+        const S a = load_state_cg(fpre + i);
+        store_state_cg(fpre + i, run);
+        run = Op::combine(run, a);
+    }
 }
 
 // The fused reverse kernel of the scan VJP.  With u_i = rbar_i * X_i^T ("what element i hands to
@@ -288,13 +339,13 @@ static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre
     const int64_t nt = tiles_of(n, NT * IPT);
     size_t zero_bytes;
     LookbackWs<S> lw = lookback_carve<S>(ws, nt, &zero_bytes);
-    if (cudaMemsetAsync(ws, 0, zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    if (MODE != MODE_TILEAGG && cudaMemsetAsync(ws, 0, zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
     auto kern = scan_lookback_kernel<Op, NT, IPT, REV, MODE>;
     const size_t smem = scan_smem_bytes<Op, NT, IPT>();
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
-    VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : K_SCAN_TILEPRE, stream)
+    VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : (MODE == MODE_TILEAGG ? K_SCAN_TILEAGG : K_SCAN_TILEPRE), stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(in),
                                              static_cast<uint32_t *>(out), n, (int)nt, lw, fpre);
     return last_launch_status();
@@ -326,9 +377,25 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     char *ws_fwd = ws;
     char *ws_rev = ws_fwd + lookback_bytes<FS>(nt);
     FS *fpre = reinterpret_cast<FS *>(ws_rev + lookback_bytes<RS>(nt));
-    // (A) forward tile prefixes
-    int rc = run_scan<Op, NT, IPT, false, MODE_TILEPRE>(n, xs, nullptr, fpre, ws_fwd, stream);
+    // (A) forward tile prefixes: streaming per-tile aggregates, then their exclusive scan by one cluster
+    int rc;
+    rc = run_scan<Op, NT, IPT, false, MODE_TILEAGG>(n, xs, nullptr, fpre, ws_fwd, stream);
     if (rc != VJP_OK) return rc;
+    constexpr int XNT = sizeof(FS) > 32 ? 128 : 512;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(XCL);
+    cfg.blockDim = dim3(XNT);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = XCL;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    VJP_LAUNCH(K_SCAN_TILEPRE, stream) {
+        if (cudaLaunchKernelEx(&cfg, tile_exscan_kernel<Op, XNT>, (int)nt, fpre) != cudaSuccess) return VJP_ERR_CUDA;
+    }
     // (B) fused reverse kernel
     size_t zero_bytes;
     LookbackWs<RS> lw = lookback_carve<RS>(ws_rev, nt, &zero_bytes);
