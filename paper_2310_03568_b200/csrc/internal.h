@@ -51,7 +51,7 @@ int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *
 // -------------------------------------------------------------- reduce-by-index (special) -
 size_t rbi_special_workspace_bytes(int code, int dtype, int64_t n, int64_t w);
 size_t rbi_forward_workspace_bytes(int code, int64_t n, int64_t w);
-bool rbi_cached_supported(int64_t w);  // '*' / satadd tables: at most 8 passes over the input
+bool rbi_cached_supported(int64_t w);  // '*' / satadd tables: w <= 2^20
 int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, const int64_t *is,
                        const void *vs, void *hist, void *ws, cudaStream_t stream);
 int launch_rbi_vjp_add(int dtype, int64_t n, int64_t w, const int64_t *is, const void *hist_bar,

@@ -461,16 +461,19 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
 //   2. hit: combine in place.  Miss: a 2-bit hit counter guards the resident entry -- a cold bin
 //      arriving at a hot slot decrements it and BYPASSES; only an entry whose counter has run out
 //      is evicted (Misra-Gries style), so hot bins stay resident whatever the key distribution;
-//   3. evictions / bypasses go to the CTA's table in shared memory with a CAS loop (cold bins only:
-//      little contention); a histogram larger than that table takes several passes over the input,
-//      one bin partition per pass.
+//   3. w > CS_SLOTS: the caches sit in front of the CTA's table in shared memory, which takes the
+//      cold elements by CTA-wide claim rounds (rbi_cached_big_kernel below) -- only the evictions /
+//      bypasses of the caches (rare) use a CAS loop.
 // With w <= CS_SLOTS a slot IS a bin: no tags, no evictions, no atomics at all.  CTA g writes its
 // result to part[g][.]; a second kernel folds the G tables per bin in a fixed order (deterministic).
 
 constexpr int CS_SLOTS = 1024, CS_WARPS = 8, CS_NT = CS_WARPS * 32, CS_CTAS_PER_SM = 5;   // w <= 1024
-constexpr int CB_SLOTS = 256, CB_WARPS = 32, CB_NT = CB_WARPS * 32;                       // w  > 1024
-constexpr int CB_PART = 36864;  // bins per pass: 144 KB of f32 next to 72 KB of warp caches
-constexpr int CB_MAX_PASSES = 8;
+constexpr int CB_SLOTS = 64, CB_WARPS = 32, CB_NT = CB_WARPS * 32;                        // w  > 1024
+constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 + 64 KB of claim words, 18 KB of warp caches
+constexpr int CB_MAX_SPLIT_LOG2 = 5;  // a group of up to 32 CTAs shares one histogram (w <= 2^20)
+constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
+constexpr int CB_HASH = 8192;         // claim words of round B
+constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
 constexpr uint32_t CB_EMPTY = 0xffffffffu;  // tag word = (bin / CB_SLOTS) << 2 | hit counter
 
 template <int ACC>
@@ -605,97 +608,235 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
-// CL = 2: a thread-block cluster of two CTAs (two SMs) shares ONE table of 2 x CB_PART bins through
-// distributed shared memory -- each CTA holds half of it and sends the cold updates for the other
-// half to its partner with a remote CAS.  w = 2^16 then takes one pass over the input instead of two.
-template <int ACC, bool COUNT_ZEROS, int CL>
+// w > CS_SLOTS.  A CTA of 1024 threads owns a table of up to CB_PART bins in shared memory.  A
+// histogram wider than that is SPLIT over the 2^c CTAs of a group by the low c bits of the bin
+// (hot neighbouring bins land on different CTAs); all CTAs of a group stream the same part of the
+// input at the same time (one of them pulls it from HBM, the others hit in L2) and each keeps the
+// elements of its own bins: one pass over the input for any w, no traffic between the CTAs.
+//
+// Per batch (U quads per thread) the table is updated WITHOUT atomics:
+//   0. an element whose bin is resident in the warp's cache is "hot" and goes to step 2 directly;
+//   1. two CTA-wide claim rounds: every pending thread stores its thread id into the bin's claim
+//      word (round A: one word per bin; round B, for the few losers of A: a small hashed array),
+//      barrier, the thread that reads its own id back owns the bin for this round and does a plain
+//      read-modify-write of the table cell (a thread's own elements of one bin are applied in
+//      program order).  Uniform keys: ~3 % of the elements lose round A, ~none round B;
+//   2. hot elements: claim rounds inside the warp on the resident cache entry (plain LDS/STS); an
+//      element that lost both CTA rounds sits in a CONTENDED bin: the warp's cache installs it
+//      unless a hotter bin guards the slot (claim_update_big above).  Hot bins therefore migrate
+//      into the caches and stop taking part in step 1; evictions and bypasses (cold, rare) fall
+//      back to a CAS on the table.
+// Barriers: [claim A] B1 [update A, claim B] B2 [update B] B3 [caches + CAS].  A foreign claim can
+// only make a thread lose; two threads never own one bin in one round because all claims of a
+// round precede its barrier and rounds A and B use different words.  CAS (after B3) and plain
+// updates (between B1 and B3 of the next batch) never overlap.
+template <int ACC, bool COUNT_ZEROS, int U>
 __global__ void __launch_bounds__(CB_NT, 1)
-rbi_cached_big_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restrict__ is,
                       const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
                       float S) {
     using OP = CachedOp<ACC>;
-    namespace cg = cooperative_groups;
     extern __shared__ uint4 smem_raw[];
-    float *table = reinterpret_cast<float *>(smem_raw);                        // [CB_PART]
-    float *vals = table + CB_PART;                                             // [CB_WARPS][CB_SLOTS]
-    uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);  // [CB_WARPS][CB_SLOTS]
-    uint8_t *claim = reinterpret_cast<uint8_t *>(tags + CB_WARPS * CB_SLOTS);   // [CB_WARPS][CB_SLOTS]
+    float *table = reinterpret_cast<float *>(smem_raw);                          // [CB_PART]
+    float *vals = table + CB_PART;                                               // [CB_WARPS][CB_SLOTS]
+    uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);    // [CB_WARPS][CB_SLOTS]
+    uint16_t *claimA = reinterpret_cast<uint16_t *>(tags + CB_WARPS * CB_SLOTS);  // [CB_PART]
+    uint16_t *claimB = claimA + CB_PART;                                          // [CB_HASH]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(claimB + CB_HASH);               // [CB_WARPS][CB_SLOTS]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint16_t tid = (uint16_t)threadIdx.x;
     float *vl = vals + warp * CB_SLOTS;
     uint32_t *tg = tags + warp * CB_SLOTS;
     uint8_t *cl = claim + warp * CB_SLOTS;
-    const int rank = CL > 1 ? (int)cg::this_cluster().block_rank() : 0;
-    float *tabs[CL];  // the cluster's table halves (own half: the plain shared-memory pointer)
-#pragma unroll
-    for (int r = 0; r < CL; r++)
-        tabs[r] = (CL > 1 && r != rank) ? cg::this_cluster().map_shared_rank(table, r) : table;
-    auto cell = [&](uint32_t rel) -> float * {
-        if (CL == 1) return table + rel;
-        const uint32_t owner = rel >= (uint32_t)CB_PART ? 1u : 0u;
-        return (owner == 0 ? tabs[0] : tabs[CL - 1]) + (rel - owner * CB_PART);
-    };
-    auto cluster_sync = [&]() {
-        if (CL > 1) cg::this_cluster().sync();
-        else __syncthreads();
-    };
-    const int64_t nquads = (n + 3) / 4;
-    const int64_t stride = (int64_t)gridDim.x * CB_NT;
-    constexpr int64_t SPAN = (int64_t)CL * CB_PART;
-    for (int64_t lo = 0; lo < w; lo += SPAN) {
-        const int nb = (int)min(SPAN, w - lo);                                  // bins of this pass
-        const int mine = max(0, min(CB_PART, nb - rank * CB_PART));             // ... held by this CTA
-        for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = OP::neutral();
-        for (int s = lane; s < CB_SLOTS; s += 32) {
-            vl[s] = OP::neutral();
-            tg[s] = CB_EMPTY;
-        }
-        cluster_sync();
-        int64_t qw = blockIdx.x * (int64_t)CB_NT + warp * 32;
-        int64_t k[4] = {-1, -1, -1, -1};
-        float v[4] = {0.f, 0.f, 0.f, 0.f};
-        if (qw < nquads) {
-            const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
-            load_vals4(vs, (qw + lane) * 4, cnt, v);
-        }
-        while (qw < nquads) {
-            int64_t kn[4] = {-1, -1, -1, -1};
-            float vn[4] = {0.f, 0.f, 0.f, 0.f};
-            const int64_t qn = qw + stride;
-            if (qn < nquads) {
-                const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
-                load_vals4(vs, (qn + lane) * 4, cnt, vn);
-            }
-#pragma unroll
-            for (int j = 0; j < 4; j++) {
-                const int64_t rel = k[j] - lo;  // other partition, or out of range: not this pass
-                bool act = (uint64_t)rel < (uint64_t)nb;
-                if (COUNT_ZEROS && act && v[j] == 0.f) {
-                    atomicAdd(zeros + k[j], 1u);
-                    act = false;
-                }
-                uint32_t eb = 0;
-                float evv = 0.f;
-                if (claim_update_big<ACC>(act, (uint32_t)rel, v[j], vl, tg, cl, S, lane, eb, evv))
-                    smem_combine<ACC>(cell(eb), evv, S);
-            }
-#pragma unroll
-            for (int j = 0; j < 4; j++) {
-                k[j] = kn[j];
-                v[j] = vn[j];
-            }
-            qw = qn;
-        }
-        __syncwarp();
-        for (int s = lane; s < CB_SLOTS; s += 32) {  // write the warp's cache back
-            const uint32_t t = tg[s];
-            if (t != CB_EMPTY) smem_combine<ACC>(cell((t >> 2) * CB_SLOTS + s), vl[s], S);
-        }
-        cluster_sync();  // every update of this pass, local and remote, has landed
-        float *dst = part + (size_t)(blockIdx.x / CL) * (size_t)w + lo + (int64_t)rank * CB_PART;
-        for (int i = threadIdx.x; i < mine; i += CB_NT) dst[i] = table[i];
-        __syncthreads();
+    const uint32_t clmask = (1u << cl_log2) - 1u;
+    const uint32_t rank = blockIdx.x & clmask;
+    const int64_t group = blockIdx.x >> cl_log2, groups = gridDim.x >> cl_log2;
+    for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = OP::neutral();
+    for (int s = lane; s < CB_SLOTS; s += 32) {
+        vl[s] = OP::neutral();
+        tg[s] = CB_EMPTY;
     }
-    if (CL > 1) cg::this_cluster().sync();  // no CTA leaves while its partner could still address it
+    __syncthreads();
+    constexpr int NI = 4 * U;
+    const int64_t nquads = (n + 3) / 4;
+    const int64_t stride = groups * (int64_t)(CB_NT * U);
+    int64_t q0 = group * (int64_t)(CB_NT * U);  // CTA-uniform: no thread leaves the barriers early
+    int64_t k[NI];
+    float v[NI];
+    auto load_batch = [&](int64_t q, int64_t (&kk)[NI], float (&vv)[NI]) {
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            int64_t k4[4] = {-1, -1, -1, -1};
+            float v4[4] = {0.f, 0.f, 0.f, 0.f};
+            const int64_t qq = q + u * CB_NT + threadIdx.x;
+            if (qq < nquads) {
+                const int cnt = load_keys4(is, qq * 4, n, k4);
+                load_vals4(vs, qq * 4, cnt, v4);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                kk[u * 4 + j] = k4[j];
+                vv[u * 4 + j] = v4[j];
+            }
+        }
+    };
+    // A claim word names the ELEMENT (thread id * NI + j): exactly one element per bin wins a round,
+    // so all claim words and table cells of a round can be read before any of them is written.
+    const uint32_t id0 = threadIdx.x * NI;
+    // Thread-private register entry (rb, racc, rcnt) in front of everything: a bin that holds a
+    // large share of the elements (one bin = 14 % at Zipf keys) is folded into a register with no
+    // shared-memory access at all.  Weighted majority vote: +CB_RW on a hit, -1 on a miss, replaced
+    // at 0 -- the displaced pair takes the element's place on the normal path.
+    uint32_t rb = CB_EMPTY, rcnt = 0;
+    float racc = OP::neutral();
+    load_batch(q0, k, v);
+    for (;;) {
+        // after the last batch of the input: one more round of the same machinery for the register
+        // entries (1024 CAS on one hot cell would serialise); q0 is CTA-uniform
+        const bool drain = q0 >= nquads;
+        int64_t kn[NI];
+        float vn[NI];
+        const int64_t qn = q0 + stride;
+        load_batch(qn, kn, vn);  // next batch's loads fly while this one is processed (none past the end)
+        uint32_t b[NI];  // table index of a pending element, CB_EMPTY = nothing pending
+        uint32_t zm = 0;
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+            const uint32_t klo = (uint32_t)k[j];
+            bool act = in_range(k[j], w) & ((klo & clmask) == rank);
+            if (COUNT_ZEROS) {
+                const bool z = act & (v[j] == 0.f);  // IEEE equality: +-0 only (Q7)
+                zm |= (uint32_t)z << j;
+                act &= !z;
+            }
+            b[j] = act ? klo >> cl_log2 : CB_EMPTY;
+        }
+        if (COUNT_ZEROS && zm) {
+#pragma unroll
+            for (int j = 0; j < NI; j++)
+                if (zm >> j & 1u) atomicAdd(zeros + k[j], 1u);
+        }
+        if (drain) {
+            b[0] = rb;
+            v[0] = racc;
+            rcnt = 1;  // keeps the loop below from re-installing it
+            rb = CB_EMPTY;
+        }
+#pragma unroll
+        for (int j = 0; j < NI; j++) {  // register entry
+            if (b[j] == CB_EMPTY) continue;
+            if (b[j] == rb) {
+                racc = OP::comb(racc, v[j], S);
+                rcnt = min(rcnt + CB_RW, CB_RMAX);
+                b[j] = CB_EMPTY;
+            } else if (rcnt == 0) {
+                const uint32_t ob = rb;
+                const float ov = racc;
+                rb = b[j];
+                racc = v[j];
+                b[j] = ob;  // CB_EMPTY the first time
+                v[j] = ov;
+            } else {
+                rcnt--;
+            }
+        }
+        uint32_t t[NI];
+#pragma unroll
+        for (int j = 0; j < NI; j++) t[j] = tg[b[j] & (CB_SLOTS - 1)];
+        uint32_t coldm = 0;  // bit j: pending and not resident in the warp's cache
+        uint32_t hotm = 0;   // bit j: pending and resident
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+            // a valid tag never equals CB_EMPTY's, and b == CB_EMPTY matches no tag
+            const bool hot = (t[j] >> 2) == b[j] / CB_SLOTS;
+            const bool cold = !hot & (b[j] != CB_EMPTY);
+            hotm |= (uint32_t)hot << j;
+            coldm |= (uint32_t)cold << j;
+            if (hot & ((t[j] & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t[j] + 1;  // racing lanes store the same word
+            if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
+        }
+        __syncthreads();  // B1
+        {
+            uint16_t c[NI];
+            float o[NI];
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                c[j] = claimA[b[j] & (CB_PART - 1)];
+                o[j] = table[b[j] & (CB_PART - 1)];
+            }
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                const bool cold = coldm >> j & 1u;
+                const bool win = cold & (c[j] == (uint16_t)(id0 + j));
+                if (win) table[b[j]] = OP::comb(o[j], v[j], S);
+                if (cold & !win) claimB[b[j] & (CB_HASH - 1)] = (uint16_t)(id0 + j);
+                coldm &= ~((uint32_t)win << j);
+            }
+        }
+        if (__syncthreads_or(coldm != 0)) {  // B2 (+ B3 only if somebody lost round A)
+            uint16_t c[NI];
+            float o[NI];
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                c[j] = claimB[b[j] & (CB_HASH - 1)];
+                o[j] = table[b[j] & (CB_PART - 1)];
+            }
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                const bool win = (coldm >> j & 1u) & (c[j] == (uint16_t)(id0 + j));
+                if (win) table[b[j]] = OP::comb(o[j], v[j], S);
+                coldm &= ~((uint32_t)win << j);
+            }
+            __syncthreads();  // B3
+        }
+        if (__any_sync(FULL_MASK, hotm != 0)) {
+#pragma unroll
+            for (int j = 0; j < NI; j++) {  // hits: the resident entry cannot change before the installs below
+                uint8_t *c = cl + (b[j] & (CB_SLOTS - 1));
+                float *a = vl + (b[j] & (CB_SLOTS - 1));
+                bool pend = hotm >> j & 1u;
+                while (__any_sync(FULL_MASK, pend)) {
+                    if (pend) *c = (uint8_t)lane;
+                    __syncwarp();
+                    if (pend && *c == lane) {
+                        *a = OP::comb(*a, v[j], S);
+                        pend = false;
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+        if (__any_sync(FULL_MASK, coldm != 0)) {
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                const bool act = coldm >> j & 1u;
+                if (__any_sync(FULL_MASK, act)) {
+                    uint32_t eb = 0;
+                    float evv = 0.f;
+                    if (claim_update_big<ACC>(act, b[j], v[j], vl, tg, cl, S, lane, eb, evv))
+                        smem_combine<ACC>(table + eb, evv, S);
+                }
+            }
+        }
+        if (drain) break;
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+            k[j] = kn[j];
+            v[j] = vn[j];
+        }
+        q0 = qn;
+    }
+    __syncthreads();
+    for (int s = lane; s < CB_SLOTS; s += 32) {  // write the warp's cache back
+        const uint32_t t = tg[s];
+        if (t != CB_EMPTY) smem_combine<ACC>(table + (t >> 2) * CB_SLOTS + s, vl[s], S);
+    }
+    __syncthreads();
+    float *dst = part + (size_t)group * (size_t)w;
+    for (int64_t i = threadIdx.x; i < CB_PART; i += CB_NT) {
+        const int64_t bin = (i << cl_log2) + rank;
+        if (bin < w) dst[bin] = table[i];
+    }
 }
 
 // Fold of the G per-CTA tables for 32 consecutive bins by a CTA of 256 threads: thread (x, y) folds
@@ -733,24 +874,31 @@ rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part, float *
 }
 
 constexpr size_t CS_SMEM = (size_t)CS_WARPS * CS_SLOTS * 5;
-constexpr size_t CB_SMEM = (size_t)CB_PART * 4 + (size_t)CB_WARPS * CB_SLOTS * 9;
+constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_HASH * 2 + (size_t)CB_WARPS * CB_SLOTS * 9;
 
-constexpr int CB_CLUSTER = 2;
-// a table that fits one CTA needs no partner (the remote updates only cost: satadd w=4096 0.21 vs 0.33 ms)
-static int cached_cluster(int64_t w) { return w > CB_PART ? CB_CLUSTER : 1; }
+// log2 of the CTAs per group: the smallest power of two with 2^c * CB_PART >= w
+static int cached_split_log2(int64_t w) {
+    int c = 0;
+    while (((int64_t)CB_PART << c) < w) c++;
+    return c;
+}
 static int cached_grid(int64_t n, int64_t w) {
     if (w <= CS_SLOTS) return grid_for(n < 1 ? 1 : n, CS_NT, CS_CTAS_PER_SM);
-    const int g = grid_for(n < 1 ? 1 : n, CB_NT, 1), c = cached_cluster(w);
-    return (g + c - 1) / c * c;  // whole clusters
+    const int c = cached_split_log2(w);
+    const int64_t quads = ((n < 1 ? 1 : n) + 3) / 4;
+    int64_t groups = (quads + CB_NT * CB_U - 1) / (CB_NT * CB_U);
+    const int64_t cap = NUM_SMS_B200 >> c > 0 ? NUM_SMS_B200 >> c : 1;
+    if (groups > cap) groups = cap;
+    return (int)(groups << c);
 }
 // number of partial tables the accumulation kernel writes
 static int cached_tables(int64_t n, int64_t w) {
-    return w <= CS_SLOTS ? cached_grid(n, w) : cached_grid(n, w) / cached_cluster(w);
+    return w <= CS_SLOTS ? cached_grid(n, w) : cached_grid(n, w) >> cached_split_log2(w);
 }
 static size_t cached_part_bytes(int64_t n, int64_t w) {
     return align_up((size_t)cached_tables(n, w) * (size_t)(w < 1 ? 1 : w) * 4, 256);
 }
-bool rbi_cached_supported(int64_t w) { return w <= (int64_t)CB_PART * CB_CLUSTER * CB_MAX_PASSES; }
+bool rbi_cached_supported(int64_t w) { return w <= ((int64_t)CB_PART << CB_MAX_SPLIT_LOG2); }
 
 // Accumulates into part[G][w]; returns G in *G_out.
 template <int ACC, bool COUNT_ZEROS>
@@ -762,26 +910,10 @@ static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, 
         auto kern = rbi_cached_small_kernel<ACC, COUNT_ZEROS>;
         VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CS_NT, CS_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
     } else {
-        const int cl = cached_cluster(w);
-        auto kern = cl > 1 ? rbi_cached_big_kernel<ACC, COUNT_ZEROS, CB_CLUSTER>
-                           : rbi_cached_big_kernel<ACC, COUNT_ZEROS, 1>;
+        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS, CB_U>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CB_SMEM) != cudaSuccess)
             return VJP_ERR_CUDA;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)G);
-        cfg.blockDim = dim3(CB_NT);
-        cfg.dynamicSmemBytes = CB_SMEM;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = (unsigned)cl;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        VJP_LAUNCH(K_CACHED_ACC, stream) {
-            if (cudaLaunchKernelEx(&cfg, kern, n, w, is, vs, part, zeros, S) != cudaSuccess) return VJP_ERR_CUDA;
-        }
+        VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CB_NT, CB_SMEM, stream>>>(n, w, cached_split_log2(w), is, vs, part, zeros, S);
     }
     return last_launch_status();
 }
