@@ -571,6 +571,8 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     int64_t qw = blockIdx.x * (int64_t)CS_NT + warp * 32;  // warp-uniform: the warp never diverges here
     int64_t k[4] = {-1, -1, -1, -1};
     float v[4] = {0.f, 0.f, 0.f, 0.f};
+    uint32_t rb = CB_EMPTY, rcnt = 0;
+    float racc = OP::neutral();
     if (qw < nquads) {
         const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
         load_vals4(vs, (qw + lane) * 4, cnt, v);
@@ -590,7 +592,26 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                 atomicAdd(zeros + k[j], 1u);
                 act = false;
             }
-            claim_update_small<ACC>(act, (uint32_t)k[j], v[j], vl, cl, S, lane);
+            uint32_t b = (uint32_t)k[j];
+            float x = v[j];
+            if (act) {  // register entry: see rbi_cached_big_kernel
+                if (b == rb) {
+                    racc = OP::comb(racc, x, S);
+                    rcnt = min(rcnt + CB_RW, CB_RMAX);
+                    act = false;
+                } else if (rcnt == 0) {
+                    act = rb != CB_EMPTY;
+                    const uint32_t ob = rb;
+                    const float ov = racc;
+                    rb = b;
+                    racc = x;
+                    b = ob;
+                    x = ov;
+                } else {
+                    rcnt--;
+                }
+            }
+            claim_update_small<ACC>(act, b, x, vl, cl, S, lane);
         }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
@@ -599,6 +620,7 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         }
         qw = qn;
     }
+    claim_update_small<ACC>(rb != CB_EMPTY, rb, racc, vl, cl, S, lane);
     __syncthreads();
     for (int s = threadIdx.x; s < (int)w; s += CS_NT) {
         float acc = vals[s];
