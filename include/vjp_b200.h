@@ -116,7 +116,7 @@ size_t vjp_reduce_by_index_workspace_bytes(const vjp_op_t *op, int64_t n, int64_
  * there is no hist_0 argument).  hist[num_bins] is fully written.
  * Supported: ADD (f32, f64), MIN, MAX, MUL, SATADD (f32).  ADD needs no workspace (ws may be NULL);
  * the others return VJP_ERR_WORKSPACE if ws is too small.  MUL and SATADD keep shared-memory tables of
- * 73728 bins per pass over the input, at most 8 passes: a larger num_bins returns VJP_ERR_UNSUPPORTED. */
+ * 32768 bins per CTA, split over groups of up to 32 CTAs: num_bins > 2^20 returns VJP_ERR_UNSUPPORTED. */
 int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
                             const void *vs, void *hist, void *ws, size_t ws_bytes, void *stream);
 
@@ -125,7 +125,7 @@ int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, con
  *   MIN/MAX:  lifted primal (index, value) per bin, lowest index on ties (Fig. 5),
  *             then vs_bar = 0 and vs_bar[arg[k]] = hist_bar[k].  Bit-exact copy.
  *   MUL:      lifted primal (zero count, product of non-zeros) (Fig. 3),
- *             then the three-way map of P:L208-219 / P:L243-246.  num_bins <= 8 x 73728, else
+ *             then the three-way map of P:L208-219 / P:L243-246.  num_bins <= 2^20, else
  *             VJP_ERR_UNSUPPORTED (force_general handles any num_bins).
  *   SATADD or force_general: stable radix sort by clamped bin, forward and reverse segmented
  *             exclusive scans, per-element derivative of l (.) x (.) r, un-permute
@@ -141,6 +141,14 @@ int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
                              const int64_t *is_host, const void *vs_host,
                              const void *hist_bar_host, void *vs_bar_host,
                              void *dev_scratch, size_t dev_scratch_bytes, void *stream);
+/* The same without the final synchronisation: copies in, kernels and the copy out are only enqueued
+ * on `stream` (host buffers should be pinned for the copies to be asynchronous).  The caller
+ * synchronises `stream` before it reads vs_bar_host or reuses dev_scratch / the host inputs; calls on
+ * different streams with different dev_scratch buffers overlap their copies with each other's kernels. */
+int vjp_reduce_by_index_host_async(const vjp_op_t *op, int64_t n, int64_t num_bins,
+                                   const int64_t *is_host, const void *vs_host,
+                                   const void *hist_bar_host, void *vs_bar_host,
+                                   void *dev_scratch, size_t dev_scratch_bytes, void *stream);
 
 /* Inspection entry points: the integer-valued intermediates, for bit-exact comparison. */
 

@@ -197,6 +197,11 @@ class RbiCase:
         h = self.host
         return B.vjp_reduce_by_index_host(self.op, self.w, h["is_"], h["vs"], h["hb"], h["out"], self.scratch)
 
+    def vjp_host_async(self, stream):
+        h = self.host
+        return B.vjp_reduce_by_index_host_async(self.op, self.w, h["is_"], h["vs"], h["hb"], h["out"],
+                                                self.scratch, stream=stream)
+
     def h2d_bytes(self):
         h = self.host
         return h["is_"].numel() * 8 + h["vs"].numel() * h["vs"].element_size() + h["hb"].numel() * h["hb"].element_size()

@@ -27,7 +27,7 @@ EXPORTS = [
     "vjp_scan_arity", "vjp_version", "vjp_scan_workspace_bytes", "scan_forward", "vjp_scan",
     "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_reduce_by_index_workspace_bytes",
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
-    "vjp_reduce_by_index_host", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
+    "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
     "vjp_kernel_count", "vjp_kernel_name", "vjp_launch_count", "vjp_profile_enable", "vjp_profile_read",
 ]
 
@@ -91,6 +91,7 @@ def load() -> ctypes.CDLL:
         "vjp_reduce_by_index": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "vjp_reduce_by_index_host_scratch_bytes": (sz, [opp, i64, i64]),
         "vjp_reduce_by_index_host": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_by_index_host_async": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
@@ -246,6 +247,16 @@ def vjp_reduce_by_index_host(op: Op, num_bins: int, is_, vs, hist_bar, out, scra
     _check(load().vjp_reduce_by_index_host(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
                                            _ptr(out), _ptr(scratch), scratch.numel(), _stream(stream)),
            "vjp_reduce_by_index_host")
+    return out
+
+
+def vjp_reduce_by_index_host_async(op: Op, num_bins: int, is_, vs, hist_bar, out, scratch, stream=None):
+    """As vjp_reduce_by_index_host, but only enqueued on `stream`: synchronise it before reading `out`."""
+    n = is_.numel()
+    o = op.c()
+    _check(load().vjp_reduce_by_index_host_async(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs),
+                                                 _ptr(hist_bar), _ptr(out), _ptr(scratch), scratch.numel(),
+                                                 _stream(stream)), "vjp_reduce_by_index_host_async")
     return out
 
 

@@ -247,10 +247,10 @@ size_t vjp_reduce_by_index_host_scratch_bytes(const vjp_op_t *op, int64_t n, int
            align_up((size_t)num_bins * e, 256) + vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
 }
 
-int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
-                             const int64_t *is_host, const void *vs_host,
-                             const void *hist_bar_host, void *vs_bar_host, void *dev_scratch,
-                             size_t dev_scratch_bytes, void *stream) {
+int vjp_reduce_by_index_host_async(const vjp_op_t *op, int64_t n, int64_t num_bins,
+                                   const int64_t *is_host, const void *vs_host,
+                                   const void *hist_bar_host, void *vs_bar_host, void *dev_scratch,
+                                   size_t dev_scratch_bytes, void *stream) {
     if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
     const int route = rbi_route(op);
     if (route == 0) return VJP_ERR_UNSUPPORTED;
@@ -282,7 +282,17 @@ int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
     if (rc != VJP_OK) return rc;
     if (cudaMemcpyAsync(vs_bar_host, dout, (size_t)n * e, cudaMemcpyDeviceToHost, s) != cudaSuccess)
         return VJP_ERR_CUDA;
-    return cuda_status(cudaStreamSynchronize(s));
+    return VJP_OK;
+}
+
+int vjp_reduce_by_index_host(const vjp_op_t *op, int64_t n, int64_t num_bins,
+                             const int64_t *is_host, const void *vs_host,
+                             const void *hist_bar_host, void *vs_bar_host, void *dev_scratch,
+                             size_t dev_scratch_bytes, void *stream) {
+    const int rc = vjp_reduce_by_index_host_async(op, n, num_bins, is_host, vs_host, hist_bar_host,
+                                                  vs_bar_host, dev_scratch, dev_scratch_bytes, stream);
+    if (rc != VJP_OK || n == 0) return rc;
+    return cuda_status(cudaStreamSynchronize(as_stream(stream)));
 }
 
 int rbi_argext(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is, const void *vs,

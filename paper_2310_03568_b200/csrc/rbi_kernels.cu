@@ -343,11 +343,24 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         smem_raw[k] = make_uint4(~0u, ~0u, ~0u, ~0u);
     __syncthreads();
     const int64_t stride = (int64_t)gridDim.x * MMF_NT;
-    for (int64_t q = blockIdx.x * (int64_t)MMF_NT + threadIdx.x; q * 4 < n; q += stride) {
-        int64_t k[4];
-        float v[4];
-        const int cnt = load_keys4(is, q * 4, n, k);
+    int64_t q = blockIdx.x * (int64_t)MMF_NT + threadIdx.x;
+    int64_t k[4] = {-1, -1, -1, -1};
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    int cnt = 0;
+    if (q * 4 < n) {
+        cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
+    }
+    while (q * 4 < n) {
+        // next iteration's loads fly while this one walks the table (its L2 round trips are dependent)
+        int64_t kn[4] = {-1, -1, -1, -1};
+        float vn[4] = {0.f, 0.f, 0.f, 0.f};
+        int cntn = 0;
+        const int64_t qn = q + stride;
+        if (qn * 4 < n) {
+            cntn = load_keys4(is, qn * 4, n, kn);
+            load_vals4(vs, qn * 4, cntn, vn);
+        }
         if (vs_bar) {
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
@@ -374,6 +387,13 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             if (TAGGED) f32[b & 32767u] = ((b >> 15) << 16) | c16;
             else f16[b] = (uint16_t)c16;
         }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            k[j] = kn[j];
+            v[j] = vn[j];
+        }
+        cnt = cntn;
+        q = qn;
     }
 }
 

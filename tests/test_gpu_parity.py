@@ -299,3 +299,87 @@ def test_rbi_rejects_bad_arguments_and_handles_empty_input():
     for name in ("add", "min", "max", "mul", "satadd"):
         out = B.vjp_reduce_by_index(B.Op.of(name, S=1.0), 5, bad, vv, torch.ones(5, device="cuda"))
         assert torch.count_nonzero(out).item() == 0
+
+
+# ----------------------------------------------------------- wide histograms, host entry ----
+
+@pytest.mark.parametrize("n,w", [(1 << 18, 40000), (300007, 300000), (100003, 1 << 20)])
+@pytest.mark.parametrize("dist", ["uniform", "zipf"])
+def test_rbi_mul_wide_histograms_split_over_cta_groups(dist, n, w):
+    """w > 32768: the table is split over 2, 16, 32 CTAs by the low bits of the bin."""
+    d = W.c2_rbi_mul(n=n, w=w, dist=dist, zero_rate=min(0.3, 0.7 * w / n))
+    is_, vs, hb = d["is_"].copy(), d["vs"], d["hist_bar"]
+    is_[::97] = w + 5
+    op = B.Op.of("mul")
+    zeros, prod = B.rbi_zero_prod(op, w, dev(is_), dev(vs))
+    got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+    ref, rz, rp = oracle.vjp_rbi_mul(w, is_, vs, hb)
+    assert np.array_equal(zeros.cpu().numpy(), rz)
+    gp = prod.cpu().numpy().astype(np.float64)
+    ok = rp > 1e-30
+    assert np.all(np.abs(gp[ok] - rp[ok]) <= 1e-4 * np.abs(rp[ok]))
+    assert nrel(got, ref) <= 1e-4
+
+
+def test_rbi_mul_one_hot_bin_and_sorted_keys():
+    """Degenerate key streams of the cached accumulation: every element in one bin; sorted keys (the hot
+    bin changes along the input); two alternating bins.  Values are signed powers of two, so every
+    product is exact in f32 whatever the association order (a 200 000-term f32 product of arbitrary
+    values differs from the f64 oracle by more than 1e-4 in ANY order but the sequential one)."""
+    n, w = 200003, 5000
+    rng = np.random.default_rng(5)
+    vs = np.ones(n, dtype=np.float32)
+    pos = rng.choice(n, 3000, replace=False)
+    vs[pos] = rng.choice(np.array([0.5, 2.0, -1.0, -2.0, -0.5], dtype=np.float32), 3000)
+    hb = rng.standard_normal(w).astype(np.float32)
+    for is_ in (np.full(n, 4321, dtype=np.int64), np.sort(rng.integers(0, w, n)).astype(np.int64),
+                (np.arange(n, dtype=np.int64) % 2) * 4999):
+        got = B.vjp_reduce_by_index(B.Op.of("mul"), w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+        ref, _, _ = oracle.vjp_rbi_mul(w, is_, vs, hb)
+        assert np.all(np.isfinite(ref)) and np.max(np.abs(ref)) > 0
+        assert nrel(got, ref) <= 1e-6
+
+
+def test_rbi_cached_rejects_too_wide_histograms():
+    is_ = torch.zeros(4, dtype=torch.int64, device="cuda")
+    v = torch.ones(4, device="cuda")
+    w = (1 << 20) + 1
+    with pytest.raises(B.VjpError):
+        B.vjp_reduce_by_index(B.Op.of("mul"), w, is_, v, torch.ones(w, device="cuda"))
+
+
+@pytest.mark.parametrize("opname", ["add", "min", "mul", "satadd"])
+def test_rbi_host_entry_points_match_the_device_path(opname):
+    """vjp_reduce_by_index_host (synchronous) and _host_async (two problems on two streams) return what
+    the device-pointer call returns: bit for bit for the copies ('+', min); to rounding for '*' and
+    satadd, whose f32 accumulation order depends on which element wins a claim round."""
+    n, w = 100003, 3000
+    op = B.Op.of(opname, S=20.0)
+    rng = np.random.default_rng(11)
+    probs = []
+    for _ in range(2):
+        is_ = keys_with_oob(rng, n, w)
+        vs = rng.uniform(0.0, 1.0, n).astype(np.float32)
+        hb = rng.standard_normal(w).astype(np.float32)
+        probs.append((is_, vs, hb))
+    want = [B.vjp_reduce_by_index(op, w, dev(i), dev(v), dev(h)).cpu().numpy() for i, v, h in probs]
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    nbytes = B.vjp_reduce_by_index_host_scratch_bytes(op, n, w)
+    outs, keep = [], []
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for (i, v, h), s in zip(probs, streams):
+        hi, hv, hh = pin(i), pin(v), pin(h)
+        out = torch.empty(n, dtype=torch.float32).pin_memory()
+        scratch = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+        keep.append((hi, hv, hh, scratch))
+        B.vjp_reduce_by_index_host_async(op, w, hi, hv, hh, out, scratch, stream=s)
+        outs.append(out)
+    for s in streams:
+        s.synchronize()
+    same = (lambda a, b: np.array_equal(a, b)) if opname in ("add", "min") else (lambda a, b: nrel(a, b) <= 1e-5)
+    for o, ref in zip(outs, want):
+        assert same(o.numpy(), ref)
+    hi, hv, hh, scratch = keep[0]
+    out = torch.empty(n, dtype=torch.float32).pin_memory()
+    B.vjp_reduce_by_index_host(op, w, hi, hv, hh, out, scratch)
+    assert same(out.numpy(), want[0])
