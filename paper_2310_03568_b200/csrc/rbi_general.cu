@@ -173,8 +173,8 @@ u32_exclusive_scan_kernel(uint32_t *data, int64_t m, int *ticket, uint64_t *stat
 // ------------------------------------------------------------------ radix sort passes -----
 
 constexpr int SORT_NT = 256;
-constexpr int SORT_IPT = 16;
-constexpr int SORT_TILE = SORT_NT * SORT_IPT;  // 4096 keys; warp w owns keys [512 w, 512 w + 512)
+constexpr int SORT_IPT = 8;
+constexpr int SORT_TILE = SORT_NT * SORT_IPT;  // 2048 keys; warp w owns keys [256 w, 256 w + 256)
 constexpr int SORT_MAX_RADIX = 256;
 
 // key' = k if 0 <= k < w else w (Q18)
@@ -361,7 +361,7 @@ struct SegComb {
 
 // ------------------------------------------------------------------ segmented scans -------
 
-constexpr int SEG_NT = 256;
+constexpr int SEG_NT = 512;
 constexpr int SEG_IPT = 8;
 constexpr int SEG_TILE = SEG_NT * SEG_IPT;
 
@@ -604,11 +604,17 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
     using PS = Stage<SEG_NT, 2 * SEG_IPT>;
     const GenOp<CODE> op{S};
     const int nt = (int)seg_tiles(n);
+    constexpr size_t FWD_SMEM = KS::SMEM_BYTES + PS::SMEM_BYTES, REV_SMEM = 2 * KS::SMEM_BYTES + PS::SMEM_BYTES;
+    if ((FWD_SMEM > 48 * 1024 &&
+         cudaFuncSetAttribute(seg_forward_kernel<CODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FWD_SMEM) != cudaSuccess) ||
+        (REV_SMEM > 48 * 1024 &&
+         cudaFuncSetAttribute(seg_reverse_vjp_kernel<CODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REV_SMEM) != cudaSuccess))
+        return VJP_ERR_CUDA;
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+    VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, FWD_SMEM, stream>>>(
         n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, 2 * KS::SMEM_BYTES + PS::SMEM_BYTES, stream>>>(
+    VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, REV_SMEM, stream>>>(
         n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status);
     return last_launch_status();
 }
