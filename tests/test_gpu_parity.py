@@ -16,8 +16,8 @@ from paper_2310_03568_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 TOL = {torch.float32: 1e-4, torch.float64: 1e-10}
-# tile shapes in use: 384 / 640 (5x5), 2048 ... 16384 elements
-SIZES = [1, 2, 33, 127, 128, 129, 383, 384, 385, 511, 513, 639, 640, 641, 1023, 1025, 2047, 2049, 4095, 4096, 4097,
+# tile shapes in use: 640 / 768 (5x5), 2048 ... 16384 elements
+SIZES = [1, 2, 33, 127, 128, 129, 383, 384, 385, 511, 513, 639, 640, 641, 767, 768, 769, 1023, 1025, 2047, 2049, 4095, 4096, 4097,
          8191, 8192, 8193, 12345, 16383, 16384, 16385, 32769, 100003, 300007]
 
 
