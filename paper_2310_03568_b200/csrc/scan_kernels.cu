@@ -416,8 +416,8 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
 using CfgAddF32 = ScanCfg<OpAdd<float>, 512, 32, 512, 32>;
 using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
-using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 512, 8>;
-using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 512, 8>;
+using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
+using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
 using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 512, 4>;
 using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
 
