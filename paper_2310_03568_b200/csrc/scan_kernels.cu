@@ -200,7 +200,7 @@ tile_exscan_kernel(int num_tiles, typename Op::Fwd *__restrict__ fpre) {
 //     rbar_i = ybar_i + u_{i+1},   xbar_i = (d(r_{i-1} (.) x_i)/dx_i)^T rbar_i,   u_n = 0,
 // and element i acts on the incoming u as the affine map z -> (ybar_i + z) * X_i^T.
 template <class Op, int NT, int IPT>
-__global__ void __launch_bounds__(NT, (Op::EW <= 4 && NT <= 512 ? 2 : 1))
+__global__ void __launch_bounds__(NT, (Op::EW <= 4 ? 1024 / NT : 1))
 scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
                         uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
                         const typename Op::Fwd *__restrict__ fpre,
@@ -418,7 +418,7 @@ using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
-using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 512, 4>;
+using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8>;
 using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
 
 #define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
