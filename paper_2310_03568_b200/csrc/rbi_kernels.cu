@@ -492,7 +492,6 @@ constexpr int CB_SLOTS = 64, CB_WARPS = 32, CB_NT = CB_WARPS * 32;              
 constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 + 64 KB of claim words, 18 KB of warp caches
 constexpr int CB_MAX_SPLIT_LOG2 = 5;  // a group of up to 32 CTAs shares one histogram (w <= 2^20)
 constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
-constexpr int CB_HASH = 8192;         // claim words of round B
 constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
 constexpr uint32_t CB_EMPTY = 0xffffffffu;  // tag word = (bin / CB_SLOTS) << 2 | hit counter
 
@@ -658,20 +657,18 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 //
 // Per batch (U quads per thread) the table is updated WITHOUT atomics:
 //   0. an element whose bin is resident in the warp's cache is "hot" and goes to step 2 directly;
-//   1. two CTA-wide claim rounds: every pending thread stores its thread id into the bin's claim
-//      word (round A: one word per bin; round B, for the few losers of A: a small hashed array),
-//      barrier, the thread that reads its own id back owns the bin for this round and does a plain
-//      read-modify-write of the table cell (a thread's own elements of one bin are applied in
-//      program order).  Uniform keys: ~3 % of the elements lose round A, ~none round B;
+//   1. one CTA-wide claim round: every pending element stores its id into the bin's claim word,
+//      barrier, the element that reads its id back owns the bin for this round and does a plain
+//      read-modify-write of the table cell.  Uniform keys at w = 2^16: ~6 % of the elements lose.
+//      A loser gets ONE compare-and-swap on the cell (uniform keys: it succeeds);
 //   2. hot elements: claim rounds inside the warp on the resident cache entry (plain LDS/STS); an
-//      element that lost both CTA rounds sits in a CONTENDED bin: the warp's cache installs it
-//      unless a hotter bin guards the slot (claim_update_big above).  Hot bins therefore migrate
-//      into the caches and stop taking part in step 1; evictions and bypasses (cold, rare) fall
-//      back to a CAS on the table.
-// Barriers: [claim A] B1 [update A, claim B] B2 [update B] B3 [caches + CAS].  A foreign claim can
-// only make a thread lose; two threads never own one bin in one round because all claims of a
-// round precede its barrier and rounds A and B use different words.  CAS (after B3) and plain
-// updates (between B1 and B3 of the next batch) never overlap.
+//      element that lost the round AND its compare-and-swap sits in a CONTENDED bin: the warp's
+//      cache installs it unless a hotter bin guards the slot (claim_update_big above).  Hot bins
+//      therefore migrate into the caches and stop taking part in step 1; evictions and bypasses
+//      (cold, rare) fall back to a CAS loop on the table.
+// Barriers: [claim] B1 [plain updates] B2 [CAS, caches].  Two elements never own one bin in a round
+// because all claims precede B1; the plain updates (between B1 and B2) never overlap a CAS (after
+// B2, before the next batch's B1).
 template <int ACC, bool COUNT_ZEROS, int U>
 __global__ void __launch_bounds__(CB_NT, 1)
 rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restrict__ is,
@@ -683,8 +680,7 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     float *vals = table + CB_PART;                                               // [CB_WARPS][CB_SLOTS]
     uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);    // [CB_WARPS][CB_SLOTS]
     uint16_t *claimA = reinterpret_cast<uint16_t *>(tags + CB_WARPS * CB_SLOTS);  // [CB_PART]
-    uint16_t *claimB = claimA + CB_PART;                                          // [CB_HASH]
-    uint8_t *claim = reinterpret_cast<uint8_t *>(claimB + CB_HASH);               // [CB_WARPS][CB_SLOTS]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(claimA + CB_PART);               // [CB_WARPS][CB_SLOTS]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint16_t tid = (uint16_t)threadIdx.x;
     float *vl = vals + warp * CB_SLOTS;
@@ -811,25 +807,20 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 const bool cold = coldm >> j & 1u;
                 const bool win = cold & (c[j] == (uint16_t)(id0 + j));
                 if (win) table[b[j]] = OP::comb(o[j], v[j], S);
-                if (cold & !win) claimB[b[j] & (CB_HASH - 1)] = (uint16_t)(id0 + j);
                 coldm &= ~((uint32_t)win << j);
             }
         }
-        if (__syncthreads_or(coldm != 0)) {  // B2 (+ B3 only if somebody lost round A)
-            uint16_t c[NI];
-            float o[NI];
+        __syncthreads();  // B2: the plain updates are done before any CAS touches the table
+        if (__any_sync(FULL_MASK, coldm != 0)) {
 #pragma unroll
-            for (int j = 0; j < NI; j++) {
-                c[j] = claimB[b[j] & (CB_HASH - 1)];
-                o[j] = table[b[j] & (CB_PART - 1)];
+            for (int j = 0; j < NI; j++) {  // losers: ONE compare-and-swap; a failure means the bin is contended
+                if (coldm >> j & 1u) {
+                    unsigned *cell = reinterpret_cast<unsigned *>(table + b[j]);
+                    const unsigned old = *(volatile unsigned *)cell;
+                    const unsigned upd = __float_as_uint(OP::comb(__uint_as_float(old), v[j], S));
+                    if (atomicCAS(cell, old, upd) == old) coldm &= ~(1u << j);
+                }
             }
-#pragma unroll
-            for (int j = 0; j < NI; j++) {
-                const bool win = (coldm >> j & 1u) & (c[j] == (uint16_t)(id0 + j));
-                if (win) table[b[j]] = OP::comb(o[j], v[j], S);
-                coldm &= ~((uint32_t)win << j);
-            }
-            __syncthreads();  // B3
         }
         if (__any_sync(FULL_MASK, hotm != 0)) {
 #pragma unroll
@@ -916,7 +907,7 @@ rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part, float *
 }
 
 constexpr size_t CS_SMEM = (size_t)CS_WARPS * CS_SLOTS * 5;
-constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_HASH * 2 + (size_t)CB_WARPS * CB_SLOTS * 9;
+constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9;
 
 // log2 of the CTAs per group: the smallest power of two with 2^c * CB_PART >= w
 static int cached_split_log2(int64_t w) {
