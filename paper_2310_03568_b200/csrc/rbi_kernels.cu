@@ -489,7 +489,7 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
 
 constexpr int CS_SLOTS = 1024, CS_WARPS = 8, CS_NT = CS_WARPS * 32, CS_CTAS_PER_SM = 5;   // w <= 1024
 constexpr int CB_SLOTS = 64, CB_WARPS = 32, CB_NT = CB_WARPS * 32;                        // w  > 1024
-constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 + 64 KB of claim words, 18 KB of warp caches
+constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 + 64 KB of claim words, 18 KB of warp caches (128-slot caches: no gain)
 constexpr int CB_MAX_SPLIT_LOG2 = 5;  // a group of up to 32 CTAs shares one histogram (w <= 2^20)
 constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
 constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
@@ -682,7 +682,6 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     uint16_t *claimA = reinterpret_cast<uint16_t *>(tags + CB_WARPS * CB_SLOTS);  // [CB_PART]
     uint8_t *claim = reinterpret_cast<uint8_t *>(claimA + CB_PART);               // [CB_WARPS][CB_SLOTS]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint16_t tid = (uint16_t)threadIdx.x;
     float *vl = vals + warp * CB_SLOTS;
     uint32_t *tg = tags + warp * CB_SLOTS;
     uint8_t *cl = claim + warp * CB_SLOTS;
@@ -961,7 +960,6 @@ static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *i
                        ? run_cached<ACC_MUL, false>(n, w, is, vs, part, nullptr, S, &G, stream)
                        : run_cached<ACC_SATADD, false>(n, w, is, vs, part, nullptr, S, &G, stream);
     if (rc != VJP_OK) return rc;
-    const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
     if (code == VJP_OP_MUL)
         VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL><<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, part, hist, S);
     else
@@ -1054,7 +1052,6 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     int G = 0;
     const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream);
     if (rc != VJP_OK) return rc;
-    const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
     VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
                                                   vs_bar ? m.coef : nullptr);
     if (vs_bar && n > 0) {
