@@ -8,7 +8,7 @@
  * Conventions common to every entry point
  *   - Pointers named xs, ys, ys_bar, xs_bar, is, vs, hist, hist_bar, vs_bar, arg, ext, zeros,
  *     prod_nz, sorted_keys, perm and ws are DEVICE pointers owned by the caller, 16-byte
- *     aligned (a torch allocation is).  The library never allocates, frees or synchronises:
+ *     aligned (a torch allocation is; a view such as x[1:] is not).  The library never allocates, frees or synchronises:
  *     a call validates its arguments on the host, enqueues kernels / memsets on `stream`
  *     (a cudaStream_t passed as void*; NULL = the legacy default stream) and returns.
  *     The *_host entry points are the exception: their data pointers are HOST pointers, they
@@ -18,8 +18,14 @@
  *   - Bin indices `is` are int64.  An index outside [0, num_bins) -- negative
  *     included -- is ignored by the primal and receives adjoint exactly 0 (P:L335-336,
  *     P:L361-362; Q3).
- *   - Outputs are overwritten with the adjoint CONTRIBUTION (the paper's "+=" target taken
- *     as zero, Q1).  Outputs must not alias inputs.
+ *   - With op.accumulate == 0 outputs are overwritten with the adjoint CONTRIBUTION (the paper's
+ *     "+=" target taken as zero, Q1); with op.accumulate != 0 the VJP calls ADD the contribution
+ *     to what xs_bar / vs_bar hold (the paper writes every return sweep as "+=": P:L83-88, P:L367,
+ *     P:L450), fused into the kernel's final store.  The primal calls ignore the field.
+ *     Outputs must not alias inputs, with one exception: vjp_scan with VJP_OP_ADD and
+ *     accumulate == 0 may run in place (xs_bar == ys_bar).
+ *   - Every data pointer must be 16-byte aligned (the kernels use 128-bit accesses); a misaligned
+ *     pointer is VJP_ERR_INVALID_ARG.
  *   - `ws` is scratch of at least *_workspace_bytes(...) bytes; its contents need not be
  *     initialised and are garbage afterwards.  Two calls that may overlap in time need two
  *     workspaces.
@@ -41,7 +47,7 @@ extern "C" {
 
 typedef enum {
     VJP_OK = 0,
-    VJP_ERR_INVALID_ARG = -1, /* NULL pointer, negative size, unknown op / dtype            */
+    VJP_ERR_INVALID_ARG = -1, /* NULL or misaligned pointer, negative size, unknown op / dtype */
     VJP_ERR_UNSUPPORTED = -2, /* op not defined for this combinator / dtype, n too large     */
     VJP_ERR_WORKSPACE = -3,   /* ws_bytes smaller than the *_workspace_bytes query          */
     VJP_ERR_CUDA = -4         /* a CUDA runtime call or launch failed                        */
@@ -70,7 +76,8 @@ typedef struct {
     int32_t force_general; /* reduce-by-index only: != 0 routes '+', '*', min, max through the
                               general rule (sort + segmented scans, Fig. 4) instead
                               of their specialisation                            */
-    int32_t reserved;      /* must be 0                                                       */
+    int32_t accumulate;    /* VJP calls only: != 0 adds the contribution to the output instead of
+                              overwriting it               */
 } vjp_op_t;
 
 /* Scalars per scan element for op, or -1 if op is not a scan operator. */

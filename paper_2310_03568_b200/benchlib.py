@@ -35,7 +35,8 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
     table = {
         "rbi_vjp_add_kernel": 8 + elem_bytes,        # is + write vs_bar
         "rbi_minmax_lifted_kernel": 8 + 4 + 4,       # is + vs + zero-fill of vs_bar
-        "rbi_cached_kernel": 8 + 4,                  # is + vs
+        "rbi_cached_small_kernel": 8 + 4,            # is + vs
+        "rbi_cached_big_kernel": 8 + 4,
         "rbi_mul_sweep_kernel": 8 + 4 + 4,           # is + vs + write vs_bar
         "rbi_forward_kernel": 8 + elem_bytes,
         "scan_lookback_kernel<MODE_SCAN>": 2 * elem_bytes,

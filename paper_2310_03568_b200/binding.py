@@ -38,7 +38,7 @@ class VjpError(RuntimeError):
 
 class _OpStruct(ctypes.Structure):
     _fields_ = [("code", ctypes.c_int32), ("dtype", ctypes.c_int32), ("param", ctypes.c_double),
-                ("force_general", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("force_general", ctypes.c_int32), ("accumulate", ctypes.c_int32)]
 
 
 @dataclass(frozen=True)
@@ -48,13 +48,16 @@ class Op:
     dtype: int = F32
     param: float = 0.0
     force_general: bool = False
+    accumulate: bool = False   # VJP calls: out += contribution (the paper's "+=") instead of out = contribution
 
     @staticmethod
-    def of(name: str, dtype=torch.float32, S: float = 0.0, force_general: bool = False) -> "Op":
-        return Op(OPCODES[name], F64 if dtype in (torch.float64, F64) else F32, float(S), bool(force_general))
+    def of(name: str, dtype=torch.float32, S: float = 0.0, force_general: bool = False,
+           accumulate: bool = False) -> "Op":
+        return Op(OPCODES[name], F64 if dtype in (torch.float64, F64) else F32, float(S), bool(force_general),
+                  bool(accumulate))
 
     def c(self) -> _OpStruct:
-        return _OpStruct(self.code, self.dtype, self.param, int(self.force_general), 0)
+        return _OpStruct(self.code, self.dtype, self.param, int(self.force_general), int(self.accumulate))
 
     @property
     def torch_dtype(self):
@@ -73,9 +76,8 @@ def load() -> ctypes.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
-    if not os.path.exists(path) or os.environ.get("VJP_B200_REBUILD"):
-        path = _build.build()
+    # build() is an mtime check when the library is up to date; a stale binary is never loaded
+    path = _build.build(force=bool(os.environ.get("VJP_B200_REBUILD")))
     lib = ctypes.CDLL(path)
     vp, i64, sz, opp = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.POINTER(_OpStruct)
     sig = {
@@ -123,16 +125,38 @@ def _stream(stream=None):
     return ctypes.c_void_p(s.cuda_stream)
 
 
-def _dev(t: torch.Tensor, dtype) -> torch.Tensor:
+def _dev(t: torch.Tensor, dtype, numel=None, what="tensor") -> torch.Tensor:
+    """An input: CUDA, right dtype and size, made contiguous, 16-byte aligned (the kernels use 128-bit
+    accesses: a view such as x[1:] is rejected here instead of faulting on the device)."""
     if not t.is_cuda:
-        raise VjpError("expected a CUDA tensor (there is no CPU path)")
+        raise VjpError("%s: expected a CUDA tensor (there is no CPU path)" % what)
     if t.dtype != dtype:
-        raise VjpError("expected dtype %s, got %s" % (dtype, t.dtype))
-    return t.contiguous()
+        raise VjpError("%s: expected dtype %s, got %s" % (what, dtype, t.dtype))
+    if numel is not None and t.numel() != numel:
+        raise VjpError("%s: expected %d elements, got %d" % (what, numel, t.numel()))
+    t = t.contiguous()
+    if t.numel() and t.data_ptr() % 16:
+        raise VjpError("%s: data pointer is not 16-byte aligned" % what)
+    return t
 
 
-def _workspace(nbytes: int, device) -> torch.Tensor:
-    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+def _out(t, dtype, numel, device, what="out") -> torch.Tensor:
+    """A caller-supplied output (or None: allocate): must be usable in place."""
+    if t is None:
+        return torch.empty(numel, dtype=dtype, device=device)
+    if not t.is_cuda or t.device != device or t.dtype != dtype or t.numel() != numel or not t.is_contiguous():
+        raise VjpError("%s: expected a contiguous %s CUDA tensor of %d elements on %s" % (what, dtype, numel, device))
+    if t.numel() and t.data_ptr() % 16:
+        raise VjpError("%s: data pointer is not 16-byte aligned" % what)
+    return t
+
+
+def _workspace(nbytes: int, device, ws=None) -> torch.Tensor:
+    if ws is None:
+        return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+    if not ws.is_cuda or ws.dtype != torch.uint8 or not ws.is_contiguous() or ws.data_ptr() % 16:
+        raise VjpError("ws: expected a contiguous, 16-byte aligned uint8 CUDA tensor")
+    return ws
 
 
 def scan_arity(op: Op) -> int:
@@ -160,10 +184,10 @@ def vjp_scan_workspace_bytes(op: Op, n: int) -> int:
 
 def scan_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
     """Primal inclusive scan."""
-    xs = _dev(xs, op.torch_dtype)
+    xs = _dev(xs, op.torch_dtype, what="xs")
     n = _scan_n(op, xs)
-    ys = torch.empty_like(xs) if out is None else out
-    ws = _workspace(vjp_scan_workspace_bytes(op, n), xs.device) if ws is None else ws
+    ys = torch.empty_like(xs) if out is None else _out(out, op.torch_dtype, xs.numel(), xs.device)
+    ws = _workspace(vjp_scan_workspace_bytes(op, n), xs.device, ws)
     o = op.c()
     _check(load().scan_forward(ctypes.byref(o), n, _ptr(xs), _ptr(ys), _ptr(ws), ws.numel(), _stream(stream)),
            "scan_forward")
@@ -172,14 +196,16 @@ def scan_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=None) -> to
 
 def vjp_scan(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
     """xs_bar = J^T ys_bar of the inclusive scan (Fig. 7).  xs may be None for '+'."""
-    ys_bar = _dev(ys_bar, op.torch_dtype)
+    ys_bar = _dev(ys_bar, op.torch_dtype, what="ys_bar")
     if xs is not None:
-        xs = _dev(xs, op.torch_dtype)
+        xs = _dev(xs, op.torch_dtype, what="xs")
         if xs.shape != ys_bar.shape:
             raise VjpError("xs and ys_bar differ in shape")
     n = _scan_n(op, ys_bar)
-    xs_bar = torch.empty_like(ys_bar) if out is None else out
-    ws = _workspace(vjp_scan_workspace_bytes(op, n), ys_bar.device) if ws is None else ws
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    xs_bar = torch.empty_like(ys_bar) if out is None else _out(out, op.torch_dtype, ys_bar.numel(), ys_bar.device)
+    ws = _workspace(vjp_scan_workspace_bytes(op, n), ys_bar.device, ws)
     o = op.c()
     _check(load().vjp_scan(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                            _stream(stream)), "vjp_scan")
@@ -191,9 +217,21 @@ def vjp_scan_host_scratch_bytes(op: Op, n: int) -> int:
     return load().vjp_scan_host_scratch_bytes(ctypes.byref(o), n)
 
 
+def _host(t, dtype, numel, what):
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != dtype or t.numel() != numel or not t.is_contiguous():
+        raise VjpError("%s: expected a contiguous %s HOST tensor of %d elements" % (what, dtype, numel))
+    return t
+
+
 def vjp_scan_host(op: Op, xs, ys_bar: torch.Tensor, out: torch.Tensor, scratch: torch.Tensor, stream=None):
     """HOST tensors in and out (pinned for speed); `scratch` is a device uint8 tensor."""
     n = _scan_n(op, ys_bar)
+    _host(ys_bar, op.torch_dtype, ys_bar.numel(), "ys_bar")
+    _host(xs, op.torch_dtype, ys_bar.numel(), "xs")
+    _host(out, op.torch_dtype, ys_bar.numel(), "out")
+    scratch = _workspace(0, None, scratch)
     o = op.c()
     _check(load().vjp_scan_host(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(out), _ptr(scratch),
                                 scratch.numel(), _stream(stream)), "vjp_scan_host")
@@ -208,10 +246,11 @@ def vjp_reduce_by_index_workspace_bytes(op: Op, n: int, num_bins: int) -> int:
 def reduce_by_index_forward(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, out=None, ws=None,
                             stream=None) -> torch.Tensor:
     """Primal reduce_by_index over a neutral-initialised histogram."""
-    is_, vs = _dev(is_, torch.int64), _dev(vs, op.torch_dtype)
+    is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
-    hist = torch.empty(num_bins, dtype=op.torch_dtype, device=is_.device) if out is None else out
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    vs = _dev(vs, op.torch_dtype, n, "vs")
+    hist = _out(out, op.torch_dtype, num_bins, is_.device, "hist")
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
     o = op.c()
     _check(load().reduce_by_index_forward(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist),
                                           _ptr(ws), ws.numel(), _stream(stream)), "reduce_by_index_forward")
@@ -221,13 +260,15 @@ def reduce_by_index_forward(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.
 def vjp_reduce_by_index(op: Op, num_bins: int, is_: torch.Tensor, vs, hist_bar: torch.Tensor, out=None,
                         ws=None, stream=None) -> torch.Tensor:
     """vs_bar of reduce_by_index given hist_bar (Fig. 4 for the general rule)."""
-    is_ = _dev(is_, torch.int64)
-    hist_bar = _dev(hist_bar, op.torch_dtype)
-    if vs is not None:
-        vs = _dev(vs, op.torch_dtype)
+    is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
-    vs_bar = torch.empty(n, dtype=op.torch_dtype, device=is_.device) if out is None else out
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    hist_bar = _dev(hist_bar, op.torch_dtype, num_bins, "hist_bar")
+    if vs is not None:
+        vs = _dev(vs, op.torch_dtype, n, "vs")
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    vs_bar = _out(out, op.torch_dtype, n, is_.device, "vs_bar")
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
     o = op.c()
     _check(load().vjp_reduce_by_index(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
                                       _ptr(vs_bar), _ptr(ws), ws.numel(), _stream(stream)),
@@ -243,6 +284,9 @@ def vjp_reduce_by_index_host_scratch_bytes(op: Op, n: int, num_bins: int) -> int
 def vjp_reduce_by_index_host(op: Op, num_bins: int, is_, vs, hist_bar, out, scratch, stream=None):
     """HOST tensors in and out (pinned for speed); `scratch` is a device uint8 tensor."""
     n = is_.numel()
+    _host(is_, torch.int64, n, "is"), _host(vs, op.torch_dtype, n, "vs")
+    _host(hist_bar, op.torch_dtype, num_bins, "hist_bar"), _host(out, op.torch_dtype, n, "out")
+    scratch = _workspace(0, None, scratch)
     o = op.c()
     _check(load().vjp_reduce_by_index_host(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
                                            _ptr(out), _ptr(scratch), scratch.numel(), _stream(stream)),
@@ -253,6 +297,9 @@ def vjp_reduce_by_index_host(op: Op, num_bins: int, is_, vs, hist_bar, out, scra
 def vjp_reduce_by_index_host_async(op: Op, num_bins: int, is_, vs, hist_bar, out, scratch, stream=None):
     """As vjp_reduce_by_index_host, but only enqueued on `stream`: synchronise it before reading `out`."""
     n = is_.numel()
+    _host(is_, torch.int64, n, "is"), _host(vs, op.torch_dtype, n, "vs")
+    _host(hist_bar, op.torch_dtype, num_bins, "hist_bar"), _host(out, op.torch_dtype, n, "out")
+    scratch = _workspace(0, None, scratch)
     o = op.c()
     _check(load().vjp_reduce_by_index_host_async(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs),
                                                  _ptr(hist_bar), _ptr(out), _ptr(scratch), scratch.numel(),
@@ -262,11 +309,12 @@ def vjp_reduce_by_index_host_async(op: Op, num_bins: int, is_, vs, hist_bar, out
 
 def rbi_argext(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=None, stream=None):
     """(arg[w] int64 with n for an empty bin, ext[w]) of the lifted min/max primal (Fig. 5)."""
-    is_, vs = _dev(is_, torch.int64), _dev(vs, torch.float32)
+    is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
+    vs = _dev(vs, torch.float32, n, "vs")
     arg = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
     ext = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
     o = op.c()
     _check(load().rbi_argext(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(arg), _ptr(ext), _ptr(ws),
                              ws.numel(), _stream(stream)), "rbi_argext")
@@ -275,11 +323,12 @@ def rbi_argext(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=No
 
 def rbi_zero_prod(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=None, stream=None):
     """(zeros[w] int64, prod_nz[w]) of the lifted '*' primal."""
-    is_, vs = _dev(is_, torch.int64), _dev(vs, torch.float32)
+    is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
+    vs = _dev(vs, torch.float32, n, "vs")
     zeros = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
     prod = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device) if ws is None else ws
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
     o = op.c()
     _check(load().rbi_zero_prod(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(zeros), _ptr(prod),
                                 _ptr(ws), ws.numel(), _stream(stream)), "rbi_zero_prod")
@@ -288,12 +337,11 @@ def rbi_zero_prod(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws
 
 def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     """(sorted_keys, perm) of the stable sort by clamped key (Fig. 4)."""
-    is_ = _dev(is_, torch.int64)
+    is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
     sk = torch.empty(n, dtype=torch.int64, device=is_.device)
     perm = torch.empty(n, dtype=torch.int64, device=is_.device)
-    if ws is None:
-        ws = _workspace(vjp_reduce_by_index_workspace_bytes(Op(OP_SATADD), n, num_bins), is_.device)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(Op(OP_SATADD), n, num_bins), is_.device, ws)
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm

@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/vjp_b200.h: argument validation, workspace accounting and
 // dispatch.  No arithmetic of the method lives here.
+#include <cstdint>
 #include <cstring>
 
 #include "internal.h"
@@ -10,8 +11,12 @@ namespace {
 
 bool op_ok(const vjp_op_t *op) {
     return op && op->code >= VJP_OP_ADD && op->code <= VJP_OP_SATADD &&
-           (op->dtype == VJP_F32 || op->dtype == VJP_F64) && op->reserved == 0;
+           (op->dtype == VJP_F32 || op->dtype == VJP_F64);
 }
+// every data pointer must be 16-byte aligned (128-bit accesses); NULL passes (checked separately)
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+template <class... P>
+bool all_aligned(P... p) { return (aligned16(p) && ...); }
 size_t dtype_bytes(int dtype) { return dtype == VJP_F64 ? 8 : 4; }
 
 bool scan_supported(const vjp_op_t *op) {
@@ -49,7 +54,7 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEAGG>",
     "tile_exscan_kernel", "scan_vjp_reverse_kernel",
     "rbi_fill_kernel", "rbi_forward_kernel", "rbi_vjp_add_kernel",
-    "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_cached_kernel",
+    "rbi_minmax_lifted_kernel", "rbi_minmax_sample_kernel", "rbi_minmax_finish_kernel", "rbi_cached_small_kernel", "rbi_cached_big_kernel",
     "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel"};
@@ -136,7 +141,7 @@ int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys, void *
     if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
     if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
-    if (!xs || !ys || !ws) return VJP_ERR_INVALID_ARG;
+    if (!xs || !ys || !ws || !all_aligned(xs, ys, ws)) return VJP_ERR_INVALID_ARG;
     if (ws_bytes < scan_workspace_bytes(op->code, op->dtype, n)) return VJP_ERR_WORKSPACE;
     return launch_scan_forward(op->code, op->dtype, n, xs, ys, ws, as_stream(stream));
 }
@@ -147,8 +152,10 @@ int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, 
     if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
     if (!ys_bar || !xs_bar || !ws || (!xs && op->code != VJP_OP_ADD)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(xs, ys_bar, xs_bar, ws)) return VJP_ERR_INVALID_ARG;
+    if (xs_bar == ys_bar && (op->code != VJP_OP_ADD || op->accumulate)) return VJP_ERR_INVALID_ARG;  // in place: '+' only
     if (ws_bytes < scan_workspace_bytes(op->code, op->dtype, n)) return VJP_ERR_WORKSPACE;
-    return launch_scan_vjp(op->code, op->dtype, n, xs, ys_bar, xs_bar, ws, as_stream(stream));
+    return launch_scan_vjp(op->code, op->dtype, n, xs, ys_bar, xs_bar, ws, op->accumulate, as_stream(stream));
 }
 
 size_t vjp_scan_host_scratch_bytes(const vjp_op_t *op, int64_t n) {
@@ -164,6 +171,7 @@ int vjp_scan_host(const vjp_op_t *op, int64_t n, const void *xs_host, const void
     if (n == 0) return VJP_OK;
     if (!ys_bar_host || !xs_bar_host || !dev_scratch || (!xs_host && op->code != VJP_OP_ADD))
         return VJP_ERR_INVALID_ARG;
+    if (!aligned16(dev_scratch)) return VJP_ERR_INVALID_ARG;
     if (dev_scratch_bytes < vjp_scan_host_scratch_bytes(op, n)) return VJP_ERR_WORKSPACE;
     cudaStream_t s = as_stream(stream);
     const size_t bytes = (size_t)n * vjp_scan_arity(op) * dtype_bytes(op->dtype);
@@ -175,7 +183,10 @@ int vjp_scan_host(const vjp_op_t *op, int64_t n, const void *xs_host, const void
         return VJP_ERR_CUDA;
     if (cudaMemcpyAsync(dy, ys_bar_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
         return VJP_ERR_CUDA;
-    int rc = launch_scan_vjp(op->code, op->dtype, n, dx, dy, dout, ws, s);
+    if (op->accumulate &&
+        cudaMemcpyAsync(dout, xs_bar_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    int rc = launch_scan_vjp(op->code, op->dtype, n, dx, dy, dout, ws, op->accumulate, s);
     if (rc != VJP_OK) return rc;
     if (cudaMemcpyAsync(xs_bar_host, dout, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess)
         return VJP_ERR_CUDA;
@@ -204,6 +215,7 @@ int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, con
     if (rbi_route(op) == 0) return VJP_ERR_UNSUPPORTED;
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if ((num_bins > 0 && !hist) || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(is, vs, hist, ws)) return VJP_ERR_INVALID_ARG;
     if (num_bins > 0 && op->code != VJP_OP_ADD &&
         (!ws || ws_bytes < rbi_forward_workspace_bytes(op->code, n, num_bins)))
         return VJP_ERR_WORKSPACE;
@@ -220,23 +232,25 @@ int vjp_reduce_by_index(const vjp_op_t *op, int64_t n, int64_t num_bins, const i
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
     if (!is || !vs_bar || (num_bins > 0 && !hist_bar) || (!vs && route != 1)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(is, vs, hist_bar, vs_bar, ws)) return VJP_ERR_INVALID_ARG;
     if (!ws || ws_bytes < vjp_reduce_by_index_workspace_bytes(op, n, num_bins)) return VJP_ERR_WORKSPACE;
     cudaStream_t s = as_stream(stream);
+    const int acc = op->accumulate != 0;
     switch (route) {
-    case 1: return launch_rbi_vjp_add(op->dtype, n, num_bins, is, hist_bar, vs_bar, s);
+    case 1: return launch_rbi_vjp_add(op->dtype, n, num_bins, is, hist_bar, vs_bar, acc, s);
     case 2:
         return launch_rbi_minmax(op->code, n, num_bins, is, static_cast<const float *>(vs),
                                  static_cast<const float *>(hist_bar), static_cast<float *>(vs_bar),
-                                 nullptr, nullptr, ws, s);
+                                 nullptr, nullptr, ws, acc, s);
     case 3:
         return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs),
                               static_cast<const float *>(hist_bar), static_cast<float *>(vs_bar),
-                              nullptr, nullptr, ws, s);
+                              nullptr, nullptr, ws, acc, s);
     default:
         return launch_rbi_general_vjp(op->code, op->param, n, num_bins, is,
                                       static_cast<const float *>(vs),
                                       static_cast<const float *>(hist_bar),
-                                      static_cast<float *>(vs_bar), ws, s);
+                                      static_cast<float *>(vs_bar), ws, acc, s);
     }
 }
 
@@ -254,7 +268,10 @@ int vjp_reduce_by_index_host_async(const vjp_op_t *op, int64_t n, int64_t num_bi
     if (!op_ok(op) || n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
     const int route = rbi_route(op);
     if (route == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;  // before anything is enqueued
+    if (route == 3 && !rbi_cached_supported(num_bins)) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
+    if (!aligned16(dev_scratch)) return VJP_ERR_INVALID_ARG;
     if (!is_host || !vs_bar_host || !dev_scratch || (num_bins > 0 && !hist_bar_host) ||
         (!vs_host && route != 1))
         return VJP_ERR_INVALID_ARG;
@@ -276,6 +293,9 @@ int vjp_reduce_by_index_host_async(const vjp_op_t *op, int64_t n, int64_t num_bi
         return VJP_ERR_CUDA;
     if (num_bins > 0 &&
         cudaMemcpyAsync(dhb, hist_bar_host, (size_t)num_bins * e, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    if (op->accumulate &&
+        cudaMemcpyAsync(dout, vs_bar_host, (size_t)n * e, cudaMemcpyHostToDevice, s) != cudaSuccess)
         return VJP_ERR_CUDA;
     int rc = vjp_reduce_by_index(op, n, num_bins, reinterpret_cast<const int64_t *>(dis), dvs, dhb,
                                  dout, ws, ws_bytes, stream);
@@ -303,10 +323,11 @@ int rbi_argext(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *i
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if (num_bins == 0) return VJP_OK;
     if (!arg || !ext || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(is, vs, arg, ext, ws)) return VJP_ERR_INVALID_ARG;
     if (!ws || ws_bytes < rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins))
         return VJP_ERR_WORKSPACE;
     return launch_rbi_minmax(op->code, n, num_bins, is, static_cast<const float *>(vs), nullptr,
-                             nullptr, arg, static_cast<float *>(ext), ws, as_stream(stream));
+                             nullptr, arg, static_cast<float *>(ext), ws, 0, as_stream(stream));
 }
 
 int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
@@ -317,10 +338,11 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if (num_bins == 0) return VJP_OK;
     if (!zeros || !prod_nz || (n > 0 && (!is || !vs))) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(is, vs, zeros, prod_nz, ws)) return VJP_ERR_INVALID_ARG;
     if (!ws || ws_bytes < rbi_special_workspace_bytes(op->code, op->dtype, n, num_bins))
         return VJP_ERR_WORKSPACE;
     return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs), nullptr, nullptr, zeros,
-                          static_cast<float *>(prod_nz), ws, as_stream(stream));
+                          static_cast<float *>(prod_nz), ws, 0, as_stream(stream));
 }
 
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
@@ -328,7 +350,7 @@ int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorte
     if (n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
     if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
-    if (!is || !sorted_keys || !perm) return VJP_ERR_INVALID_ARG;
+    if (!is || !sorted_keys || !perm || !all_aligned(is, sorted_keys, perm, ws)) return VJP_ERR_INVALID_ARG;
     if (!ws || ws_bytes < rbi_general_workspace_bytes(n, num_bins)) return VJP_ERR_WORKSPACE;
     return launch_rbi_sort_perm(n, num_bins, is, sorted_keys, perm, ws, as_stream(stream));
 }

@@ -16,23 +16,6 @@ constexpr int NUM_SMS_B200 = 148;
 
 // ------------------------------------------------------------------ memory ordering ----
 
-VJP_DEVINL void st_release_s32(int *p, int v) {
-    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-VJP_DEVINL int ld_acquire_s32(const int *p) {
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-VJP_DEVINL unsigned ld_relaxed_u32(const unsigned *p) {
-    unsigned v;
-    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-VJP_DEVINL void st_relaxed_u32(unsigned *p, unsigned v) {
-    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
 // streaming 128-bit accesses (data touched once: do not keep it in L1)
 VJP_DEVINL uint4 ldg_stream(const uint4 *p) {
     uint4 r;
@@ -45,18 +28,6 @@ VJP_DEVINL void stg_stream(uint4 *p, const uint4 &v) {
     asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x),
                  "r"(v.y), "r"(v.z), "r"(v.w)
                  : "memory");
-}
-
-// asynchronous 16-byte global -> shared copies (LDGSTS): the next tile is fetched while the current
-// one is processed
-VJP_DEVINL void cp_async16(void *smem_dst, const void *gsrc) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
-}
-VJP_DEVINL void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-VJP_DEVINL void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
 // ------------------------------------------------------------------ POD word helpers ---
@@ -263,6 +234,39 @@ VJP_DEVINL typename M::State lookback_warp(const TileSlots<typename M::State> &t
     return acc;
 }
 
+// 16 bytes of T plus 16 bytes of T (the "+=" of an accumulating VJP call, fused into the final store)
+template <class T>
+VJP_DEVINL uint4 chunk_add(const uint4 &a, const uint4 &b);
+template <>
+VJP_DEVINL uint4 chunk_add<float>(const uint4 &a, const uint4 &b) {
+    return make_uint4(__float_as_uint(__uint_as_float(a.x) + __uint_as_float(b.x)),
+                      __float_as_uint(__uint_as_float(a.y) + __uint_as_float(b.y)),
+                      __float_as_uint(__uint_as_float(a.z) + __uint_as_float(b.z)),
+                      __float_as_uint(__uint_as_float(a.w) + __uint_as_float(b.w)));
+}
+template <>
+VJP_DEVINL uint4 chunk_add<double>(const uint4 &a, const uint4 &b) {
+    const double x = __hiloint2double((int)a.y, (int)a.x) + __hiloint2double((int)b.y, (int)b.x);
+    const double y = __hiloint2double((int)a.w, (int)a.z) + __hiloint2double((int)b.w, (int)b.z);
+    return make_uint4((uint32_t)__double2loint(x), (uint32_t)__double2hiint(x), (uint32_t)__double2loint(y),
+                      (uint32_t)__double2hiint(y));
+}
+// one element of T at word offset wi of g: g = (acc ? g : 0) + the words at s
+template <class T>
+VJP_DEVINL void elem_store(uint32_t *g, const uint32_t *s, bool acc);
+template <>
+VJP_DEVINL void elem_store<float>(uint32_t *g, const uint32_t *s, bool acc) {
+    const float x = __uint_as_float(s[0]);
+    g[0] = __float_as_uint(acc ? __uint_as_float(g[0]) + x : x);
+}
+template <>
+VJP_DEVINL void elem_store<double>(uint32_t *g, const uint32_t *s, bool acc) {
+    double x = __hiloint2double((int)s[1], (int)s[0]);
+    if (acc) x += __hiloint2double((int)g[1], (int)g[0]);
+    g[0] = (uint32_t)__double2loint(x);
+    g[1] = (uint32_t)__double2hiint(x);
+}
+
 // ------------------------------------------------------------------ tile staging -------
 //
 // A tile is NT rows (one per thread) of RW 32-bit words; in shared memory a row has a pitch
@@ -305,27 +309,26 @@ struct TileStage {
         }
     }
 
-    // Whole tile, asynchronously (the caller commits and waits).
-    static VJP_DEVINL void load_async(uint4 *smem, const uint32_t *__restrict__ g) {
-        const uint4 *g4 = reinterpret_cast<const uint4 *>(g);
-#pragma unroll
-        for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) cp_async16(smem + smem_chunk(c), g4 + c);
-    }
-
-    // Store the first `valid_words` words of the staged tile to `g`.
-    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words) {
+    // Store the first `valid_words` words of the staged tile (elements of type T) to `g`; acc: g += tile.
+    template <class T>
+    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words, bool acc) {
         uint4 *g4 = reinterpret_cast<uint4 *>(g);
         if (valid_words == TILE_WORDS) {
 #pragma unroll
-            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) stg_stream(g4 + c, smem[smem_chunk(c)]);
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) {
+                uint4 v = smem[smem_chunk(c)];
+                if (acc) v = chunk_add<T>(v, g4[c]);
+                stg_stream(g4 + c, v);
+            }
         } else {
+            constexpr int TW = sizeof(T) / 4;
             for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) {
                 const uint4 v = smem[smem_chunk(c)];
                 const uint32_t w[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
-                for (int j = 0; j < 4; j++) {
+                for (int j = 0; j < 4; j += TW) {
                     const int wi = c * 4 + j;
-                    if (wi < valid_words) g[wi] = w[j];
+                    if (wi < valid_words) elem_store<T>(g + wi, w + j, acc);
                 }
             }
         }
@@ -374,19 +377,20 @@ struct TileStageLinear {
                 s[wi] = (wi < valid_words) ? __ldg(g + wi) : fill[wi % FW];
         }
     }
-    static VJP_DEVINL void load_async(uint4 *smem, const uint32_t *__restrict__ g) {
-        const uint4 *g4 = reinterpret_cast<const uint4 *>(g);
-#pragma unroll
-        for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) cp_async16(smem + c, g4 + c);
-    }
-    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words) {
+    template <class T>
+    static VJP_DEVINL void store(const uint4 *smem, uint32_t *__restrict__ g, int valid_words, bool acc) {
+        static_assert(sizeof(T) == 4, "linear tiles hold f32 elements");
         uint4 *g4 = reinterpret_cast<uint4 *>(g);
         if (valid_words == TILE_WORDS) {
 #pragma unroll
-            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) stg_stream(g4 + c, smem[c]);
+            for (int c = threadIdx.x; c < TILE_CHUNKS; c += NT) {
+                uint4 v = smem[c];
+                if (acc) v = chunk_add<T>(v, g4[c]);
+                stg_stream(g4 + c, v);
+            }
         } else {
             const uint32_t *s = reinterpret_cast<const uint32_t *>(smem);
-            for (int wi = threadIdx.x; wi < valid_words; wi += NT) g[wi] = s[wi];
+            for (int wi = threadIdx.x; wi < valid_words; wi += NT) elem_store<T>(g + wi, s + wi, acc);
         }
     }
     static VJP_DEVINL uint32_t *row_ptr(uint4 *smem, int row) {

@@ -24,9 +24,9 @@ inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 // Every kernel launch of the library goes through a LaunchScope: it counts the launch and, while
 // profiling is enabled (vjp_profile_enable), brackets it with CUDA events on the launching stream.
 enum KernelId : int {
-    K_SCAN_LOOKBACK = 0, K_SCAN_TILEAGG, K_SCAN_TILEPRE, K_SCAN_VJP_REVERSE,
+    K_SCAN_LOOKBACK = 0, K_SCAN_TILEAGG, K_SCAN_TILEPRE /* tile_exscan_kernel */, K_SCAN_VJP_REVERSE,
     K_RBI_FILL, K_RBI_FORWARD, K_RBI_GATHER,
-    K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_ACC, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
+    K_MINMAX_LIFTED, K_MINMAX_SAMPLE, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_COUNT
 };
@@ -46,7 +46,7 @@ size_t scan_workspace_bytes(int code, int dtype, int64_t n);
 int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,
                         cudaStream_t stream);
 int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *ys_bar,
-                    void *xs_bar, void *ws, cudaStream_t stream);
+                    void *xs_bar, void *ws, int accumulate, cudaStream_t stream);
 
 // -------------------------------------------------------------- reduce-by-index (special) -
 size_t rbi_special_workspace_bytes(int code, int dtype, int64_t n, int64_t w);
@@ -55,21 +55,21 @@ bool rbi_cached_supported(int64_t w);  // '*' / satadd tables: w <= 2^20
 int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, const int64_t *is,
                        const void *vs, void *hist, void *ws, cudaStream_t stream);
 int launch_rbi_vjp_add(int dtype, int64_t n, int64_t w, const int64_t *is, const void *hist_bar,
-                       void *vs_bar, cudaStream_t stream);
+                       void *vs_bar, int accumulate, cudaStream_t stream);
 // MIN / MAX: lifted primal into ws, then (arg, ext) and / or the return sweep.
 int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const float *vs,
                       const float *hist_bar, float *vs_bar, int64_t *arg, float *ext, void *ws,
-                      cudaStream_t stream);
+                      int accumulate, cudaStream_t stream);
 // MUL: lifted primal into ws, then (zeros, prod_nz) and / or the return sweep.
 int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
                    const float *hist_bar, float *vs_bar, int64_t *zeros, float *prod_nz, void *ws,
-                   cudaStream_t stream);
+                   int accumulate, cudaStream_t stream);
 
 // -------------------------------------------------------------- reduce-by-index (general) -
 size_t rbi_general_workspace_bytes(int64_t n, int64_t w);
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
                            const float *vs, const float *hist_bar, float *vs_bar, void *ws,
-                           cudaStream_t stream);
+                           int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
                          int64_t *perm, void *ws, cudaStream_t stream);
 

@@ -427,7 +427,7 @@ seg_forward_kernel(int64_t n, const uint32_t *__restrict__ keys, const uint2 *__
     __syncthreads();  // every thread has read its key row
     KS::write_row(sk, threadIdx.x, out);
     __syncthreads();
-    KS::store(sk, reinterpret_cast<uint32_t *>(ls) + base, valid);
+    KS::template store<float>(sk, reinterpret_cast<uint32_t *>(ls) + base, valid, false);
 }
 
 // G5-G7 fused: reverse segmented exclusive scan, per-element derivative, un-permute.
@@ -436,7 +436,7 @@ __global__ void __launch_bounds__(SEG_NT)
 seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
                        const uint2 *__restrict__ pay, const float *__restrict__ ls,
                        const float *__restrict__ hist_bar, float *__restrict__ vs_bar,
-                       GenOp<CODE> op, int num_tiles, int *ticket, uint64_t *status) {
+                       GenOp<CODE> op, int num_tiles, int *ticket, uint64_t *status, int accumulate) {
     using KS = Stage<SEG_NT, SEG_IPT>;
     using PS = Stage<SEG_NT, 2 * SEG_IPT>;
     extern __shared__ uint4 smem[];
@@ -497,7 +497,7 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
             float g = 0.f;
             if (k[j] < (uint32_t)w)  // out-of-range keys were clamped to w: adjoint 0
                 g = op.dfdx(__uint_as_float(lw[j]), v, r) * __ldg(hist_bar + k[j]);
-            vs_bar[pw[2 * j]] = g;
+            vs_bar[pw[2 * j]] = accumulate ? vs_bar[pw[2 * j]] + g : g;  // the permutation names every index once
         }
     }
 }
@@ -596,7 +596,7 @@ static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, co
 
 template <int CODE>
 static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
-                       const float *hist_bar, float *vs_bar, const GenWs &g, cudaStream_t stream) {
+                       const float *hist_bar, float *vs_bar, const GenWs &g, int accumulate, cudaStream_t stream) {
     int buf;
     int rc = run_sort(n, w, is, vs, g, &buf, stream);
     if (rc != VJP_OK) return rc;
@@ -615,22 +615,22 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
         n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
     VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, REV_SMEM, stream>>>(
-        n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status);
+        n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status, accumulate);
     return last_launch_status();
 }
 
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
                            const float *vs, const float *hist_bar, float *vs_bar, void *ws,
-                           cudaStream_t stream) {
+                           int accumulate, cudaStream_t stream) {
     if (n == 0) return VJP_OK;
     const GenWs g = gen_carve(ws, n);
     const float S = (float)param;
     switch (code) {
-    case VJP_OP_ADD: return run_general<G_ADD>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
-    case VJP_OP_MIN: return run_general<G_MIN>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
-    case VJP_OP_MAX: return run_general<G_MAX>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
-    case VJP_OP_MUL: return run_general<G_MUL>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
-    case VJP_OP_SATADD: return run_general<G_SATADD>(S, n, w, is, vs, hist_bar, vs_bar, g, stream);
+    case VJP_OP_ADD: return run_general<G_ADD>(S, n, w, is, vs, hist_bar, vs_bar, g, accumulate, stream);
+    case VJP_OP_MIN: return run_general<G_MIN>(S, n, w, is, vs, hist_bar, vs_bar, g, accumulate, stream);
+    case VJP_OP_MAX: return run_general<G_MAX>(S, n, w, is, vs, hist_bar, vs_bar, g, accumulate, stream);
+    case VJP_OP_MUL: return run_general<G_MUL>(S, n, w, is, vs, hist_bar, vs_bar, g, accumulate, stream);
+    case VJP_OP_SATADD: return run_general<G_SATADD>(S, n, w, is, vs, hist_bar, vs_bar, g, accumulate, stream);
     default: return VJP_ERR_UNSUPPORTED;
     }
 }

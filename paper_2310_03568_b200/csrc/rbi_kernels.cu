@@ -81,6 +81,18 @@ VJP_DEVINL void store_vals4(double *__restrict__ out, int64_t i, int cnt, const 
     for (int j = 0; j < cnt; j++) out[i + j] = v[j];
 }
 
+// vs_bar[i..i+cnt) = (acc ? vs_bar : 0) + v: the "+=" of an accumulating call fused into the store
+template <class T>
+VJP_DEVINL void store_adj4(T *__restrict__ out, int64_t i, int cnt, T (&v)[4], bool acc) {
+    if (acc) {
+        T p[4];
+        load_vals4(out, i, cnt, p);
+#pragma unroll
+        for (int j = 0; j < 4; j++) v[j] += p[j];
+    }
+    store_vals4(out, i, cnt, v);
+}
+
 VJP_DEVINL bool in_range(int64_t k, int64_t w) { return (uint64_t)k < (uint64_t)w; }
 
 static int grid_for(int64_t n, int nt, int ctas_per_sm) {
@@ -210,7 +222,7 @@ int launch_rbi_forward(int code, int dtype, double param, int64_t n, int64_t w, 
     case VJP_OP_MIN:  // the packed-key kernels of the lifted operator, value part only
     case VJP_OP_MAX:
         return launch_rbi_minmax(code, n, w, is, static_cast<const float *>(vs), nullptr, nullptr, nullptr,
-                                 static_cast<float *>(hist), ws, stream);
+                                 static_cast<float *>(hist), ws, 0, stream);
     case VJP_OP_MUL:
     case VJP_OP_SATADD:
         return launch_cached_primal(code, n, w, is, static_cast<const float *>(vs),
@@ -226,7 +238,7 @@ constexpr size_t GATHER_SMEM_MAX = 64 * 1024;
 template <class T, bool SMEM>
 __global__ void __launch_bounds__(RBI_NT)
 rbi_vjp_add_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
-                   const T *__restrict__ hist_bar, T *__restrict__ vs_bar) {
+                   const T *__restrict__ hist_bar, T *__restrict__ vs_bar, int accumulate) {
     extern __shared__ uint4 smem_raw[];
     T *sh = reinterpret_cast<T *>(smem_raw);
     if (SMEM) {
@@ -241,29 +253,29 @@ rbi_vjp_add_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 #pragma unroll
         for (int j = 0; j < 4; j++)
             o[j] = in_range(k[j], w) ? (SMEM ? sh[k[j]] : __ldg(hist_bar + k[j])) : T(0);
-        store_vals4(vs_bar, q * 4, cnt, o);
+        store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
     }
 }
 
 template <class T>
 static int run_vjp_add(int64_t n, int64_t w, const int64_t *is, const void *hist_bar, void *vs_bar,
-                       cudaStream_t stream) {
+                       int accumulate, cudaStream_t stream) {
     const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
     const size_t bytes = (size_t)w * sizeof(T);
     if (bytes <= GATHER_SMEM_MAX / 2) {
         VJP_LAUNCH(K_RBI_GATHER, stream) rbi_vjp_add_kernel<T, true><<<grid, RBI_NT, bytes, stream>>>(
-            n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar));
+            n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar), accumulate);
     } else {
         VJP_LAUNCH(K_RBI_GATHER, stream) rbi_vjp_add_kernel<T, false><<<grid, RBI_NT, 0, stream>>>(
-            n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar));
+            n, w, is, static_cast<const T *>(hist_bar), static_cast<T *>(vs_bar), accumulate);
     }
     return last_launch_status();
 }
 
 int launch_rbi_vjp_add(int dtype, int64_t n, int64_t w, const int64_t *is, const void *hist_bar,
-                       void *vs_bar, cudaStream_t stream) {
-    return dtype == VJP_F32 ? run_vjp_add<float>(n, w, is, hist_bar, vs_bar, stream)
-                            : run_vjp_add<double>(n, w, is, hist_bar, vs_bar, stream);
+                       void *vs_bar, int accumulate, cudaStream_t stream) {
+    return dtype == VJP_F32 ? run_vjp_add<float>(n, w, is, hist_bar, vs_bar, accumulate, stream)
+                            : run_vjp_add<double>(n, w, is, hist_bar, vs_bar, accumulate, stream);
 }
 
 // ------------------------------------------------------------------ min / max VJP ---------
@@ -335,22 +347,23 @@ template <bool IS_MAX, bool TAGGED>
 __global__ void __launch_bounds__(MMF_NT, 1)
 rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                            const float *__restrict__ vs, unsigned long long *tab,
+                           const uint4 *__restrict__ seed /* [8192] packed 16-bit bounds, or NULL */,
                            float *__restrict__ vs_bar) {
     extern __shared__ uint4 smem_raw[];
     uint16_t *f16 = reinterpret_cast<uint16_t *>(smem_raw);  // [65536]
     uint32_t *f32 = reinterpret_cast<uint32_t *>(smem_raw);  // [32768]
-    for (int k = threadIdx.x; k < (int)(MMF_SMEM / 16); k += MMF_NT)
-        smem_raw[k] = make_uint4(~0u, ~0u, ~0u, ~0u);
-    __syncthreads();
     const int64_t stride = (int64_t)gridDim.x * MMF_NT;
     int64_t q = blockIdx.x * (int64_t)MMF_NT + threadIdx.x;
     int64_t k[4] = {-1, -1, -1, -1};
     float v[4] = {0.f, 0.f, 0.f, 0.f};
     int cnt = 0;
-    if (q * 4 < n) {
+    if (q * 4 < n) {  // the first loads fly while the filter is initialised
         cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
     }
+    for (int i = threadIdx.x; i < (int)(MMF_SMEM / 16); i += MMF_NT)
+        smem_raw[i] = (!TAGGED && seed) ? __ldg(seed + i) : make_uint4(~0u, ~0u, ~0u, ~0u);
+    __syncthreads();
     while (q * 4 < n) {
         // next iteration's loads fly while this one walks the table (its L2 round trips are dependent)
         int64_t kn[4] = {-1, -1, -1, -1};
@@ -371,9 +384,10 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             const uint32_t vk = ext_key<IS_MAX>(v[j]);
             const uint32_t p16 = vk >> 16;
             const uint32_t b = (uint32_t)k[j];
+            const bool wide = TAGGED && (b >> 31);  // the 16-bit tag cannot name bins >= 2^31: no filter
             if (TAGGED) {
                 const uint32_t e = f32[b & 32767u];
-                if ((e >> 16) == (b >> 15) && p16 > (e & 0xffffu)) continue;
+                if (!wide && (e >> 16) == (b >> 15) && p16 > (e & 0xffffu)) continue;
             } else {
                 if (p16 > f16[b]) continue;
             }
@@ -384,8 +398,11 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                 if (key < cur) cur = key;
             }
             const uint32_t c16 = (uint32_t)(cur >> 48);
-            if (TAGGED) f32[b & 32767u] = ((b >> 15) << 16) | c16;
-            else f16[b] = (uint16_t)c16;
+            if (TAGGED) {
+                if (!wide) f32[b & 32767u] = ((b >> 15) << 16) | c16;
+            } else {
+                f16[b] = (uint16_t)c16;
+            }
         }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
@@ -397,12 +414,46 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
+// Seeding of the filter (w <= 65536).  With 148 private filters a CTA sees a bin of a wide histogram
+// only a few times (uniform keys, w = 2^16, n = 2^24: 1.7 times), so a filter that starts empty lets
+// most elements through to L2 (profiles/r1l: one dependent L2 sector read per element, 34 % DRAM).  A
+// SAMPLE pass first runs the lifted operator over every 16th block of 1024 elements -- the packed keys
+// it leaves in `tab` are valid partial results, the main pass simply continues from them -- and the
+// 16-bit prefixes of those keys become the initial bound of every CTA's filter: an element then passes
+// with probability ~ 1/17 instead of ~ 1/1.7.
+constexpr int MMS_NT = 256, MMS_EVERY = 16;
+
+template <bool IS_MAX>
+__global__ void __launch_bounds__(MMS_NT)
+rbi_minmax_sample_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                         const float *__restrict__ vs, unsigned long long *tab) {
+    const int64_t q = ((int64_t)blockIdx.x * MMS_EVERY) * MMS_NT + threadIdx.x;
+    if (q * 4 >= n) return;
+    int64_t k[4];
+    float v[4];
+    const int cnt = load_keys4(is, q * 4, n, k);
+    load_vals4(vs, q * 4, cnt, v);
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        if (!in_range(k[j], w)) continue;
+        const unsigned long long key =
+            ((unsigned long long)ext_key<IS_MAX>(v[j]) << 32) | (unsigned)(q * 4 + j);
+        if (key < __ldcg(tab + k[j])) atomicMin(tab + k[j], key);
+    }
+}
+
+__global__ void rbi_minmax_seed_kernel(int64_t w, const unsigned long long *__restrict__ tab,
+                                       uint16_t *__restrict__ seed /* [65536] */) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < 65536) seed[k] = k < w ? (uint16_t)(__ldcg(tab + k) >> 48) : (uint16_t)0xffffu;
+}
+
 // arg / ext of every bin (an empty bin is (n, +-inf)) and the scatter of the return sweep
 // (P:L438-441).  vs_bar has been zeroed before.
 template <bool IS_MAX>
 __global__ void rbi_minmax_finish_kernel(int64_t n, int64_t w, const unsigned long long *tab,
                                          const float *__restrict__ hist_bar, float *vs_bar,
-                                         int64_t *arg, float *ext) {
+                                         int64_t *arg, float *ext, int accumulate) {
     for (int64_t k = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; k < w;
          k += (int64_t)gridDim.x * blockDim.x) {
         const unsigned long long key = tab[k];
@@ -412,17 +463,21 @@ __global__ void rbi_minmax_finish_kernel(int64_t n, int64_t w, const unsigned lo
         if (ext)
             ext[k] = empty ? (IS_MAX ? -CUDART_INF_F : CUDART_INF_F)
                            : ext_value<IS_MAX>((uint32_t)(key >> 32));
-        if (vs_bar && !empty) vs_bar[idx] = hist_bar[k];
+        if (vs_bar && !empty) vs_bar[idx] = accumulate ? vs_bar[idx] + hist_bar[k] : hist_bar[k];  // one bin per index
     }
 }
 
 constexpr size_t MINMAX_SMEM_MAX = 64 * 1024;
+// packed keys [w] + (8192 < w <= 65536) the 65536 16-bit filter seeds
+static size_t minmax_ws_bytes(int64_t w) { return align_up((size_t)w * 8, 256) + ((size_t)w * 8 > MINMAX_SMEM_MAX && w <= 65536 ? 65536 * 2 : 0); }
 
 template <bool IS_MAX>
 static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
-                      const float *hist_bar, float *vs_bar, int64_t *arg, float *ext, void *ws,
-                      cudaStream_t stream) {
+                      const float *hist_bar, float *vs_bar_out, int64_t *arg, float *ext, void *ws,
+                      int accumulate, cudaStream_t stream) {
     unsigned long long *tab = static_cast<unsigned long long *>(ws);
+    // accumulate: the lifted pass does not zero-fill vs_bar, the finish kernel adds instead of storing
+    float *vs_bar = accumulate ? nullptr : vs_bar_out;
     if (w == 0) {  // no bins: every adjoint is 0
         if (vs_bar && n > 0 &&
             cudaMemsetAsync(vs_bar, 0, (size_t)n * sizeof(float), stream) != cudaSuccess)
@@ -444,24 +499,32 @@ static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
             auto kern = rbi_minmax_filtered_kernel<IS_MAX, false>;
             if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
                 return VJP_ERR_CUDA;
-            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
+            const uint4 *seed = nullptr;
+            const int64_t quads = (n + 3) / 4, sblocks = (quads + (int64_t)MMS_NT * MMS_EVERY - 1) / ((int64_t)MMS_NT * MMS_EVERY);
+            if (sblocks >= 64) {  // enough input for the sample to be worth two more launches
+                uint16_t *seed16 = reinterpret_cast<uint16_t *>(static_cast<char *>(ws) + align_up((size_t)w * 8, 256));
+                VJP_LAUNCH(K_MINMAX_SAMPLE, stream) rbi_minmax_sample_kernel<IS_MAX><<<(unsigned)sblocks, MMS_NT, 0, stream>>>(n, w, is, vs, tab);
+                VJP_LAUNCH(K_MINMAX_SAMPLE, stream) rbi_minmax_seed_kernel<<<256, 256, 0, stream>>>(w, tab, seed16);
+                seed = reinterpret_cast<const uint4 *>(seed16);
+            }
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, seed, vs_bar);
         } else {
             auto kern = rbi_minmax_filtered_kernel<IS_MAX, true>;
             if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
                 return VJP_ERR_CUDA;
-            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, nullptr, vs_bar);
         }
     }
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
-    VJP_LAUNCH(K_MINMAX_FINISH, stream) rbi_minmax_finish_kernel<IS_MAX><<<fb, 256, 0, stream>>>(n, w, tab, hist_bar, vs_bar, arg, ext);
+    VJP_LAUNCH(K_MINMAX_FINISH, stream) rbi_minmax_finish_kernel<IS_MAX><<<fb, 256, 0, stream>>>(n, w, tab, hist_bar, vs_bar_out, arg, ext, accumulate);
     return last_launch_status();
 }
 
 int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const float *vs,
                       const float *hist_bar, float *vs_bar, int64_t *arg, float *ext, void *ws,
-                      cudaStream_t stream) {
-    return code == VJP_OP_MAX ? run_minmax<true>(n, w, is, vs, hist_bar, vs_bar, arg, ext, ws, stream)
-                              : run_minmax<false>(n, w, is, vs, hist_bar, vs_bar, arg, ext, ws, stream);
+                      int accumulate, cudaStream_t stream) {
+    return code == VJP_OP_MAX ? run_minmax<true>(n, w, is, vs, hist_bar, vs_bar, arg, ext, ws, accumulate, stream)
+                              : run_minmax<false>(n, w, is, vs, hist_bar, vs_bar, arg, ext, ws, accumulate, stream);
 }
 
 
@@ -471,28 +534,35 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
 // Operators with no hardware atomic (the paper's "atomicMul-class update").  One
 // shared-memory atomicCAS per element is not affordable: ATOMS costs 2 cycles per lane on the SM's
 // LSU pipe, 64x a plain LDS/STS, and a CAS loop on a hot bin retries without bound (profiles/r1a:
-// 5 ms at Zipf keys).  match.any is no way out either: it issues about once per 30 cycles per SM
-// (profiles/r1b).  So every WARP owns a private direct-mapped write-back cache of (bin, partial
-// result) entries in shared memory that it updates with plain loads and stores only:
-//   1. the lanes of a warp arbitrate per slot through a claim byte: every pending lane stores its
-//      lane id, the warp syncs, the lane that reads its own id back owns the slot for this round
-//      and does a plain read-modify-write; the others retry.  Rounds = the largest number of lanes
-//      on one slot (1-2 for uniform keys, ~6 when one bin holds 18 % of the elements);
-//   2. hit: combine in place.  Miss: a 2-bit hit counter guards the resident entry -- a cold bin
-//      arriving at a hot slot decrements it and BYPASSES; only an entry whose counter has run out
-//      is evicted (Misra-Gries style), so hot bins stay resident whatever the key distribution;
-//   3. w > CS_SLOTS: the caches sit in front of the CTA's table in shared memory, which takes the
-//      cold elements by CTA-wide claim rounds (rbi_cached_big_kernel below) -- only the evictions /
-//      bypasses of the caches (rare) use a CAS loop.
-// With w <= CS_SLOTS a slot IS a bin: no tags, no evictions, no atomics at all.  CTA g writes its
-// result to part[g][.]; a second kernel folds the G tables per bin in a fixed order (deterministic).
+// 5 ms at Zipf keys); match.any issues about once per 30 cycles per SM (profiles/r1b).  So tables
+// in shared memory are updated with plain loads and stores under a CLAIM ROUND:
+//   A. every pending element reads its bin's cell and, unless the cell already holds a claim,
+//      overwrites it with a claim word naming the element -- a NaN-boxed pattern (sign 1, exponent
+//      0xff, mantissa 0x7xxxxx | id) that no value the operators produce ever has (NaN inputs are
+//      unsupported; FMUL / FADD generate the canonical NaN 0x7fffffff).  No separate claim array.
+//   B. after a barrier the element that reads its own claim back OWNS the bin for this round and
+//      stores comb(old value, its value); every claimed cell has exactly one owner (the last
+//      claim written), and every claim writer has read the cell's real value (values only change
+//      in B, claims only appear in A).  Uniform keys: 3 - 6 % of the elements lose.
+//   C. losers: one compare-and-swap loop on the cell (few, uncontended at uniform keys).
+// Skewed keys would make C the whole kernel, so every WARP keeps a small DIRECTORY of hot bins
+// (DIR_S direct-mapped slots) whose accumulators are LANE-PRIVATE (hot[slot][lane]: bank = lane):
+// an element of a resident bin is folded into its lane's accumulator with a plain read-modify-write
+// -- no claim, no conflict, whatever the multiplicity of the bin.  The directory is trained by the
+// warp itself: a bin seen contended twice and hotter (in the current batch) than the slot's
+// resident replaces it (the resident's 32 accumulators are folded with shuffles and written back).
+// The directory is consulted only once it holds an entry: uniform keys never pay for it.
+// CTA g writes its result to part[g][.]; a second kernel folds the G tables per bin in a fixed order.
 
-constexpr int CS_SLOTS = 1024, CS_WARPS = 8, CS_NT = CS_WARPS * 32, CS_CTAS_PER_SM = 5;   // w <= 1024
+constexpr uint32_t CLAIM = 0xFFF00000u;     // claim words are >= CLAIM as unsigned integers
+constexpr uint32_t BIN_NONE = 0xffffffffu;  // no pending element
+constexpr uint32_t DIR_EMPTY = 0xfffffffeu;
+constexpr int DIR_S = 16;                   // directory slots per warp (2 KB of accumulators)
+
+constexpr int CS_SLOTS = 1024, CS_WARPS = 8, CS_NT = CS_WARPS * 32, CS_CTAS_PER_SM = 4;   // w <= 1024
 constexpr int CB_SLOTS = 64, CB_WARPS = 32, CB_NT = CB_WARPS * 32;                        // w  > 1024
-constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 + 64 KB of claim words, 18 KB of warp caches (128-slot caches: no gain)
+constexpr int CB_PART = 32768;  // bins per CTA: 128 KB of f32 cells
 constexpr int CB_MAX_SPLIT_LOG2 = 5;  // a group of up to 32 CTAs shares one histogram (w <= 2^20)
-constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
-constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
 constexpr uint32_t CB_EMPTY = 0xffffffffu;  // tag word = (bin / CB_SLOTS) << 2 | hit counter
 
 template <int ACC>
@@ -509,32 +579,227 @@ struct CachedOp<ACC_SATADD> {
 };
 
 template <int ACC>
-VJP_DEVINL void smem_combine(float *cell, float v, float S) {
-    unsigned *a = reinterpret_cast<unsigned *>(cell);
-    unsigned old = *(volatile unsigned *)a, assumed;
+VJP_DEVINL void smem_combine(uint32_t *cell, float v, float S) {
+    unsigned old = *(volatile unsigned *)cell, assumed;
     do {
         assumed = old;
-        old = atomicCAS(a, assumed, __float_as_uint(CachedOp<ACC>::comb(__uint_as_float(assumed), v, S)));
+        old = atomicCAS(cell, assumed, __float_as_uint(CachedOp<ACC>::comb(__uint_as_float(assumed), v, S)));
     } while (old != assumed);
 }
 
-// w <= CS_SLOTS.  32 elements, one per lane; lanes with act hold (bin b, value x).
+// fold of one value per lane over the warp (the operators are commutative)
 template <int ACC>
-VJP_DEVINL void claim_update_small(bool act, uint32_t b, float x, float *vl, uint8_t *cl, float S,
-                                   int lane) {
-    bool pend = act;
-    while (__any_sync(FULL_MASK, pend)) {
-        if (pend) cl[b] = (uint8_t)lane;
-        __syncwarp();
-        if (pend && cl[b] == lane) {
-            vl[b] = CachedOp<ACC>::comb(vl[b], x, S);
-            pend = false;
+VJP_DEVINL float warp_fold(float x, float S) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1)
+        x = CachedOp<ACC>::comb(x, __shfl_xor_sync(FULL_MASK, x, off), S);
+    return x;
+}
+
+// Directory of one warp: dir[DIR_S] resident bins, seen[DIR_S] last contended candidate per slot,
+// hot[DIR_S][32] lane-private accumulators.
+struct WarpDir {
+    uint32_t *dir, *seen;
+    float *hot;
+};
+
+// Lookup of NI elements; a hit is folded into the lane's accumulator and removed from b[].
+// hitm: bit s set if this lane hit slot s.
+template <int ACC, int NI>
+VJP_DEVINL void dir_lookup(const WarpDir &d, uint32_t (&b)[NI], const float (&v)[NI], int lane, float S,
+                           uint32_t &hitm) {
+#pragma unroll
+    for (int j = 0; j < NI; j++) {
+        const uint32_t s = b[j] & (DIR_S - 1);
+        if (d.dir[s] == b[j]) {  // BIN_NONE never matches: entries are bins or DIR_EMPTY
+            float *h = d.hot + s * 32 + lane;
+            *h = CachedOp<ACC>::comb(*h, v[j], S);
+            hitm |= 1u << s;
+            b[j] = BIN_NONE;
         }
-        __syncwarp();
     }
 }
 
-// w > CS_SLOTS.  Returns true if (eb, evv) must go to the CTA table.
+// Called by the whole warp with a contended candidate bin `cand` (warp-uniform) that `c` lanes hold
+// in elements still pending.  Installs it if it was the slot's candidate before and the slot's resident
+// is colder in this batch; then the pending elements of cand are absorbed.  Returns true on install.
+// flush(bin, value): adds the evicted resident's fold to the table (called by lane 0 only).
+template <int ACC, int NI, class Flush>
+VJP_DEVINL bool dir_train(const WarpDir &d, uint32_t cand, int c, uint32_t hitm, uint32_t (&b)[NI],
+                          const float (&v)[NI], int lane, float S, int &ndir, Flush flush) {
+    const uint32_t s = cand & (DIR_S - 1);
+    const uint32_t prev = d.seen[s];
+    __syncwarp();
+    if (prev != cand) {
+        if (lane == 0) d.seen[s] = cand;
+        __syncwarp();
+        return false;
+    }
+    const int h = __popc(__ballot_sync(FULL_MASK, (hitm >> s) & 1u));
+    if (c <= h) return false;
+    const uint32_t old = d.dir[s];
+    float *hp = d.hot + s * 32 + lane;
+    if (old != DIR_EMPTY) {
+        const float x = warp_fold<ACC>(*hp, S);
+        if (lane == 0) flush(old, x);
+    } else {
+        ndir++;
+    }
+    float acc = CachedOp<ACC>::neutral();
+#pragma unroll
+    for (int j = 0; j < NI; j++)
+        if (b[j] == cand) {
+            acc = CachedOp<ACC>::comb(acc, v[j], S);
+            b[j] = BIN_NONE;
+        }
+    *hp = acc;
+    __syncwarp();
+    if (lane == 0) d.dir[s] = cand;
+    __syncwarp();
+    return true;
+}
+
+// COUNT_ZEROS: the lifted '*' of the VJP (P:L460): zeros are counted (integer atomics, exact) and
+// kept out of the product.  Otherwise: the plain primal histogram of the operator.
+//
+// w <= CS_SLOTS: every warp owns a private table (a slot IS a bin) and runs the claim round over the
+// 128 elements of its batch (one quad per lane) with __syncwarp as the barrier.
+constexpr size_t CS_SMEM = (size_t)CS_WARPS * (CS_SLOTS * 4 + DIR_S * 32 * 4 + 2 * DIR_S * 4);
+
+template <int ACC, bool COUNT_ZEROS>
+__global__ void __launch_bounds__(CS_NT, CS_CTAS_PER_SM)
+rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
+                        const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
+                        float S) {
+    using OP = CachedOp<ACC>;
+    extern __shared__ uint4 smem_raw[];
+    uint32_t *tabs = reinterpret_cast<uint32_t *>(smem_raw);                  // [CS_WARPS][CS_SLOTS]
+    float *hots = reinterpret_cast<float *>(tabs + CS_WARPS * CS_SLOTS);      // [CS_WARPS][DIR_S][32]
+    uint32_t *dirs = reinterpret_cast<uint32_t *>(hots + CS_WARPS * DIR_S * 32);  // [CS_WARPS][2][DIR_S]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *tab = tabs + warp * CS_SLOTS;
+    WarpDir d;
+    d.hot = hots + warp * DIR_S * 32;
+    d.dir = dirs + warp * 2 * DIR_S;
+    d.seen = d.dir + DIR_S;
+    for (int s = lane; s < CS_SLOTS; s += 32) tab[s] = __float_as_uint(OP::neutral());
+    for (int s = lane; s < DIR_S * 32; s += 32) d.hot[s] = OP::neutral();
+    if (lane < 2 * DIR_S) d.dir[lane] = DIR_EMPTY;
+    __syncwarp();
+    int ndir = 0;  // warp-uniform: resident directory entries
+    const uint32_t myid = CLAIM | (uint32_t)(lane * 4);
+    auto flush = [&](uint32_t bin, float x) { tab[bin] = __float_as_uint(OP::comb(__uint_as_float(tab[bin]), x, S)); };
+
+    const int64_t nquads = (n + 3) / 4;
+    const int64_t stride = (int64_t)gridDim.x * CS_NT;
+    int64_t qw = blockIdx.x * (int64_t)CS_NT + warp * 32;  // warp-uniform: the warp never diverges here
+    int64_t k[4] = {-1, -1, -1, -1};
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    if (qw < nquads && qw + lane < nquads) {
+        const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
+        load_vals4(vs, (qw + lane) * 4, cnt, v);
+    }
+    while (qw < nquads) {
+        int64_t kn[4] = {-1, -1, -1, -1};
+        float vn[4] = {0.f, 0.f, 0.f, 0.f};
+        const int64_t qn = qw + stride;
+        if (qn + lane < nquads) {  // next iteration's loads fly while this one is processed
+            const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
+            load_vals4(vs, (qn + lane) * 4, cnt, vn);
+        }
+        uint32_t b[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            bool act = in_range(k[j], w);
+            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
+                atomicAdd(zeros + k[j], 1u);
+                act = false;
+            }
+            b[j] = act ? (uint32_t)k[j] : BIN_NONE;
+        }
+        uint32_t hitm = 0;
+        if (ndir) dir_lookup<ACC, 4>(d, b, v, lane, S, hitm);
+        // claim round over the warp's 128 elements
+        uint32_t o[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) o[j] = tab[b[j] & (CS_SLOTS - 1)];
+#pragma unroll
+        for (int j = 0; j < 4; j++)
+            if (b[j] != BIN_NONE && o[j] < CLAIM) tab[b[j]] = myid + j;
+        __syncwarp();
+        uint32_t c[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) c[j] = tab[b[j] & (CS_SLOTS - 1)];
+        bool lost = false;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            if (b[j] == BIN_NONE) continue;
+            if (c[j] == myid + j) {
+                tab[b[j]] = __float_as_uint(OP::comb(__uint_as_float(o[j]), v[j], S));
+                b[j] = BIN_NONE;
+            } else {
+                lost = true;
+            }
+        }
+        __syncwarp();
+        const unsigned lm = __ballot_sync(FULL_MASK, lost);
+        if (lm) {
+            // directory training: the first loser of the lowest lane is this batch's candidate
+            const uint32_t mine = b[0] != BIN_NONE ? b[0] : b[1] != BIN_NONE ? b[1] : b[2] != BIN_NONE ? b[2] : b[3];
+            const uint32_t cand = __shfl_sync(FULL_MASK, mine, __ffs(lm) - 1);
+            const bool has = (b[0] == cand) | (b[1] == cand) | (b[2] == cand) | (b[3] == cand);
+            const int cl = __popc(__ballot_sync(FULL_MASK, has));
+            dir_train<ACC, 4>(d, cand, cl, hitm, b, v, lane, S, ndir, flush);
+            // the remaining losers: claim rounds over one element per lane (a shared-memory atomicCAS
+            // instead costs the LSU ~64 cycles per warp instruction whatever the number of lanes: three of
+            // them per batch made this kernel no faster than the one it replaced)
+            uint32_t pm = (uint32_t)(b[0] != BIN_NONE) | (uint32_t)(b[1] != BIN_NONE) << 1 |
+                          (uint32_t)(b[2] != BIN_NONE) << 2 | (uint32_t)(b[3] != BIN_NONE) << 3;
+            while (__any_sync(FULL_MASK, pm != 0)) {
+                uint32_t pb = BIN_NONE;
+                float pv = 0.f;
+                if (pm & 1u) { pb = b[0]; pv = v[0]; }
+                else if (pm & 2u) { pb = b[1]; pv = v[1]; }
+                else if (pm & 4u) { pb = b[2]; pv = v[2]; }
+                else if (pm & 8u) { pb = b[3]; pv = v[3]; }
+                const uint32_t o1 = tab[pb & (CS_SLOTS - 1)];
+                if (pb != BIN_NONE && o1 < CLAIM) tab[pb] = myid;
+                __syncwarp();
+                const uint32_t c1 = tab[pb & (CS_SLOTS - 1)];
+                if (pb != BIN_NONE && c1 == myid) {
+                    tab[pb] = __float_as_uint(OP::comb(__uint_as_float(o1), pv, S));
+                    pm &= pm - 1;
+                }
+                __syncwarp();
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            k[j] = kn[j];
+            v[j] = vn[j];
+        }
+        qw = qn;
+    }
+    for (int s = 0; s < DIR_S; s++) {  // write the directory back
+        const uint32_t bin = d.dir[s];
+        if (bin == DIR_EMPTY) continue;
+        const float x = warp_fold<ACC>(d.hot[s * 32 + lane], S);
+        if (lane == 0) flush(bin, x);
+    }
+    __syncthreads();
+    for (int s = threadIdx.x; s < (int)w; s += CS_NT) {
+        float acc = __uint_as_float(tabs[s]);
+#pragma unroll
+        for (int wp = 1; wp < CS_WARPS; wp++) acc = OP::comb(acc, __uint_as_float(tabs[wp * CS_SLOTS + s]), S);
+        part[(size_t)blockIdx.x * (size_t)w + s] = acc;
+    }
+}
+
+// w > CS_SLOTS, warp cache: returns true if (eb, evv) must go to the CTA table.  The lanes of a warp
+// arbitrate per slot through a claim byte (every pending lane stores its lane id, the warp syncs, the
+// lane that reads its own id back owns the slot for this round); a 2-bit hit counter guards the
+// resident entry -- a cold bin arriving at a hot slot decrements it and BYPASSES; only an entry whose
+// counter has run out is evicted (Misra-Gries style).
 template <int ACC>
 VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint32_t *tg, uint8_t *cl,
                                  float S, int lane, uint32_t &eb, float &evv) {
@@ -569,268 +834,182 @@ VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint3
     return ev;
 }
 
-// COUNT_ZEROS: the lifted '*' of the VJP (P:L460): zeros are counted (integer atomics, exact) and
-// kept out of the product.  Otherwise: the plain primal histogram of the operator.
-template <int ACC, bool COUNT_ZEROS>
-__global__ void __launch_bounds__(CS_NT, CS_CTAS_PER_SM)
-rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
-                        const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
-                        float S) {
-    using OP = CachedOp<ACC>;
-    extern __shared__ uint4 smem_raw[];
-    float *vals = reinterpret_cast<float *>(smem_raw);                       // [CS_WARPS][CS_SLOTS]
-    uint8_t *claim = reinterpret_cast<uint8_t *>(vals + CS_WARPS * CS_SLOTS);  // [CS_WARPS][CS_SLOTS]
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    float *vl = vals + warp * CS_SLOTS;
-    uint8_t *cl = claim + warp * CS_SLOTS;
-    for (int s = lane; s < CS_SLOTS; s += 32) vl[s] = OP::neutral();
-    __syncwarp();
-    const int64_t nquads = (n + 3) / 4;
-    const int64_t stride = (int64_t)gridDim.x * CS_NT;
-    int64_t qw = blockIdx.x * (int64_t)CS_NT + warp * 32;  // warp-uniform: the warp never diverges here
-    int64_t k[4] = {-1, -1, -1, -1};
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    uint32_t rb = CB_EMPTY, rcnt = 0;
-    float racc = OP::neutral();
-    if (qw < nquads) {
-        const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
-        load_vals4(vs, (qw + lane) * 4, cnt, v);
-    }
-    while (qw < nquads) {
-        int64_t kn[4] = {-1, -1, -1, -1};
-        float vn[4] = {0.f, 0.f, 0.f, 0.f};
-        const int64_t qn = qw + stride;
-        if (qn < nquads) {  // next iteration's loads fly while this one is processed
-            const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
-            load_vals4(vs, (qn + lane) * 4, cnt, vn);
-        }
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            bool act = in_range(k[j], w);
-            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
-                atomicAdd(zeros + k[j], 1u);
-                act = false;
-            }
-            uint32_t b = (uint32_t)k[j];
-            float x = v[j];
-            if (act) {  // register entry: see rbi_cached_big_kernel
-                if (b == rb) {
-                    racc = OP::comb(racc, x, S);
-                    rcnt = min(rcnt + CB_RW, CB_RMAX);
-                    act = false;
-                } else if (rcnt == 0) {
-                    act = rb != CB_EMPTY;
-                    const uint32_t ob = rb;
-                    const float ov = racc;
-                    rb = b;
-                    racc = x;
-                    b = ob;
-                    x = ov;
-                } else {
-                    rcnt--;
-                }
-            }
-            claim_update_small<ACC>(act, b, x, vl, cl, S, lane);
-        }
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            k[j] = kn[j];
-            v[j] = vn[j];
-        }
-        qw = qn;
-    }
-    claim_update_small<ACC>(rb != CB_EMPTY, rb, racc, vl, cl, S, lane);
-    __syncthreads();
-    for (int s = threadIdx.x; s < (int)w; s += CS_NT) {
-        float acc = vals[s];
-#pragma unroll
-        for (int wp = 1; wp < CS_WARPS; wp++) acc = OP::comb(acc, vals[wp * CS_SLOTS + s], S);
-        part[(size_t)blockIdx.x * (size_t)w + s] = acc;
-    }
-}
-
 // w > CS_SLOTS.  A CTA of 1024 threads owns a table of up to CB_PART bins in shared memory.  A
 // histogram wider than that is SPLIT over the 2^c CTAs of a group by the low c bits of the bin
 // (hot neighbouring bins land on different CTAs); all CTAs of a group stream the same part of the
 // input at the same time (one of them pulls it from HBM, the others hit in L2) and each keeps the
 // elements of its own bins: one pass over the input for any w, no traffic between the CTAs.
 //
-// Per batch (U quads per thread) the table is updated WITHOUT atomics:
-//   0. an element whose bin is resident in the warp's cache is "hot" and goes to step 2 directly;
-//   1. one CTA-wide claim round: every pending element stores its id into the bin's claim word,
-//      barrier, the element that reads its id back owns the bin for this round and does a plain
-//      read-modify-write of the table cell.  Uniform keys at w = 2^16: ~6 % of the elements lose.
-//      A loser gets ONE compare-and-swap on the cell (uniform keys: it succeeds);
-//   2. hot elements: claim rounds inside the warp on the resident cache entry (plain LDS/STS); an
-//      element that lost the round AND its compare-and-swap sits in a CONTENDED bin: the warp's
-//      cache installs it unless a hotter bin guards the slot (claim_update_big above).  Hot bins
-//      therefore migrate into the caches and stop taking part in step 1; evictions and bypasses
-//      (cold, rare) fall back to a CAS loop on the table.
-// Barriers: [claim] B1 [plain updates] B2 [CAS, caches].  Two elements never own one bin in a round
-// because all claims precede B1; the plain updates (between B1 and B2) never overlap a CAS (after
-// B2, before the next batch's B1).
-template <int ACC, bool COUNT_ZEROS, int U>
+// Per batch of 4096 elements (one quad per thread), three barriers:
+//   [directory / warp-cache lookups (skew mode only); claims (A)]  B1  [owners update (B)]  B2
+//   [losers: one compare-and-swap; elements of bins resident in the warp cache: claim-byte rounds on
+//    the entry; a failed compare-and-swap = contended bin -> the warp cache installs it unless a hotter
+//    bin guards the slot; directory training]  B3
+// B3 keeps the compare-and-swaps of C away from the value reads of the next A.  SKEW MODE is switched
+// per batch by the fraction of threads that saw a loser, a cache hit or a directory hit (counted by
+// B2 itself): with uniform keys (3 % losers at w = 2^16) the lookups are skipped altogether; with
+// skewed keys the top bins live in the lane-private directories, the middle ones in the warp caches
+// (fed by failed compare-and-swaps) and only the cold tail takes part in the claim round.
+constexpr size_t CB_SMEM = (size_t)CB_PART * 4 + (size_t)CB_WARPS * (DIR_S * 32 * 4 + 2 * DIR_S * 4) +
+                           (size_t)CB_WARPS * CB_SLOTS * 9;
+constexpr int CB_SKEW_ON = 400, CB_SKEW_OFF = 250;  // threads (of 1024) with a loser / hit in a batch
+
+template <int ACC, bool COUNT_ZEROS>
 __global__ void __launch_bounds__(CB_NT, 1)
 rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restrict__ is,
                       const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
                       float S) {
     using OP = CachedOp<ACC>;
     extern __shared__ uint4 smem_raw[];
-    float *table = reinterpret_cast<float *>(smem_raw);                          // [CB_PART]
-    float *vals = table + CB_PART;                                               // [CB_WARPS][CB_SLOTS]
+    uint32_t *table = reinterpret_cast<uint32_t *>(smem_raw);                     // [CB_PART]
+    float *hots = reinterpret_cast<float *>(table + CB_PART);                     // [CB_WARPS][DIR_S][32]
+    uint32_t *dirs = reinterpret_cast<uint32_t *>(hots + CB_WARPS * DIR_S * 32);  // [CB_WARPS][2][DIR_S]
+    float *vals = reinterpret_cast<float *>(dirs + CB_WARPS * 2 * DIR_S);         // [CB_WARPS][CB_SLOTS]
     uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);    // [CB_WARPS][CB_SLOTS]
-    uint16_t *claimA = reinterpret_cast<uint16_t *>(tags + CB_WARPS * CB_SLOTS);  // [CB_PART]
-    uint8_t *claim = reinterpret_cast<uint8_t *>(claimA + CB_PART);               // [CB_WARPS][CB_SLOTS]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(tags + CB_WARPS * CB_SLOTS);     // [CB_WARPS][CB_SLOTS]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float *vl = vals + warp * CB_SLOTS;
     uint32_t *tg = tags + warp * CB_SLOTS;
     uint8_t *cl = claim + warp * CB_SLOTS;
+    WarpDir d;
+    d.hot = hots + warp * DIR_S * 32;
+    d.dir = dirs + warp * 2 * DIR_S;
+    d.seen = d.dir + DIR_S;
     const uint32_t clmask = (1u << cl_log2) - 1u;
     const uint32_t rank = blockIdx.x & clmask;
     const int64_t group = blockIdx.x >> cl_log2, groups = gridDim.x >> cl_log2;
-    for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = OP::neutral();
+    for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = __float_as_uint(OP::neutral());
+    for (int s = lane; s < DIR_S * 32; s += 32) d.hot[s] = OP::neutral();
+    if (lane < 2 * DIR_S) d.dir[lane] = DIR_EMPTY;
     for (int s = lane; s < CB_SLOTS; s += 32) {
         vl[s] = OP::neutral();
         tg[s] = CB_EMPTY;
     }
     __syncthreads();
-    constexpr int NI = 4 * U;
+    int ndir = 0;       // warp-uniform
+    bool skew = false;  // CTA-uniform
+    // Losers of a claim round are not resolved with atomics (a shared-memory atomicCAS costs the LSU ~64
+    // cycles per warp instruction): a thread CARRIES up to two of them into the next batch's claim round.
+    uint32_t cb0 = BIN_NONE, cb1 = BIN_NONE;
+    float cv0 = 0.f, cv1 = 0.f;
+    const uint32_t myid = CLAIM | (uint32_t)(threadIdx.x * 8);  // + slot: 0-3 new elements, 4-5 carries
+    auto flush = [&](uint32_t bin, float x) { smem_combine<ACC>(table + bin, x, S); };
+
     const int64_t nquads = (n + 3) / 4;
-    const int64_t stride = groups * (int64_t)(CB_NT * U);
-    int64_t q0 = group * (int64_t)(CB_NT * U);  // CTA-uniform: no thread leaves the barriers early
-    int64_t k[NI];
-    float v[NI];
-    auto load_batch = [&](int64_t q, int64_t (&kk)[NI], float (&vv)[NI]) {
-#pragma unroll
-        for (int u = 0; u < U; u++) {
-            int64_t k4[4] = {-1, -1, -1, -1};
-            float v4[4] = {0.f, 0.f, 0.f, 0.f};
-            const int64_t qq = q + u * CB_NT + threadIdx.x;
-            if (qq < nquads) {
-                const int cnt = load_keys4(is, qq * 4, n, k4);
-                load_vals4(vs, qq * 4, cnt, v4);
-            }
-#pragma unroll
-            for (int j = 0; j < 4; j++) {
-                kk[u * 4 + j] = k4[j];
-                vv[u * 4 + j] = v4[j];
-            }
-        }
-    };
-    // A claim word names the ELEMENT (thread id * NI + j): exactly one element per bin wins a round,
-    // so all claim words and table cells of a round can be read before any of them is written.
-    const uint32_t id0 = threadIdx.x * NI;
-    // Thread-private register entry (rb, racc, rcnt) in front of everything: a bin that holds a
-    // large share of the elements (one bin = 14 % at Zipf keys) is folded into a register with no
-    // shared-memory access at all.  Weighted majority vote: +CB_RW on a hit, -1 on a miss, replaced
-    // at 0 -- the displaced pair takes the element's place on the normal path.
-    uint32_t rb = CB_EMPTY, rcnt = 0;
-    float racc = OP::neutral();
-    load_batch(q0, k, v);
-    for (;;) {
-        // after the last batch of the input: one more round of the same machinery for the register
-        // entries (1024 CAS on one hot cell would serialise); q0 is CTA-uniform
-        const bool drain = q0 >= nquads;
-        int64_t kn[NI];
-        float vn[NI];
+    const int64_t stride = groups * (int64_t)CB_NT;
+    int64_t q0 = group * (int64_t)CB_NT;  // CTA-uniform: no thread leaves the barriers early
+    int64_t k[4] = {-1, -1, -1, -1};
+    float v[4] = {0.f, 0.f, 0.f, 0.f};
+    if (q0 + threadIdx.x < nquads) {
+        const int cnt = load_keys4(is, (q0 + threadIdx.x) * 4, n, k);
+        load_vals4(vs, (q0 + threadIdx.x) * 4, cnt, v);
+    }
+    while (q0 < nquads) {
+        int64_t kn[4] = {-1, -1, -1, -1};
+        float vn[4] = {0.f, 0.f, 0.f, 0.f};
         const int64_t qn = q0 + stride;
-        load_batch(qn, kn, vn);  // next batch's loads fly while this one is processed (none past the end)
-        uint32_t b[NI];  // table index of a pending element, CB_EMPTY = nothing pending
-        uint32_t zm = 0;
+        if (qn + threadIdx.x < nquads) {  // next batch's loads fly while this one is processed
+            const int cnt = load_keys4(is, (qn + threadIdx.x) * 4, n, kn);
+            load_vals4(vs, (qn + threadIdx.x) * 4, cnt, vn);
+        }
+        uint32_t b[4];  // table index of a pending element
 #pragma unroll
-        for (int j = 0; j < NI; j++) {
+        for (int j = 0; j < 4; j++) {
             const uint32_t klo = (uint32_t)k[j];
             bool act = in_range(k[j], w) & ((klo & clmask) == rank);
-            if (COUNT_ZEROS) {
-                const bool z = act & (v[j] == 0.f);  // IEEE equality: +-0 only (Q7)
-                zm |= (uint32_t)z << j;
-                act &= !z;
+            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
+                atomicAdd(zeros + k[j], 1u);
+                act = false;
             }
-            b[j] = act ? klo >> cl_log2 : CB_EMPTY;
+            b[j] = act ? klo >> cl_log2 : BIN_NONE;
         }
-        if (COUNT_ZEROS && zm) {
+        uint32_t hitm = 0, hotm = 0;  // hotm bit j: resident in the warp cache
+        bool busy = false;            // this thread saw a directory hit, a cache hit or a loser
+        if (skew) {
+            if (ndir) dir_lookup<ACC, 4>(d, b, v, lane, S, hitm);
 #pragma unroll
-            for (int j = 0; j < NI; j++)
-                if (zm >> j & 1u) atomicAdd(zeros + k[j], 1u);
-        }
-        if (drain) {
-            b[0] = rb;
-            v[0] = racc;
-            rcnt = 1;  // keeps the loop below from re-installing it
-            rb = CB_EMPTY;
-        }
-#pragma unroll
-        for (int j = 0; j < NI; j++) {  // register entry
-            if (b[j] == CB_EMPTY) continue;
-            if (b[j] == rb) {
-                racc = OP::comb(racc, v[j], S);
-                rcnt = min(rcnt + CB_RW, CB_RMAX);
-                b[j] = CB_EMPTY;
-            } else if (rcnt == 0) {
-                const uint32_t ob = rb;
-                const float ov = racc;
-                rb = b[j];
-                racc = v[j];
-                b[j] = ob;  // CB_EMPTY the first time
-                v[j] = ov;
-            } else {
-                rcnt--;
+            for (int j = 0; j < 4; j++) {
+                const uint32_t t = tg[b[j] & (CB_SLOTS - 1)];
+                // a valid tag never equals CB_EMPTY's, and BIN_NONE matches no tag
+                const bool hot = (t >> 2) == b[j] / CB_SLOTS;
+                hotm |= (uint32_t)hot << j;
+                if (hot & ((t & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t + 1;  // racing lanes store the same word
             }
+            busy = (hitm | hotm) != 0;
         }
-        uint32_t t[NI];
+        // A: claims of the cold pending elements and of the carried ones
+        const bool any1 = __any_sync(FULL_MASK, cb1 != BIN_NONE);
+        uint32_t o[4], oc0, oc1 = 0;
 #pragma unroll
-        for (int j = 0; j < NI; j++) t[j] = tg[b[j] & (CB_SLOTS - 1)];
-        uint32_t coldm = 0;  // bit j: pending and not resident in the warp's cache
-        uint32_t hotm = 0;   // bit j: pending and resident
+        for (int j = 0; j < 4; j++) o[j] = table[b[j] & (CB_PART - 1)];
+        oc0 = table[cb0 & (CB_PART - 1)];
+        if (any1) oc1 = table[cb1 & (CB_PART - 1)];
 #pragma unroll
-        for (int j = 0; j < NI; j++) {
-            // a valid tag never equals CB_EMPTY's, and b == CB_EMPTY matches no tag
-            const bool hot = (t[j] >> 2) == b[j] / CB_SLOTS;
-            const bool cold = !hot & (b[j] != CB_EMPTY);
-            hotm |= (uint32_t)hot << j;
-            coldm |= (uint32_t)cold << j;
-            if (hot & ((t[j] & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t[j] + 1;  // racing lanes store the same word
-            if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
-        }
+        for (int j = 0; j < 4; j++)
+            if (b[j] != BIN_NONE && !(hotm >> j & 1u) && o[j] < CLAIM) table[b[j]] = myid + j;
+        if (cb0 != BIN_NONE && oc0 < CLAIM) table[cb0] = myid + 4;
+        if (any1 && cb1 != BIN_NONE && oc1 < CLAIM) table[cb1] = myid + 5;
         __syncthreads();  // B1
-        {
-            uint16_t c[NI];
-            float o[NI];
+        uint32_t c[4], cc0, cc1 = 0;
 #pragma unroll
-            for (int j = 0; j < NI; j++) {
-                c[j] = claimA[b[j] & (CB_PART - 1)];
-                o[j] = table[b[j] & (CB_PART - 1)];
-            }
+        for (int j = 0; j < 4; j++) c[j] = table[b[j] & (CB_PART - 1)];
+        cc0 = table[cb0 & (CB_PART - 1)];
+        if (any1) cc1 = table[cb1 & (CB_PART - 1)];
+        uint32_t coldm = 0;  // bit j: lost the claim round
 #pragma unroll
-            for (int j = 0; j < NI; j++) {
-                const bool cold = coldm >> j & 1u;
-                const bool win = cold & (c[j] == (uint16_t)(id0 + j));
-                if (win) table[b[j]] = OP::comb(o[j], v[j], S);
-                coldm &= ~((uint32_t)win << j);
-            }
-        }
-        __syncthreads();  // B2: the plain updates are done before any CAS touches the table
-        if (__any_sync(FULL_MASK, coldm != 0)) {
-#pragma unroll
-            for (int j = 0; j < NI; j++) {  // losers: ONE compare-and-swap; a failure means the bin is contended
-                if (coldm >> j & 1u) {
-                    unsigned *cell = reinterpret_cast<unsigned *>(table + b[j]);
-                    const unsigned old = *(volatile unsigned *)cell;
-                    const unsigned upd = __float_as_uint(OP::comb(__uint_as_float(old), v[j], S));
-                    if (atomicCAS(cell, old, upd) == old) coldm &= ~(1u << j);
-                }
+        for (int j = 0; j < 4; j++) {
+            if (b[j] == BIN_NONE || (hotm >> j & 1u)) continue;
+            if (c[j] == myid + j) {
+                table[b[j]] = __float_as_uint(OP::comb(__uint_as_float(o[j]), v[j], S));
+                b[j] = BIN_NONE;
+            } else {
+                coldm |= 1u << j;
             }
         }
+        bool again0 = false, again1 = false;  // a carried element lost once more: its bin is contended
+        if (cb0 != BIN_NONE) {
+            if (cc0 == myid + 4) {
+                table[cb0] = __float_as_uint(OP::comb(__uint_as_float(oc0), cv0, S));
+                cb0 = BIN_NONE;
+            } else {
+                again0 = true;
+            }
+        }
+        if (any1 && cb1 != BIN_NONE) {
+            if (cc1 == myid + 5) {
+                table[cb1] = __float_as_uint(OP::comb(__uint_as_float(oc1), cv1, S));
+                cb1 = BIN_NONE;
+            } else {
+                again1 = true;
+            }
+        }
+        const int nbusy = __syncthreads_count(busy | (coldm != 0));  // B2
+        // C
         if (__any_sync(FULL_MASK, hotm != 0)) {
 #pragma unroll
-            for (int j = 0; j < NI; j++) {  // hits: the resident entry cannot change before the installs below
-                uint8_t *c = cl + (b[j] & (CB_SLOTS - 1));
+            for (int j = 0; j < 4; j++) {
+                const unsigned hm = __ballot_sync(FULL_MASK, hotm >> j & 1u);
+                if (hm == 0) continue;
+                // directory training: a bin that several lanes of this row hold in the warp cache
+                const uint32_t cand = __shfl_sync(FULL_MASK, b[j], __ffs(hm) - 1);
+                const int cn = __popc(__ballot_sync(FULL_MASK, (hotm >> j & 1u) && b[j] == cand));
+                if (cn >= 2) {
+                    uint32_t bb[1] = {(hotm >> j & 1u) ? b[j] : BIN_NONE};
+                    const float vv[1] = {v[j]};
+                    if (dir_train<ACC, 1>(d, cand, cn, hitm, bb, vv, lane, S, ndir, flush) && bb[0] == BIN_NONE &&
+                        (hotm >> j & 1u)) {
+                        hotm &= ~(1u << j);
+                        b[j] = BIN_NONE;
+                    }
+                }
+                // hits: the resident entry cannot change before the installs below
+                uint8_t *cbyte = cl + (b[j] & (CB_SLOTS - 1));
                 float *a = vl + (b[j] & (CB_SLOTS - 1));
                 bool pend = hotm >> j & 1u;
                 while (__any_sync(FULL_MASK, pend)) {
-                    if (pend) *c = (uint8_t)lane;
+                    if (pend) *cbyte = (uint8_t)lane;
                     __syncwarp();
-                    if (pend && *c == lane) {
+                    if (pend && *cbyte == lane) {
                         *a = OP::comb(*a, v[j], S);
                         pend = false;
                     }
@@ -838,27 +1017,64 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 }
             }
         }
+        // carried elements that lost again sit in contended bins: in skew mode the warp cache takes them
+        // (installing the bin unless a hotter one guards the slot); evictions and bypasses (cold, rare)
+        // fall back to a compare-and-swap loop on the table
+        if (skew) {
+            if (__any_sync(FULL_MASK, again0)) {
+                uint32_t eb = 0;
+                float evv = 0.f;
+                if (claim_update_big<ACC>(again0, cb0, cv0, vl, tg, cl, S, lane, eb, evv)) smem_combine<ACC>(table + eb, evv, S);
+                if (again0) cb0 = BIN_NONE;
+            }
+            if (__any_sync(FULL_MASK, again1)) {
+                uint32_t eb = 0;
+                float evv = 0.f;
+                if (claim_update_big<ACC>(again1, cb1, cv1, vl, tg, cl, S, lane, eb, evv)) smem_combine<ACC>(table + eb, evv, S);
+                if (again1) cb1 = BIN_NONE;
+            }
+        }
+        // new losers: into a free carry slot; a thread that has none left (rare) updates the table directly
         if (__any_sync(FULL_MASK, coldm != 0)) {
 #pragma unroll
-            for (int j = 0; j < NI; j++) {
-                const bool act = coldm >> j & 1u;
-                if (__any_sync(FULL_MASK, act)) {
-                    uint32_t eb = 0;
-                    float evv = 0.f;
-                    if (claim_update_big<ACC>(act, b[j], v[j], vl, tg, cl, S, lane, eb, evv))
-                        smem_combine<ACC>(table + eb, evv, S);
+            for (int j = 0; j < 4; j++) {
+                if (!(coldm >> j & 1u)) continue;
+                if (cb0 == BIN_NONE) { cb0 = b[j]; cv0 = v[j]; coldm &= ~(1u << j); }
+                else if (cb1 == BIN_NONE) { cb1 = b[j]; cv1 = v[j]; coldm &= ~(1u << j); }
+            }
+            if (__any_sync(FULL_MASK, coldm != 0)) {
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    const bool act = coldm >> j & 1u;
+                    if (!__any_sync(FULL_MASK, act)) continue;
+                    if (skew) {
+                        uint32_t eb = 0;
+                        float evv = 0.f;
+                        if (claim_update_big<ACC>(act, b[j], v[j], vl, tg, cl, S, lane, eb, evv))
+                            smem_combine<ACC>(table + eb, evv, S);
+                    } else if (act) {
+                        smem_combine<ACC>(table + b[j], v[j], S);
+                    }
                 }
             }
         }
-        if (drain) break;
+        skew = skew ? nbusy >= CB_SKEW_OFF : nbusy > CB_SKEW_ON;
+        __syncthreads();  // B3
 #pragma unroll
-        for (int j = 0; j < NI; j++) {
+        for (int j = 0; j < 4; j++) {
             k[j] = kn[j];
             v[j] = vn[j];
         }
         q0 = qn;
     }
-    __syncthreads();
+    if (cb0 != BIN_NONE) smem_combine<ACC>(table + cb0, cv0, S);  // the last carries
+    if (cb1 != BIN_NONE) smem_combine<ACC>(table + cb1, cv1, S);
+    for (int s = 0; s < DIR_S; s++) {  // write the directory back
+        const uint32_t bin = d.dir[s];
+        if (bin == DIR_EMPTY) continue;
+        const float x = warp_fold<ACC>(d.hot[s * 32 + lane], S);
+        if (lane == 0) flush(bin, x);
+    }
     for (int s = lane; s < CB_SLOTS; s += 32) {  // write the warp's cache back
         const uint32_t t = tg[s];
         if (t != CB_EMPTY) smem_combine<ACC>(table + (t >> 2) * CB_SLOTS + s, vl[s], S);
@@ -867,7 +1083,7 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     float *dst = part + (size_t)group * (size_t)w;
     for (int64_t i = threadIdx.x; i < CB_PART; i += CB_NT) {
         const int64_t bin = (i << cl_log2) + rank;
-        if (bin < w) dst[bin] = table[i];
+        if (bin < w) dst[bin] = __uint_as_float(table[i]);
     }
 }
 
@@ -905,9 +1121,6 @@ rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part, float *
     if (threadIdx.x < 32 && k < w) out[k] = p;
 }
 
-constexpr size_t CS_SMEM = (size_t)CS_WARPS * CS_SLOTS * 5;
-constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9;
-
 // log2 of the CTAs per group: the smallest power of two with 2^c * CB_PART >= w
 static int cached_split_log2(int64_t w) {
     int c = 0;
@@ -918,7 +1131,7 @@ static int cached_grid(int64_t n, int64_t w) {
     if (w <= CS_SLOTS) return grid_for(n < 1 ? 1 : n, CS_NT, CS_CTAS_PER_SM);
     const int c = cached_split_log2(w);
     const int64_t quads = ((n < 1 ? 1 : n) + 3) / 4;
-    int64_t groups = (quads + CB_NT * CB_U - 1) / (CB_NT * CB_U);
+    int64_t groups = (quads + CB_NT - 1) / CB_NT;
     const int64_t cap = NUM_SMS_B200 >> c > 0 ? NUM_SMS_B200 >> c : 1;
     if (groups > cap) groups = cap;
     return (int)(groups << c);
@@ -940,12 +1153,14 @@ static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, 
     *G_out = cached_tables(n, w);
     if (w <= CS_SLOTS) {
         auto kern = rbi_cached_small_kernel<ACC, COUNT_ZEROS>;
-        VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CS_NT, CS_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CS_SMEM) != cudaSuccess)
+            return VJP_ERR_CUDA;
+        VJP_LAUNCH(K_CACHED_SMALL, stream) kern<<<G, CS_NT, CS_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
     } else {
-        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS, CB_U>;
+        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CB_SMEM) != cudaSuccess)
             return VJP_ERR_CUDA;
-        VJP_LAUNCH(K_CACHED_ACC, stream) kern<<<G, CB_NT, CB_SMEM, stream>>>(n, w, cached_split_log2(w), is, vs, part, zeros, S);
+        VJP_LAUNCH(K_CACHED_BIG, stream) kern<<<G, CB_NT, CB_SMEM, stream>>>(n, w, cached_split_log2(w), is, vs, part, zeros, S);
     }
     return last_launch_status();
 }
@@ -995,7 +1210,7 @@ template <bool SMEM>
 __global__ void __launch_bounds__(RBI_NT)
 rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                      const float *__restrict__ vs, const float2 *__restrict__ coef,
-                     float *__restrict__ vs_bar) {
+                     float *__restrict__ vs_bar, int accumulate) {
     extern __shared__ uint4 smem_raw[];
     float2 *sh = reinterpret_cast<float2 *>(smem_raw);
     if (SMEM) {
@@ -1017,7 +1232,7 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             if (z == 0) o[j] = c.x / v[j];
             else if (z == 1 && v[j] == 0.f) o[j] = c.x;
         }
-        store_vals4(vs_bar, q * 4, cnt, o);
+        store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
     }
 }
 
@@ -1039,9 +1254,9 @@ static MulWs mul_carve(void *ws, int64_t w) {
 
 int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
                    const float *hist_bar, float *vs_bar, int64_t *zeros, float *prod_nz, void *ws,
-                   cudaStream_t stream) {
+                   int accumulate, cudaStream_t stream) {
     if (w == 0) {
-        if (vs_bar && n > 0 &&
+        if (vs_bar && n > 0 && !accumulate &&
             cudaMemsetAsync(vs_bar, 0, (size_t)n * sizeof(float), stream) != cudaSuccess)
             return VJP_ERR_CUDA;
         return VJP_OK;
@@ -1058,9 +1273,9 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         const size_t bytes = (size_t)w * sizeof(float2);
         if (bytes <= GATHER_SMEM_MAX / 2)
-            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<true><<<grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar);
+            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<true><<<grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar, accumulate);
         else
-            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<false><<<grid, RBI_NT, 0, stream>>>(n, w, is, vs, m.coef, vs_bar);
+            VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<false><<<grid, RBI_NT, 0, stream>>>(n, w, is, vs, m.coef, vs_bar, accumulate);
     }
     return last_launch_status();
 }
@@ -1070,7 +1285,7 @@ size_t rbi_special_workspace_bytes(int code, int, int64_t n, int64_t w) {
     if (w < 1) w = 1;
     switch (code) {
     case VJP_OP_MIN:
-    case VJP_OP_MAX: return align_up((size_t)w * 8, 256);
+    case VJP_OP_MAX: return minmax_ws_bytes(w);
     case VJP_OP_MUL:
         return align_up((size_t)w * 4, 256) + align_up((size_t)w * 8, 256) + cached_part_bytes(n, w);
     default: return 256;
@@ -1078,7 +1293,7 @@ size_t rbi_special_workspace_bytes(int code, int, int64_t n, int64_t w) {
 }
 size_t rbi_forward_workspace_bytes(int code, int64_t n, int64_t w) {
     if (code == VJP_OP_MUL || code == VJP_OP_SATADD) return cached_part_bytes(n, w);
-    if (code == VJP_OP_MIN || code == VJP_OP_MAX) return align_up((size_t)(w < 1 ? 1 : w) * 8, 256);
+    if (code == VJP_OP_MIN || code == VJP_OP_MAX) return minmax_ws_bytes(w < 1 ? 1 : w);
     return 256;
 }
 

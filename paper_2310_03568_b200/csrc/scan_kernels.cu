@@ -9,8 +9,7 @@
 //                      reduction); tile_exscan_kernel turns the aggregates into exclusive tile
 //                      prefixes fpre[t] = fold of all elements before tile t: the forward
 //                      re-execution the return sweep needs (r_{i-1} of P:L613; re-execution
-//                      instead of a tape).  MODE_TILEPRE (prefixes by look-back) is kept
-//                      for reference; the VJP no longer uses it.
+//                      instead of a tape).
 //   scan_vjp_reverse_kernel<Op, NT, IPT>
 //       the general rule of Fig. 7 in one kernel: Jacobians formed on the fly
 //       (never stored), reverse linear-recurrence scan with lin_o
@@ -25,7 +24,7 @@
 
 namespace vjp {
 
-enum : int { MODE_SCAN = 0, MODE_TILEPRE = 1, MODE_TILEAGG = 2 };
+enum : int { MODE_SCAN = 0, MODE_TILEAGG = 2 };
 
 template <class S>
 struct LookbackWs {
@@ -73,10 +72,10 @@ template <class Op, int NT, int IPT, bool REV, int MODE>
 __global__ void __launch_bounds__(NT)
 scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int64_t n,
                      int num_tiles, LookbackWs<typename Op::Fwd> ws,
-                     typename Op::Fwd *__restrict__ fpre) {
+                     typename Op::Fwd *__restrict__ fpre, int accumulate) {
     using M = FwdMonoid<Op>;
     using S = typename Op::Fwd;
-    constexpr int EW = Op::EW, RW = IPT * EW, SW = sizeof(S) / 4;
+    constexpr int EW = Op::EW, RW = IPT * EW;
     using St = Stage<NT, RW>;
     using BS = BlockScan<M, NT>;
     extern __shared__ uint4 smem[];
@@ -131,10 +130,6 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     __syncthreads();
     const S pre = load_state_smem<S>(bcast);
 
-    if (MODE == MODE_TILEPRE) {
-        if (threadIdx.x == 0) store_state_cg(fpre + t, pre);
-        return;
-    }
     // REV is only instantiated for commutative operators ('+'): operand order is immaterial there
     S run = Op::combine(pre, ex);
     if (!REV) {
@@ -152,7 +147,7 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     }
     if constexpr (!WIDE) St::write_row(smem, threadIdx.x, rr);
     __syncthreads();
-    St::store(smem, out + base * EW, valid * EW);
+    St::template store<typename Op::T>(smem, out + base * EW, valid * EW, accumulate != 0);
 }
 
 // In-place exclusive scan of the per-tile aggregates (a few thousand states) by ONE thread-block
@@ -180,6 +175,7 @@ tile_exscan_kernel(int num_tiles, typename Op::Fwd *__restrict__ fpre) {
     for (int i = lo; i < hi; i++) acc = Op::combine(acc, load_state_cg(fpre + i));
     S total;
     const S ex = BS::template exclusive<false>(acc, total, scratch);
+    cluster.sync();  // every CTA of the cluster has started: its shared memory may be written remotely
     if (threadIdx.x < XCL) {  // thread r delivers this CTA's total to CTA r
         uint32_t *dst = cluster.map_shared_rank(&tot[0][0], threadIdx.x) + rank * SW;
         store_state_smem(dst, total);
@@ -204,7 +200,7 @@ __global__ void __launch_bounds__(NT, (Op::EW <= 4 ? 1024 / NT : 1))
 scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
                         uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
                         const typename Op::Fwd *__restrict__ fpre,
-                        LookbackWs<typename RevMonoid<Op>::State> ws) {
+                        LookbackWs<typename RevMonoid<Op>::State> ws, int accumulate) {
     using RM = RevMonoid<Op>;
     using RS = typename RM::State;
     using FM = FwdMonoid<Op>;
@@ -303,7 +299,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
         St::write_row(sy, threadIdx.x, rry);
     }
     __syncthreads();
-    St::store(sy, xbar + base * EW, valid * EW);
+    St::template store<typename Op::T>(sy, xbar + base * EW, valid * EW, accumulate != 0);
 }
 
 // ------------------------------------------------------------------ host side ------------
@@ -334,7 +330,7 @@ static int64_t tiles_of(int64_t n, int tile) { return (n + tile - 1) / tile; }
 
 template <class Op, int NT, int IPT, bool REV, int MODE>
 static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre, char *ws,
-                    cudaStream_t stream) {
+                    int accumulate, cudaStream_t stream) {
     using S = typename Op::Fwd;
     const int64_t nt = tiles_of(n, NT * IPT);
     size_t zero_bytes;
@@ -345,9 +341,9 @@ static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
-    VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : (MODE == MODE_TILEAGG ? K_SCAN_TILEAGG : K_SCAN_TILEPRE), stream)
+    VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : K_SCAN_TILEAGG, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(in),
-                                             static_cast<uint32_t *>(out), n, (int)nt, lw, fpre);
+                                             static_cast<uint32_t *>(out), n, (int)nt, lw, fpre, accumulate);
     return last_launch_status();
 }
 
@@ -368,7 +364,7 @@ static size_t ws_bytes_vjp_cfg(int64_t n) {
 
 template <class Cfg>
 static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, char *ws,
-                   cudaStream_t stream) {
+                   int accumulate, cudaStream_t stream) {
     using Op = typename Cfg::op;
     using FS = typename Op::Fwd;
     using RS = typename RevMonoid<Op>::State;
@@ -379,7 +375,7 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     FS *fpre = reinterpret_cast<FS *>(ws_rev + lookback_bytes<RS>(nt));
     // (A) forward tile prefixes: streaming per-tile aggregates, then their exclusive scan by one cluster
     int rc;
-    rc = run_scan<Op, NT, IPT, false, MODE_TILEAGG>(n, xs, nullptr, fpre, ws_fwd, stream);
+    rc = run_scan<Op, NT, IPT, false, MODE_TILEAGG>(n, xs, nullptr, fpre, ws_fwd, 0, stream);
     if (rc != VJP_OK) return rc;
     constexpr int XNT = sizeof(FS) > 32 ? 128 : 512;
     cudaLaunchConfig_t cfg = {};
@@ -408,7 +404,7 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     VJP_LAUNCH(K_SCAN_VJP_REVERSE, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(xs),
                                              static_cast<const uint32_t *>(ys_bar),
-                                             static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw);
+                                             static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw, accumulate);
     return last_launch_status();
 }
 
@@ -450,22 +446,22 @@ size_t scan_workspace_bytes(int code, int dtype, int64_t n) {
 
 int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,
                         cudaStream_t stream) {
-#define F(C) return run_scan<typename C::op, C::NT, C::IPT, false, MODE_SCAN>(n, xs, ys, nullptr, (char *)ws, stream);
+#define F(C) return run_scan<typename C::op, C::NT, C::IPT, false, MODE_SCAN>(n, xs, ys, nullptr, (char *)ws, 0, stream);
     VJP_SCAN_DISPATCH(code, dtype, F, return VJP_ERR_UNSUPPORTED;)
 #undef F
     return VJP_ERR_UNSUPPORTED;
 }
 
 int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *ys_bar,
-                    void *xs_bar, void *ws, cudaStream_t stream) {
+                    void *xs_bar, void *ws, int accumulate, cudaStream_t stream) {
     if (code == VJP_OP_ADD) {  // reverse inclusive sum of ys_bar
         if (dtype == VJP_F32)
             return run_scan<OpAdd<float>, CfgAddF32::NT, CfgAddF32::IPT, true, MODE_SCAN>(
-                n, ys_bar, xs_bar, nullptr, (char *)ws, stream);
+                n, ys_bar, xs_bar, nullptr, (char *)ws, accumulate, stream);
         return run_scan<OpAdd<double>, CfgAddF64::NT, CfgAddF64::IPT, true, MODE_SCAN>(
-            n, ys_bar, xs_bar, nullptr, (char *)ws, stream);
+            n, ys_bar, xs_bar, nullptr, (char *)ws, accumulate, stream);
     }
-#define F(C) return run_vjp<C>(n, xs, ys_bar, xs_bar, (char *)ws, stream);
+#define F(C) return run_vjp<C>(n, xs, ys_bar, xs_bar, (char *)ws, accumulate, stream);
     switch (code) {
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
     case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } break;
