@@ -50,8 +50,10 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
     return float(table.get(name, 0.0))
 
 
-def event_time_ms(fn, reps: int, warmup: int = 3):
-    """Per-call device times (ms) of fn() on the current stream, CUDA events, after warm-up."""
+def event_time_ms(fn, reps: int, warmup: int = 3, inner: int = 4):
+    """Per-call device times (ms) of fn() on the current stream, CUDA events, after warm-up.  Each sample
+    brackets `inner` back-to-back calls (divided out): with one call per event pair the host-side cost of a
+    call (ctypes + argument checks, ~20 us) would be measured instead of a kernel that takes 12 us."""
     for _ in range(warmup):
         fn()
     torch.cuda.synchronize()
@@ -59,10 +61,11 @@ def event_time_ms(fn, reps: int, warmup: int = 3):
     for _ in range(reps):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        fn()
+        for _ in range(inner):
+            fn()
         b.record()
         b.synchronize()
-        out.append(a.elapsed_time(b))
+        out.append(a.elapsed_time(b) / inner)
     return out
 
 

@@ -54,7 +54,7 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "scan_lookback_kernel<MODE_SCAN>", "scan_lookback_kernel<MODE_TILEAGG>",
     "tile_exscan_kernel", "scan_vjp_reverse_kernel",
     "rbi_fill_kernel", "rbi_forward_kernel", "rbi_vjp_add_kernel",
-    "rbi_minmax_lifted_kernel", "rbi_minmax_sample_kernel", "rbi_minmax_finish_kernel", "rbi_cached_small_kernel", "rbi_cached_big_kernel",
+    "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_cached_small_kernel", "rbi_cached_big_kernel",
     "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel"};

@@ -26,7 +26,7 @@ inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 enum KernelId : int {
     K_SCAN_LOOKBACK = 0, K_SCAN_TILEAGG, K_SCAN_TILEPRE /* tile_exscan_kernel */, K_SCAN_VJP_REVERSE,
     K_RBI_FILL, K_RBI_FORWARD, K_RBI_GATHER,
-    K_MINMAX_LIFTED, K_MINMAX_SAMPLE, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
+    K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_COUNT
 };

@@ -347,7 +347,6 @@ template <bool IS_MAX, bool TAGGED>
 __global__ void __launch_bounds__(MMF_NT, 1)
 rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                            const float *__restrict__ vs, unsigned long long *tab,
-                           const uint4 *__restrict__ seed /* [8192] packed 16-bit bounds, or NULL */,
                            float *__restrict__ vs_bar) {
     extern __shared__ uint4 smem_raw[];
     uint16_t *f16 = reinterpret_cast<uint16_t *>(smem_raw);  // [65536]
@@ -361,8 +360,7 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
     }
-    for (int i = threadIdx.x; i < (int)(MMF_SMEM / 16); i += MMF_NT)
-        smem_raw[i] = (!TAGGED && seed) ? __ldg(seed + i) : make_uint4(~0u, ~0u, ~0u, ~0u);
+    for (int i = threadIdx.x; i < (int)(MMF_SMEM / 16); i += MMF_NT) smem_raw[i] = make_uint4(~0u, ~0u, ~0u, ~0u);
     __syncthreads();
     while (q * 4 < n) {
         // next iteration's loads fly while this one walks the table (its L2 round trips are dependent)
@@ -378,13 +376,14 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
         }
+        // one element at a time (filter, table read, update): a hot bin's elements meet a fresh bound
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             if (!in_range(k[j], w)) continue;
             const uint32_t vk = ext_key<IS_MAX>(v[j]);
             const uint32_t p16 = vk >> 16;
             const uint32_t b = (uint32_t)k[j];
-            const bool wide = TAGGED && (b >> 31);  // the 16-bit tag cannot name bins >= 2^31: no filter
+            const bool wide = TAGGED && (b >> 31);  // the 16-bit tag cannot name bins >= 2^31: never filtered
             if (TAGGED) {
                 const uint32_t e = f32[b & 32767u];
                 if (!wide && (e >> 16) == (b >> 15) && p16 > (e & 0xffffu)) continue;
@@ -414,40 +413,6 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
-// Seeding of the filter (w <= 65536).  With 148 private filters a CTA sees a bin of a wide histogram
-// only a few times (uniform keys, w = 2^16, n = 2^24: 1.7 times), so a filter that starts empty lets
-// most elements through to L2 (profiles/r1l: one dependent L2 sector read per element, 34 % DRAM).  A
-// SAMPLE pass first runs the lifted operator over every 16th block of 1024 elements -- the packed keys
-// it leaves in `tab` are valid partial results, the main pass simply continues from them -- and the
-// 16-bit prefixes of those keys become the initial bound of every CTA's filter: an element then passes
-// with probability ~ 1/17 instead of ~ 1/1.7.
-constexpr int MMS_NT = 256, MMS_EVERY = 16;
-
-template <bool IS_MAX>
-__global__ void __launch_bounds__(MMS_NT)
-rbi_minmax_sample_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
-                         const float *__restrict__ vs, unsigned long long *tab) {
-    const int64_t q = ((int64_t)blockIdx.x * MMS_EVERY) * MMS_NT + threadIdx.x;
-    if (q * 4 >= n) return;
-    int64_t k[4];
-    float v[4];
-    const int cnt = load_keys4(is, q * 4, n, k);
-    load_vals4(vs, q * 4, cnt, v);
-#pragma unroll
-    for (int j = 0; j < 4; j++) {
-        if (!in_range(k[j], w)) continue;
-        const unsigned long long key =
-            ((unsigned long long)ext_key<IS_MAX>(v[j]) << 32) | (unsigned)(q * 4 + j);
-        if (key < __ldcg(tab + k[j])) atomicMin(tab + k[j], key);
-    }
-}
-
-__global__ void rbi_minmax_seed_kernel(int64_t w, const unsigned long long *__restrict__ tab,
-                                       uint16_t *__restrict__ seed /* [65536] */) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < 65536) seed[k] = k < w ? (uint16_t)(__ldcg(tab + k) >> 48) : (uint16_t)0xffffu;
-}
-
 // arg / ext of every bin (an empty bin is (n, +-inf)) and the scatter of the return sweep
 // (P:L438-441).  vs_bar has been zeroed before.
 template <bool IS_MAX>
@@ -468,8 +433,7 @@ __global__ void rbi_minmax_finish_kernel(int64_t n, int64_t w, const unsigned lo
 }
 
 constexpr size_t MINMAX_SMEM_MAX = 64 * 1024;
-// packed keys [w] + (8192 < w <= 65536) the 65536 16-bit filter seeds
-static size_t minmax_ws_bytes(int64_t w) { return align_up((size_t)w * 8, 256) + ((size_t)w * 8 > MINMAX_SMEM_MAX && w <= 65536 ? 65536 * 2 : 0); }
+static size_t minmax_ws_bytes(int64_t w) { return align_up((size_t)w * 8, 256); }  // packed keys [w]
 
 template <bool IS_MAX>
 static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
@@ -499,20 +463,12 @@ static int run_minmax(int64_t n, int64_t w, const int64_t *is, const float *vs,
             auto kern = rbi_minmax_filtered_kernel<IS_MAX, false>;
             if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
                 return VJP_ERR_CUDA;
-            const uint4 *seed = nullptr;
-            const int64_t quads = (n + 3) / 4, sblocks = (quads + (int64_t)MMS_NT * MMS_EVERY - 1) / ((int64_t)MMS_NT * MMS_EVERY);
-            if (sblocks >= 64) {  // enough input for the sample to be worth two more launches
-                uint16_t *seed16 = reinterpret_cast<uint16_t *>(static_cast<char *>(ws) + align_up((size_t)w * 8, 256));
-                VJP_LAUNCH(K_MINMAX_SAMPLE, stream) rbi_minmax_sample_kernel<IS_MAX><<<(unsigned)sblocks, MMS_NT, 0, stream>>>(n, w, is, vs, tab);
-                VJP_LAUNCH(K_MINMAX_SAMPLE, stream) rbi_minmax_seed_kernel<<<256, 256, 0, stream>>>(w, tab, seed16);
-                seed = reinterpret_cast<const uint4 *>(seed16);
-            }
-            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, seed, vs_bar);
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
         } else {
             auto kern = rbi_minmax_filtered_kernel<IS_MAX, true>;
             if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MMF_SMEM) != cudaSuccess)
                 return VJP_ERR_CUDA;
-            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, nullptr, vs_bar);
+            VJP_LAUNCH(K_MINMAX_LIFTED, stream) kern<<<grid_for(n, MMF_NT, 1), MMF_NT, MMF_SMEM, stream>>>(n, w, is, vs, tab, vs_bar);
         }
     }
     const int fb = (int)((w + 255) / 256 < 1184 ? (w + 255) / 256 : 1184);
@@ -531,28 +487,36 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
 
 // ------------------------------------------------- cached accumulation ('*', satadd) -------
 //
-// Operators with no hardware atomic (the paper's "atomicMul-class update").  One
-// shared-memory atomicCAS per element is not affordable: ATOMS costs 2 cycles per lane on the SM's
-// LSU pipe, 64x a plain LDS/STS, and a CAS loop on a hot bin retries without bound (profiles/r1a:
-// 5 ms at Zipf keys); match.any issues about once per 30 cycles per SM (profiles/r1b).  So tables
-// in shared memory are updated with plain loads and stores under a CLAIM ROUND:
+// Operators with no hardware atomic (the paper's "atomicMul-class update").  A shared-memory
+// atomicCAS is not affordable on any common path: one ATOMS.CAS warp instruction occupies the LSU for
+// ~64 cycles WHATEVER the number of active lanes (profiles/r2a: three of them per batch of 128 elements
+// cost as much as everything else together), and a CAS loop on a hot bin retries without bound
+// (profiles/r1a: 5 ms at Zipf keys); match.any issues about once per 30 cycles per SM (profiles/r1b).
+// So tables in shared memory are updated with plain loads and stores under a CLAIM ROUND.
+//
+// w <= CS_SLOTS (rbi_cached_small_kernel): a table per WARP, claims NaN-boxed into the table cells:
 //   A. every pending element reads its bin's cell and, unless the cell already holds a claim,
 //      overwrites it with a claim word naming the element -- a NaN-boxed pattern (sign 1, exponent
 //      0xff, mantissa 0x7xxxxx | id) that no value the operators produce ever has (NaN inputs are
 //      unsupported; FMUL / FADD generate the canonical NaN 0x7fffffff).  No separate claim array.
-//   B. after a barrier the element that reads its own claim back OWNS the bin for this round and
+//   B. after a __syncwarp the element that reads its own claim back OWNS the bin for this round and
 //      stores comb(old value, its value); every claimed cell has exactly one owner (the last
 //      claim written), and every claim writer has read the cell's real value (values only change
-//      in B, claims only appear in A).  Uniform keys: 3 - 6 % of the elements lose.
-//   C. losers: one compare-and-swap loop on the cell (few, uncontended at uniform keys).
-// Skewed keys would make C the whole kernel, so every WARP keeps a small DIRECTORY of hot bins
+//      in B, claims only appear in A).  Uniform keys at w = 1024: 6 % of the elements lose.
+//   C. losers: further claim rounds over one element per lane -- no atomics anywhere.
+// Skewed keys would make C the whole kernel, so every warp keeps a small DIRECTORY of hot bins
 // (DIR_S direct-mapped slots) whose accumulators are LANE-PRIVATE (hot[slot][lane]: bank = lane):
 // an element of a resident bin is folded into its lane's accumulator with a plain read-modify-write
 // -- no claim, no conflict, whatever the multiplicity of the bin.  The directory is trained by the
-// warp itself: a bin seen contended twice and hotter (in the current batch) than the slot's
-// resident replaces it (the resident's 32 accumulators are folded with shuffles and written back).
+// warp itself: a bin whose elements are still pending after two retry rounds (multiplicity >= 4 in a
+// batch: rare at uniform keys) and that is hotter in the current batch than the slot's resident
+// replaces it (the resident's 32 accumulators are folded with shuffles and written back).
 // The directory is consulted only once it holds an entry: uniform keys never pay for it.
-// CTA g writes its result to part[g][.]; a second kernel folds the G tables per bin in a fixed order.
+//
+// w > CS_SLOTS (rbi_cached_big_kernel): one table per CTA, CTA-wide claim rounds through a separate
+// claim array, guarded warp caches and a thread-private register entry for contended bins (described
+// at the kernel).  CTA g writes its result to part[g][.]; a second kernel folds the G tables per bin
+// in a fixed order.
 
 constexpr uint32_t CLAIM = 0xFFF00000u;     // claim words are >= CLAIM as unsigned integers
 constexpr uint32_t BIN_NONE = 0xffffffffu;  // no pending element
@@ -596,10 +560,9 @@ VJP_DEVINL float warp_fold(float x, float S) {
     return x;
 }
 
-// Directory of one warp: dir[DIR_S] resident bins, seen[DIR_S] last contended candidate per slot,
-// hot[DIR_S][32] lane-private accumulators.
+// Directory of one warp: dir[DIR_S] resident bins, hot[DIR_S][32] lane-private accumulators.
 struct WarpDir {
-    uint32_t *dir, *seen;
+    uint32_t *dir;
     float *hot;
 };
 
@@ -621,20 +584,13 @@ VJP_DEVINL void dir_lookup(const WarpDir &d, uint32_t (&b)[NI], const float (&v)
 }
 
 // Called by the whole warp with a contended candidate bin `cand` (warp-uniform) that `c` lanes hold
-// in elements still pending.  Installs it if it was the slot's candidate before and the slot's resident
-// is colder in this batch; then the pending elements of cand are absorbed.  Returns true on install.
+// in elements still pending.  Installs it if the slot's resident is colder in this batch (fewer lanes hit
+// it than hold the candidate); then the pending elements of cand are absorbed.  Returns true on install.
 // flush(bin, value): adds the evicted resident's fold to the table (called by lane 0 only).
 template <int ACC, int NI, class Flush>
 VJP_DEVINL bool dir_train(const WarpDir &d, uint32_t cand, int c, uint32_t hitm, uint32_t (&b)[NI],
                           const float (&v)[NI], int lane, float S, int &ndir, Flush flush) {
     const uint32_t s = cand & (DIR_S - 1);
-    const uint32_t prev = d.seen[s];
-    __syncwarp();
-    if (prev != cand) {
-        if (lane == 0) d.seen[s] = cand;
-        __syncwarp();
-        return false;
-    }
     const int h = __popc(__ballot_sync(FULL_MASK, (hitm >> s) & 1u));
     if (c <= h) return false;
     const uint32_t old = d.dir[s];
@@ -663,8 +619,12 @@ VJP_DEVINL bool dir_train(const WarpDir &d, uint32_t cand, int c, uint32_t hitm,
 // kept out of the product.  Otherwise: the plain primal histogram of the operator.
 //
 // w <= CS_SLOTS: every warp owns a private table (a slot IS a bin) and runs the claim round over the
-// 128 elements of its batch (one quad per lane) with __syncwarp as the barrier.
-constexpr size_t CS_SMEM = (size_t)CS_WARPS * (CS_SLOTS * 4 + DIR_S * 32 * 4 + 2 * DIR_S * 4);
+// 128 elements of its batch (one quad per lane) with __syncwarp as the barrier.  The hot loop is
+// branch-free: an element that takes no part (key out of range, a counted zero, a directory hit) is
+// pointed at its lane's DUMMY cell behind the table and goes through the same loads and stores
+// (profiles/r2a: the first version spent 340 instructions per quad, most of them control flow).
+constexpr int CS_TAB = CS_SLOTS + 32;  // + one dummy cell per lane
+constexpr size_t CS_SMEM = (size_t)CS_WARPS * (CS_TAB * 4 + DIR_S * 32 * 4 + DIR_S * 4);
 
 template <int ACC, bool COUNT_ZEROS>
 __global__ void __launch_bounds__(CS_NT, CS_CTAS_PER_SM)
@@ -673,112 +633,160 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                         float S) {
     using OP = CachedOp<ACC>;
     extern __shared__ uint4 smem_raw[];
-    uint32_t *tabs = reinterpret_cast<uint32_t *>(smem_raw);                  // [CS_WARPS][CS_SLOTS]
-    float *hots = reinterpret_cast<float *>(tabs + CS_WARPS * CS_SLOTS);      // [CS_WARPS][DIR_S][32]
-    uint32_t *dirs = reinterpret_cast<uint32_t *>(hots + CS_WARPS * DIR_S * 32);  // [CS_WARPS][2][DIR_S]
+    uint32_t *tabs = reinterpret_cast<uint32_t *>(smem_raw);                  // [CS_WARPS][CS_TAB]
+    float *hots = reinterpret_cast<float *>(tabs + CS_WARPS * CS_TAB);        // [CS_WARPS][DIR_S][32]
+    uint32_t *dirs = reinterpret_cast<uint32_t *>(hots + CS_WARPS * DIR_S * 32);  // [CS_WARPS][DIR_S]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *tab = tabs + warp * CS_SLOTS;
+    uint32_t *tab = tabs + warp * CS_TAB;
     WarpDir d;
     d.hot = hots + warp * DIR_S * 32;
-    d.dir = dirs + warp * 2 * DIR_S;
-    d.seen = d.dir + DIR_S;
-    for (int s = lane; s < CS_SLOTS; s += 32) tab[s] = __float_as_uint(OP::neutral());
+    d.dir = dirs + warp * DIR_S;
+    for (int s = lane; s < CS_TAB; s += 32) tab[s] = __float_as_uint(OP::neutral());
     for (int s = lane; s < DIR_S * 32; s += 32) d.hot[s] = OP::neutral();
-    if (lane < 2 * DIR_S) d.dir[lane] = DIR_EMPTY;
+    if (lane < DIR_S) d.dir[lane] = DIR_EMPTY;
     __syncwarp();
     int ndir = 0;  // warp-uniform: resident directory entries
     const uint32_t myid = CLAIM | (uint32_t)(lane * 4);
+    const uint32_t dummy = CS_SLOTS + lane, w32 = (uint32_t)w;
     auto flush = [&](uint32_t bin, float x) { tab[bin] = __float_as_uint(OP::comb(__uint_as_float(tab[bin]), x, S)); };
 
-    const int64_t nquads = (n + 3) / 4;
-    const int64_t stride = (int64_t)gridDim.x * CS_NT;
-    int64_t qw = blockIdx.x * (int64_t)CS_NT + warp * 32;  // warp-uniform: the warp never diverges here
-    int64_t k[4] = {-1, -1, -1, -1};
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (qw < nquads && qw + lane < nquads) {
-        const int cnt = load_keys4(is, (qw + lane) * 4, n, k);
-        load_vals4(vs, (qw + lane) * 4, cnt, v);
-    }
-    while (qw < nquads) {
-        int64_t kn[4] = {-1, -1, -1, -1};
-        float vn[4] = {0.f, 0.f, 0.f, 0.f};
-        const int64_t qn = qw + stride;
-        if (qn + lane < nquads) {  // next iteration's loads fly while this one is processed
-            const int cnt = load_keys4(is, (qn + lane) * 4, n, kn);
-            load_vals4(vs, (qn + lane) * 4, cnt, vn);
-        }
-        uint32_t b[4];
+    // one batch: the quad (k, v) of every lane
+    auto process = [&](const int64_t (&k)[4], const float (&v)[4]) {
+        uint32_t b[4];  // table index of a pending element, `dummy` otherwise
+        bool zq = false;
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            bool act = in_range(k[j], w);
-            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
-                atomicAdd(zeros + k[j], 1u);
-                act = false;
+            const uint32_t lo = (uint32_t)k[j], hi = (uint32_t)((uint64_t)k[j] >> 32);
+            bool act = (hi == 0u) & (lo < w32);
+            if (COUNT_ZEROS) {
+                const bool z = act & (v[j] == 0.f);  // IEEE equality: +-0 only (Q7)
+                zq |= z;
+                act &= !z;
             }
-            b[j] = act ? (uint32_t)k[j] : BIN_NONE;
+            b[j] = act ? lo : dummy;
+        }
+        if (COUNT_ZEROS && zq) {  // rare
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                if (in_range(k[j], w) && v[j] == 0.f) atomicAdd(zeros + k[j], 1u);
         }
         uint32_t hitm = 0;
-        if (ndir) dir_lookup<ACC, 4>(d, b, v, lane, S, hitm);
-        // claim round over the warp's 128 elements
-        uint32_t o[4];
+        if (ndir) {
 #pragma unroll
-        for (int j = 0; j < 4; j++) o[j] = tab[b[j] & (CS_SLOTS - 1)];
+            for (int j = 0; j < 4; j++) {
+                const uint32_t s = b[j] & (DIR_S - 1);
+                if (d.dir[s] == b[j]) {  // a dummy index never matches: entries are bins or DIR_EMPTY
+                    float *h = d.hot + s * 32 + lane;
+                    *h = OP::comb(*h, v[j], S);
+                    hitm |= 1u << s;
+                    b[j] = dummy;
+                }
+            }
+        }
+        // claim round over the warp's 128 elements
+        uint32_t o[4], c[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) o[j] = tab[b[j]];
 #pragma unroll
         for (int j = 0; j < 4; j++)
-            if (b[j] != BIN_NONE && o[j] < CLAIM) tab[b[j]] = myid + j;
+            if (o[j] < CLAIM) tab[b[j]] = myid + j;
         __syncwarp();
-        uint32_t c[4];
 #pragma unroll
-        for (int j = 0; j < 4; j++) c[j] = tab[b[j] & (CS_SLOTS - 1)];
-        bool lost = false;
+        for (int j = 0; j < 4; j++) c[j] = tab[b[j]];
+        uint32_t pm = 0;  // bit j: a real element that lost
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            if (b[j] == BIN_NONE) continue;
-            if (c[j] == myid + j) {
-                tab[b[j]] = __float_as_uint(OP::comb(__uint_as_float(o[j]), v[j], S));
-                b[j] = BIN_NONE;
-            } else {
-                lost = true;
-            }
+            const bool win = c[j] == myid + j;
+            if (win) tab[b[j]] = __float_as_uint(OP::comb(__uint_as_float(o[j]), v[j], S));
+            pm |= (uint32_t)(!win & (b[j] < (uint32_t)CS_SLOTS)) << j;
         }
         __syncwarp();
-        const unsigned lm = __ballot_sync(FULL_MASK, lost);
-        if (lm) {
-            // directory training: the first loser of the lowest lane is this batch's candidate
-            const uint32_t mine = b[0] != BIN_NONE ? b[0] : b[1] != BIN_NONE ? b[1] : b[2] != BIN_NONE ? b[2] : b[3];
-            const uint32_t cand = __shfl_sync(FULL_MASK, mine, __ffs(lm) - 1);
-            const bool has = (b[0] == cand) | (b[1] == cand) | (b[2] == cand) | (b[3] == cand);
-            const int cl = __popc(__ballot_sync(FULL_MASK, has));
-            dir_train<ACC, 4>(d, cand, cl, hitm, b, v, lane, S, ndir, flush);
-            // the remaining losers: claim rounds over one element per lane (a shared-memory atomicCAS
-            // instead costs the LSU ~64 cycles per warp instruction whatever the number of lanes: three of
-            // them per batch made this kernel no faster than the one it replaced)
-            uint32_t pm = (uint32_t)(b[0] != BIN_NONE) | (uint32_t)(b[1] != BIN_NONE) << 1 |
-                          (uint32_t)(b[2] != BIN_NONE) << 2 | (uint32_t)(b[3] != BIN_NONE) << 3;
-            while (__any_sync(FULL_MASK, pm != 0)) {
-                uint32_t pb = BIN_NONE;
-                float pv = 0.f;
-                if (pm & 1u) { pb = b[0]; pv = v[0]; }
-                else if (pm & 2u) { pb = b[1]; pv = v[1]; }
-                else if (pm & 4u) { pb = b[2]; pv = v[2]; }
-                else if (pm & 8u) { pb = b[3]; pv = v[3]; }
-                const uint32_t o1 = tab[pb & (CS_SLOTS - 1)];
-                if (pb != BIN_NONE && o1 < CLAIM) tab[pb] = myid;
-                __syncwarp();
-                const uint32_t c1 = tab[pb & (CS_SLOTS - 1)];
-                if (pb != BIN_NONE && c1 == myid) {
-                    tab[pb] = __float_as_uint(OP::comb(__uint_as_float(o1), pv, S));
-                    pm &= pm - 1;
+        // The losers: claim rounds over one element per lane (a shared-memory atomicCAS instead costs the
+        // LSU ~64 cycles per warp instruction whatever the number of lanes: three of them per batch made this
+        // kernel no faster than the one it replaced).  Elements still pending after two such rounds sit in a
+        // bin of multiplicity >= 4: skewed keys -- the directory is trained with that bin.
+        for (int it = 0; __any_sync(FULL_MASK, pm != 0); it++) {
+            if (it >= 2 && (it & 1) == 0) {
+                const unsigned lm = __ballot_sync(FULL_MASK, pm != 0);
+                const uint32_t mine = (pm & 1u) ? b[0] : (pm & 2u) ? b[1] : (pm & 4u) ? b[2] : b[3];
+                const uint32_t cand = __shfl_sync(FULL_MASK, mine, __ffs(lm) - 1);
+                uint32_t pb[4];
+#pragma unroll
+                for (int j = 0; j < 4; j++) pb[j] = (pm >> j & 1u) ? b[j] : BIN_NONE;
+                const bool has = (pb[0] == cand) | (pb[1] == cand) | (pb[2] == cand) | (pb[3] == cand);
+                const int cl = __popc(__ballot_sync(FULL_MASK, has));
+                if (dir_train<ACC, 4>(d, cand, cl, hitm, pb, v, lane, S, ndir, flush)) {
+#pragma unroll
+                    for (int j = 0; j < 4; j++)
+                        if (pb[j] == BIN_NONE) pm &= ~(1u << j);
+                    continue;
                 }
-                __syncwarp();
             }
+            uint32_t pb = dummy;
+            float pv = 0.f;
+            if (pm & 1u) { pb = b[0]; pv = v[0]; }
+            else if (pm & 2u) { pb = b[1]; pv = v[1]; }
+            else if (pm & 4u) { pb = b[2]; pv = v[2]; }
+            else if (pm & 8u) { pb = b[3]; pv = v[3]; }
+            const uint32_t o1 = tab[pb];
+            if (o1 < CLAIM) tab[pb] = myid;
+            __syncwarp();
+            const uint32_t c1 = tab[pb];
+            if (c1 == myid) {
+                tab[pb] = __float_as_uint(OP::comb(__uint_as_float(o1), pv, S));
+                pm &= pm - 1;
+            }
+            __syncwarp();
         }
-#pragma unroll
-        for (int j = 0; j < 4; j++) {
-            k[j] = kn[j];
-            v[j] = vn[j];
+    };
+
+    const uint32_t nfull = (uint32_t)(n / 4);  // quads that exist entirely
+    const uint32_t stride = gridDim.x * CS_NT;
+    // Whole batches: unconditional 128-bit loads, TWO batches in flight per warp (one was not enough: with
+    // half the instructions of the first version the kernel waited on its loads, profiles/r2b).
+    struct Quad {
+        longlong2 a, b;
+        uint4 v;
+    };
+    auto fetch = [&](uint32_t q, Quad &x) {  // warp-uniform q; only whole batches are fetched here
+        if (q + 32 <= nfull) {
+            const longlong2 *kp = reinterpret_cast<const longlong2 *>(is) + 2 * (size_t)(q + lane);
+            x.a = ldg_stream_ll2(kp);
+            x.b = ldg_stream_ll2(kp + 1);
+            x.v = ldg_stream(reinterpret_cast<const uint4 *>(vs) + (q + lane));
         }
-        qw = qn;
+    };
+    auto run = [&](const Quad &x) {
+        const int64_t k[4] = {x.a.x, x.a.y, x.b.x, x.b.y};
+        const float v[4] = {__uint_as_float(x.v.x), __uint_as_float(x.v.y), __uint_as_float(x.v.z), __uint_as_float(x.v.w)};
+        process(k, v);
+    };
+    uint32_t q0 = blockIdx.x * CS_NT + warp * 32, q1 = q0 + stride;  // warp-uniform: the warp never diverges here
+    Quad A = {}, B = {};
+    fetch(q0, A);
+    fetch(q1, B);
+    for (;;) {
+        if (q0 + 32 > nfull) break;
+        const Quad cur = A;
+        q0 += 2 * stride;
+        fetch(q0, A);
+        run(cur);
+        if (q1 + 32 > nfull) break;
+        const Quad cur1 = B;
+        q1 += 2 * stride;
+        fetch(q1, B);
+        run(cur1);
+    }
+    // the ragged end of the input (at most one batch per warp: the first one that is not whole)
+    const uint32_t qw = q0 < q1 ? q0 : q1;
+    if ((int64_t)qw * 4 < n) {
+        int64_t k[4] = {-1, -1, -1, -1};
+        float v[4] = {0.f, 0.f, 0.f, 0.f};
+        if ((int64_t)(qw + lane) * 4 < n) {
+            const int cnt = load_keys4(is, (int64_t)(qw + lane) * 4, n, k);
+            load_vals4(vs, (int64_t)(qw + lane) * 4, cnt, v);
+        }
+        process(k, v);
     }
     for (int s = 0; s < DIR_S; s++) {  // write the directory back
         const uint32_t bin = d.dir[s];
@@ -790,16 +798,12 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     for (int s = threadIdx.x; s < (int)w; s += CS_NT) {
         float acc = __uint_as_float(tabs[s]);
 #pragma unroll
-        for (int wp = 1; wp < CS_WARPS; wp++) acc = OP::comb(acc, __uint_as_float(tabs[wp * CS_SLOTS + s]), S);
+        for (int wp = 1; wp < CS_WARPS; wp++) acc = OP::comb(acc, __uint_as_float(tabs[wp * CS_TAB + s]), S);
         part[(size_t)blockIdx.x * (size_t)w + s] = acc;
     }
 }
 
-// w > CS_SLOTS, warp cache: returns true if (eb, evv) must go to the CTA table.  The lanes of a warp
-// arbitrate per slot through a claim byte (every pending lane stores its lane id, the warp syncs, the
-// lane that reads its own id back owns the slot for this round); a 2-bit hit counter guards the
-// resident entry -- a cold bin arriving at a hot slot decrements it and BYPASSES; only an entry whose
-// counter has run out is evicted (Misra-Gries style).
+// w > CS_SLOTS.  Returns true if (eb, evv) must go to the CTA table.
 template <int ACC>
 VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint32_t *tg, uint8_t *cl,
                                  float S, int lane, uint32_t &eb, float &evv) {
@@ -834,182 +838,192 @@ VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint3
     return ev;
 }
 
+constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
+constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
+constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9;
+
 // w > CS_SLOTS.  A CTA of 1024 threads owns a table of up to CB_PART bins in shared memory.  A
 // histogram wider than that is SPLIT over the 2^c CTAs of a group by the low c bits of the bin
 // (hot neighbouring bins land on different CTAs); all CTAs of a group stream the same part of the
 // input at the same time (one of them pulls it from HBM, the others hit in L2) and each keeps the
 // elements of its own bins: one pass over the input for any w, no traffic between the CTAs.
 //
-// Per batch of 4096 elements (one quad per thread), three barriers:
-//   [directory / warp-cache lookups (skew mode only); claims (A)]  B1  [owners update (B)]  B2
-//   [losers: one compare-and-swap; elements of bins resident in the warp cache: claim-byte rounds on
-//    the entry; a failed compare-and-swap = contended bin -> the warp cache installs it unless a hotter
-//    bin guards the slot; directory training]  B3
-// B3 keeps the compare-and-swaps of C away from the value reads of the next A.  SKEW MODE is switched
-// per batch by the fraction of threads that saw a loser, a cache hit or a directory hit (counted by
-// B2 itself): with uniform keys (3 % losers at w = 2^16) the lookups are skipped altogether; with
-// skewed keys the top bins live in the lane-private directories, the middle ones in the warp caches
-// (fed by failed compare-and-swaps) and only the cold tail takes part in the claim round.
-constexpr size_t CB_SMEM = (size_t)CB_PART * 4 + (size_t)CB_WARPS * (DIR_S * 32 * 4 + 2 * DIR_S * 4) +
-                           (size_t)CB_WARPS * CB_SLOTS * 9;
-constexpr int CB_SKEW_ON = 400, CB_SKEW_OFF = 250;  // threads (of 1024) with a loser / hit in a batch
-
-template <int ACC, bool COUNT_ZEROS>
+// Per batch (U quads per thread) the table is updated WITHOUT atomics:
+//   0. an element whose bin is resident in the warp's cache is "hot" and goes to step 2 directly;
+//   1. one CTA-wide claim round: every pending element stores its id into the bin's claim word,
+//      barrier, the element that reads its id back owns the bin for this round and does a plain
+//      read-modify-write of the table cell.  Uniform keys at w = 2^16: ~6 % of the elements lose.
+//      A loser gets ONE compare-and-swap on the cell (uniform keys: it succeeds);
+//   2. hot elements: claim rounds inside the warp on the resident cache entry (plain LDS/STS); an
+//      element that lost the round AND its compare-and-swap sits in a CONTENDED bin: the warp's
+//      cache installs it unless a hotter bin guards the slot (claim_update_big above).  Hot bins
+//      therefore migrate into the caches and stop taking part in step 1; evictions and bypasses
+//      (cold, rare) fall back to a CAS loop on the table.
+// Barriers: [claim] B1 [plain updates] B2 [CAS, caches].  Two elements never own one bin in a round
+// because all claims precede B1; the plain updates (between B1 and B2) never overlap a CAS (after
+// B2, before the next batch's B1).
+template <int ACC, bool COUNT_ZEROS, int U>
 __global__ void __launch_bounds__(CB_NT, 1)
 rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restrict__ is,
                       const float *__restrict__ vs, float *__restrict__ part, unsigned *zeros,
                       float S) {
     using OP = CachedOp<ACC>;
     extern __shared__ uint4 smem_raw[];
-    uint32_t *table = reinterpret_cast<uint32_t *>(smem_raw);                     // [CB_PART]
-    float *hots = reinterpret_cast<float *>(table + CB_PART);                     // [CB_WARPS][DIR_S][32]
-    uint32_t *dirs = reinterpret_cast<uint32_t *>(hots + CB_WARPS * DIR_S * 32);  // [CB_WARPS][2][DIR_S]
-    float *vals = reinterpret_cast<float *>(dirs + CB_WARPS * 2 * DIR_S);         // [CB_WARPS][CB_SLOTS]
+    float *table = reinterpret_cast<float *>(smem_raw);                          // [CB_PART]
+    float *vals = table + CB_PART;                                               // [CB_WARPS][CB_SLOTS]
     uint32_t *tags = reinterpret_cast<uint32_t *>(vals + CB_WARPS * CB_SLOTS);    // [CB_WARPS][CB_SLOTS]
-    uint8_t *claim = reinterpret_cast<uint8_t *>(tags + CB_WARPS * CB_SLOTS);     // [CB_WARPS][CB_SLOTS]
+    uint16_t *claimA = reinterpret_cast<uint16_t *>(tags + CB_WARPS * CB_SLOTS);  // [CB_PART]
+    uint8_t *claim = reinterpret_cast<uint8_t *>(claimA + CB_PART);               // [CB_WARPS][CB_SLOTS]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float *vl = vals + warp * CB_SLOTS;
     uint32_t *tg = tags + warp * CB_SLOTS;
     uint8_t *cl = claim + warp * CB_SLOTS;
-    WarpDir d;
-    d.hot = hots + warp * DIR_S * 32;
-    d.dir = dirs + warp * 2 * DIR_S;
-    d.seen = d.dir + DIR_S;
     const uint32_t clmask = (1u << cl_log2) - 1u;
     const uint32_t rank = blockIdx.x & clmask;
     const int64_t group = blockIdx.x >> cl_log2, groups = gridDim.x >> cl_log2;
-    for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = __float_as_uint(OP::neutral());
-    for (int s = lane; s < DIR_S * 32; s += 32) d.hot[s] = OP::neutral();
-    if (lane < 2 * DIR_S) d.dir[lane] = DIR_EMPTY;
+    for (int i = threadIdx.x; i < CB_PART; i += CB_NT) table[i] = OP::neutral();
     for (int s = lane; s < CB_SLOTS; s += 32) {
         vl[s] = OP::neutral();
         tg[s] = CB_EMPTY;
     }
     __syncthreads();
-    int ndir = 0;       // warp-uniform
-    bool skew = false;  // CTA-uniform
-    // Losers of a claim round are not resolved with atomics (a shared-memory atomicCAS costs the LSU ~64
-    // cycles per warp instruction): a thread CARRIES up to two of them into the next batch's claim round.
-    uint32_t cb0 = BIN_NONE, cb1 = BIN_NONE;
-    float cv0 = 0.f, cv1 = 0.f;
-    const uint32_t myid = CLAIM | (uint32_t)(threadIdx.x * 8);  // + slot: 0-3 new elements, 4-5 carries
-    auto flush = [&](uint32_t bin, float x) { smem_combine<ACC>(table + bin, x, S); };
-
+    constexpr int NI = 4 * U;
     const int64_t nquads = (n + 3) / 4;
-    const int64_t stride = groups * (int64_t)CB_NT;
-    int64_t q0 = group * (int64_t)CB_NT;  // CTA-uniform: no thread leaves the barriers early
-    int64_t k[4] = {-1, -1, -1, -1};
-    float v[4] = {0.f, 0.f, 0.f, 0.f};
-    if (q0 + threadIdx.x < nquads) {
-        const int cnt = load_keys4(is, (q0 + threadIdx.x) * 4, n, k);
-        load_vals4(vs, (q0 + threadIdx.x) * 4, cnt, v);
-    }
-    while (q0 < nquads) {
-        int64_t kn[4] = {-1, -1, -1, -1};
-        float vn[4] = {0.f, 0.f, 0.f, 0.f};
-        const int64_t qn = q0 + stride;
-        if (qn + threadIdx.x < nquads) {  // next batch's loads fly while this one is processed
-            const int cnt = load_keys4(is, (qn + threadIdx.x) * 4, n, kn);
-            load_vals4(vs, (qn + threadIdx.x) * 4, cnt, vn);
-        }
-        uint32_t b[4];  // table index of a pending element
+    const int64_t stride = groups * (int64_t)(CB_NT * U);
+    int64_t q0 = group * (int64_t)(CB_NT * U);  // CTA-uniform: no thread leaves the barriers early
+    int64_t k[NI];
+    float v[NI];
+    auto load_batch = [&](int64_t q, int64_t (&kk)[NI], float (&vv)[NI]) {
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int u = 0; u < U; u++) {
+            int64_t k4[4] = {-1, -1, -1, -1};
+            float v4[4] = {0.f, 0.f, 0.f, 0.f};
+            const int64_t qq = q + u * CB_NT + threadIdx.x;
+            if (qq < nquads) {
+                const int cnt = load_keys4(is, qq * 4, n, k4);
+                load_vals4(vs, qq * 4, cnt, v4);
+            }
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                kk[u * 4 + j] = k4[j];
+                vv[u * 4 + j] = v4[j];
+            }
+        }
+    };
+    // A claim word names the ELEMENT (thread id * NI + j): exactly one element per bin wins a round,
+    // so all claim words and table cells of a round can be read before any of them is written.
+    const uint32_t id0 = threadIdx.x * NI;
+    // Thread-private register entry (rb, racc, rcnt) in front of everything: a bin that holds a
+    // large share of the elements (one bin = 14 % at Zipf keys) is folded into a register with no
+    // shared-memory access at all.  Weighted majority vote: +CB_RW on a hit, -1 on a miss, replaced
+    // at 0 -- the displaced pair takes the element's place on the normal path.
+    uint32_t rb = CB_EMPTY, rcnt = 0;
+    float racc = OP::neutral();
+    load_batch(q0, k, v);
+    for (;;) {
+        // after the last batch of the input: one more round of the same machinery for the register
+        // entries (1024 CAS on one hot cell would serialise); q0 is CTA-uniform
+        const bool drain = q0 >= nquads;
+        int64_t kn[NI];
+        float vn[NI];
+        const int64_t qn = q0 + stride;
+        load_batch(qn, kn, vn);  // next batch's loads fly while this one is processed (none past the end)
+        uint32_t b[NI];  // table index of a pending element, CB_EMPTY = nothing pending
+        uint32_t zm = 0;
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
             const uint32_t klo = (uint32_t)k[j];
             bool act = in_range(k[j], w) & ((klo & clmask) == rank);
-            if (COUNT_ZEROS && act && v[j] == 0.f) {  // IEEE equality: +-0 only (Q7)
-                atomicAdd(zeros + k[j], 1u);
-                act = false;
+            if (COUNT_ZEROS) {
+                const bool z = act & (v[j] == 0.f);  // IEEE equality: +-0 only (Q7)
+                zm |= (uint32_t)z << j;
+                act &= !z;
             }
-            b[j] = act ? klo >> cl_log2 : BIN_NONE;
+            b[j] = act ? klo >> cl_log2 : CB_EMPTY;
         }
-        uint32_t hitm = 0, hotm = 0;  // hotm bit j: resident in the warp cache
-        bool busy = false;            // this thread saw a directory hit, a cache hit or a loser
-        if (skew) {
-            if (ndir) dir_lookup<ACC, 4>(d, b, v, lane, S, hitm);
+        if (COUNT_ZEROS && zm) {
 #pragma unroll
-            for (int j = 0; j < 4; j++) {
-                const uint32_t t = tg[b[j] & (CB_SLOTS - 1)];
-                // a valid tag never equals CB_EMPTY's, and BIN_NONE matches no tag
-                const bool hot = (t >> 2) == b[j] / CB_SLOTS;
-                hotm |= (uint32_t)hot << j;
-                if (hot & ((t & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t + 1;  // racing lanes store the same word
+            for (int j = 0; j < NI; j++)
+                if (zm >> j & 1u) atomicAdd(zeros + k[j], 1u);
+        }
+        if (drain) {
+            b[0] = rb;
+            v[0] = racc;
+            rcnt = 1;  // keeps the loop below from re-installing it
+            rb = CB_EMPTY;
+        }
+#pragma unroll
+        for (int j = 0; j < NI; j++) {  // register entry
+            if (b[j] == CB_EMPTY) continue;
+            if (b[j] == rb) {
+                racc = OP::comb(racc, v[j], S);
+                rcnt = min(rcnt + CB_RW, CB_RMAX);
+                b[j] = CB_EMPTY;
+            } else if (rcnt == 0) {
+                const uint32_t ob = rb;
+                const float ov = racc;
+                rb = b[j];
+                racc = v[j];
+                b[j] = ob;  // CB_EMPTY the first time
+                v[j] = ov;
+            } else {
+                rcnt--;
             }
-            busy = (hitm | hotm) != 0;
         }
-        // A: claims of the cold pending elements and of the carried ones
-        const bool any1 = __any_sync(FULL_MASK, cb1 != BIN_NONE);
-        uint32_t o[4], oc0, oc1 = 0;
+        uint32_t t[NI];
 #pragma unroll
-        for (int j = 0; j < 4; j++) o[j] = table[b[j] & (CB_PART - 1)];
-        oc0 = table[cb0 & (CB_PART - 1)];
-        if (any1) oc1 = table[cb1 & (CB_PART - 1)];
+        for (int j = 0; j < NI; j++) t[j] = tg[b[j] & (CB_SLOTS - 1)];
+        uint32_t coldm = 0;  // bit j: pending and not resident in the warp's cache
+        uint32_t hotm = 0;   // bit j: pending and resident
 #pragma unroll
-        for (int j = 0; j < 4; j++)
-            if (b[j] != BIN_NONE && !(hotm >> j & 1u) && o[j] < CLAIM) table[b[j]] = myid + j;
-        if (cb0 != BIN_NONE && oc0 < CLAIM) table[cb0] = myid + 4;
-        if (any1 && cb1 != BIN_NONE && oc1 < CLAIM) table[cb1] = myid + 5;
+        for (int j = 0; j < NI; j++) {
+            // a valid tag never equals CB_EMPTY's, and b == CB_EMPTY matches no tag
+            const bool hot = (t[j] >> 2) == b[j] / CB_SLOTS;
+            const bool cold = !hot & (b[j] != CB_EMPTY);
+            hotm |= (uint32_t)hot << j;
+            coldm |= (uint32_t)cold << j;
+            if (hot & ((t[j] & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t[j] + 1;  // racing lanes store the same word
+            if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
+        }
         __syncthreads();  // B1
-        uint32_t c[4], cc0, cc1 = 0;
+        {
+            uint16_t c[NI];
+            float o[NI];
 #pragma unroll
-        for (int j = 0; j < 4; j++) c[j] = table[b[j] & (CB_PART - 1)];
-        cc0 = table[cb0 & (CB_PART - 1)];
-        if (any1) cc1 = table[cb1 & (CB_PART - 1)];
-        uint32_t coldm = 0;  // bit j: lost the claim round
+            for (int j = 0; j < NI; j++) {
+                c[j] = claimA[b[j] & (CB_PART - 1)];
+                o[j] = table[b[j] & (CB_PART - 1)];
+            }
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            if (b[j] == BIN_NONE || (hotm >> j & 1u)) continue;
-            if (c[j] == myid + j) {
-                table[b[j]] = __float_as_uint(OP::comb(__uint_as_float(o[j]), v[j], S));
-                b[j] = BIN_NONE;
-            } else {
-                coldm |= 1u << j;
+            for (int j = 0; j < NI; j++) {
+                const bool cold = coldm >> j & 1u;
+                const bool win = cold & (c[j] == (uint16_t)(id0 + j));
+                if (win) table[b[j]] = OP::comb(o[j], v[j], S);
+                coldm &= ~((uint32_t)win << j);
             }
         }
-        bool again0 = false, again1 = false;  // a carried element lost once more: its bin is contended
-        if (cb0 != BIN_NONE) {
-            if (cc0 == myid + 4) {
-                table[cb0] = __float_as_uint(OP::comb(__uint_as_float(oc0), cv0, S));
-                cb0 = BIN_NONE;
-            } else {
-                again0 = true;
+        __syncthreads();  // B2: the plain updates are done before any CAS touches the table
+        if (__any_sync(FULL_MASK, coldm != 0)) {
+#pragma unroll
+            for (int j = 0; j < NI; j++) {  // losers: ONE compare-and-swap; a failure means the bin is contended
+                if (coldm >> j & 1u) {
+                    unsigned *cell = reinterpret_cast<unsigned *>(table + b[j]);
+                    const unsigned old = *(volatile unsigned *)cell;
+                    const unsigned upd = __float_as_uint(OP::comb(__uint_as_float(old), v[j], S));
+                    if (atomicCAS(cell, old, upd) == old) coldm &= ~(1u << j);
+                }
             }
         }
-        if (any1 && cb1 != BIN_NONE) {
-            if (cc1 == myid + 5) {
-                table[cb1] = __float_as_uint(OP::comb(__uint_as_float(oc1), cv1, S));
-                cb1 = BIN_NONE;
-            } else {
-                again1 = true;
-            }
-        }
-        const int nbusy = __syncthreads_count(busy | (coldm != 0));  // B2
-        // C
         if (__any_sync(FULL_MASK, hotm != 0)) {
 #pragma unroll
-            for (int j = 0; j < 4; j++) {
-                const unsigned hm = __ballot_sync(FULL_MASK, hotm >> j & 1u);
-                if (hm == 0) continue;
-                // directory training: a bin that several lanes of this row hold in the warp cache
-                const uint32_t cand = __shfl_sync(FULL_MASK, b[j], __ffs(hm) - 1);
-                const int cn = __popc(__ballot_sync(FULL_MASK, (hotm >> j & 1u) && b[j] == cand));
-                if (cn >= 2) {
-                    uint32_t bb[1] = {(hotm >> j & 1u) ? b[j] : BIN_NONE};
-                    const float vv[1] = {v[j]};
-                    if (dir_train<ACC, 1>(d, cand, cn, hitm, bb, vv, lane, S, ndir, flush) && bb[0] == BIN_NONE &&
-                        (hotm >> j & 1u)) {
-                        hotm &= ~(1u << j);
-                        b[j] = BIN_NONE;
-                    }
-                }
-                // hits: the resident entry cannot change before the installs below
-                uint8_t *cbyte = cl + (b[j] & (CB_SLOTS - 1));
+            for (int j = 0; j < NI; j++) {  // hits: the resident entry cannot change before the installs below
+                uint8_t *c = cl + (b[j] & (CB_SLOTS - 1));
                 float *a = vl + (b[j] & (CB_SLOTS - 1));
                 bool pend = hotm >> j & 1u;
                 while (__any_sync(FULL_MASK, pend)) {
-                    if (pend) *cbyte = (uint8_t)lane;
+                    if (pend) *c = (uint8_t)lane;
                     __syncwarp();
-                    if (pend && *cbyte == lane) {
+                    if (pend && *c == lane) {
                         *a = OP::comb(*a, v[j], S);
                         pend = false;
                     }
@@ -1017,73 +1031,36 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 }
             }
         }
-        // carried elements that lost again sit in contended bins: in skew mode the warp cache takes them
-        // (installing the bin unless a hotter one guards the slot); evictions and bypasses (cold, rare)
-        // fall back to a compare-and-swap loop on the table
-        if (skew) {
-            if (__any_sync(FULL_MASK, again0)) {
-                uint32_t eb = 0;
-                float evv = 0.f;
-                if (claim_update_big<ACC>(again0, cb0, cv0, vl, tg, cl, S, lane, eb, evv)) smem_combine<ACC>(table + eb, evv, S);
-                if (again0) cb0 = BIN_NONE;
-            }
-            if (__any_sync(FULL_MASK, again1)) {
-                uint32_t eb = 0;
-                float evv = 0.f;
-                if (claim_update_big<ACC>(again1, cb1, cv1, vl, tg, cl, S, lane, eb, evv)) smem_combine<ACC>(table + eb, evv, S);
-                if (again1) cb1 = BIN_NONE;
-            }
-        }
-        // new losers: into a free carry slot; a thread that has none left (rare) updates the table directly
         if (__any_sync(FULL_MASK, coldm != 0)) {
 #pragma unroll
-            for (int j = 0; j < 4; j++) {
-                if (!(coldm >> j & 1u)) continue;
-                if (cb0 == BIN_NONE) { cb0 = b[j]; cv0 = v[j]; coldm &= ~(1u << j); }
-                else if (cb1 == BIN_NONE) { cb1 = b[j]; cv1 = v[j]; coldm &= ~(1u << j); }
-            }
-            if (__any_sync(FULL_MASK, coldm != 0)) {
-#pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    const bool act = coldm >> j & 1u;
-                    if (!__any_sync(FULL_MASK, act)) continue;
-                    if (skew) {
-                        uint32_t eb = 0;
-                        float evv = 0.f;
-                        if (claim_update_big<ACC>(act, b[j], v[j], vl, tg, cl, S, lane, eb, evv))
-                            smem_combine<ACC>(table + eb, evv, S);
-                    } else if (act) {
-                        smem_combine<ACC>(table + b[j], v[j], S);
-                    }
+            for (int j = 0; j < NI; j++) {
+                const bool act = coldm >> j & 1u;
+                if (__any_sync(FULL_MASK, act)) {
+                    uint32_t eb = 0;
+                    float evv = 0.f;
+                    if (claim_update_big<ACC>(act, b[j], v[j], vl, tg, cl, S, lane, eb, evv))
+                        smem_combine<ACC>(reinterpret_cast<uint32_t *>(table + eb), evv, S);
                 }
             }
         }
-        skew = skew ? nbusy >= CB_SKEW_OFF : nbusy > CB_SKEW_ON;
-        __syncthreads();  // B3
+        if (drain) break;
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
+        for (int j = 0; j < NI; j++) {
             k[j] = kn[j];
             v[j] = vn[j];
         }
         q0 = qn;
     }
-    if (cb0 != BIN_NONE) smem_combine<ACC>(table + cb0, cv0, S);  // the last carries
-    if (cb1 != BIN_NONE) smem_combine<ACC>(table + cb1, cv1, S);
-    for (int s = 0; s < DIR_S; s++) {  // write the directory back
-        const uint32_t bin = d.dir[s];
-        if (bin == DIR_EMPTY) continue;
-        const float x = warp_fold<ACC>(d.hot[s * 32 + lane], S);
-        if (lane == 0) flush(bin, x);
-    }
+    __syncthreads();
     for (int s = lane; s < CB_SLOTS; s += 32) {  // write the warp's cache back
         const uint32_t t = tg[s];
-        if (t != CB_EMPTY) smem_combine<ACC>(table + (t >> 2) * CB_SLOTS + s, vl[s], S);
+        if (t != CB_EMPTY) smem_combine<ACC>(reinterpret_cast<uint32_t *>(table + (t >> 2) * CB_SLOTS + s), vl[s], S);
     }
     __syncthreads();
     float *dst = part + (size_t)group * (size_t)w;
     for (int64_t i = threadIdx.x; i < CB_PART; i += CB_NT) {
         const int64_t bin = (i << cl_log2) + rank;
-        if (bin < w) dst[bin] = __uint_as_float(table[i]);
+        if (bin < w) dst[bin] = table[i];
     }
 }
 
@@ -1131,7 +1108,7 @@ static int cached_grid(int64_t n, int64_t w) {
     if (w <= CS_SLOTS) return grid_for(n < 1 ? 1 : n, CS_NT, CS_CTAS_PER_SM);
     const int c = cached_split_log2(w);
     const int64_t quads = ((n < 1 ? 1 : n) + 3) / 4;
-    int64_t groups = (quads + CB_NT - 1) / CB_NT;
+    int64_t groups = (quads + CB_NT * CB_U - 1) / (CB_NT * CB_U);
     const int64_t cap = NUM_SMS_B200 >> c > 0 ? NUM_SMS_B200 >> c : 1;
     if (groups > cap) groups = cap;
     return (int)(groups << c);
@@ -1157,7 +1134,7 @@ static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, 
             return VJP_ERR_CUDA;
         VJP_LAUNCH(K_CACHED_SMALL, stream) kern<<<G, CS_NT, CS_SMEM, stream>>>(n, w, is, vs, part, zeros, S);
     } else {
-        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS>;
+        auto kern = rbi_cached_big_kernel<ACC, COUNT_ZEROS, CB_U>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CB_SMEM) != cudaSuccess)
             return VJP_ERR_CUDA;
         VJP_LAUNCH(K_CACHED_BIG, stream) kern<<<G, CB_NT, CB_SMEM, stream>>>(n, w, cached_split_log2(w), is, vs, part, zeros, S);
@@ -1223,14 +1200,21 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         float v[4], o[4];
         const int cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
+        // the four coefficient gathers are issued together (clamped index, unconditional load): one L2 round
+        // trip per quad instead of four dependent ones (profiles/r2c: 32 long-scoreboard stall cycles per issue)
+        float2 c[4];
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            o[j] = 0.f;
-            if (!in_range(k[j], w)) continue;
-            const float2 c = SMEM ? sh[k[j]] : __ldg(coef + k[j]);
-            const int z = __float_as_int(c.y);
-            if (z == 0) o[j] = c.x / v[j];
-            else if (z == 1 && v[j] == 0.f) o[j] = c.x;
+            const int64_t kk = in_range(k[j], w) ? k[j] : 0;
+            c[j] = SMEM ? sh[kk] : __ldg(coef + kk);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const int z = __float_as_int(c[j].y);
+            float r = 0.f;
+            if (z == 0) r = c[j].x / v[j];
+            else if (z == 1 && v[j] == 0.f) r = c[j].x;
+            o[j] = in_range(k[j], w) ? r : 0.f;
         }
         store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
     }
