@@ -24,7 +24,6 @@ namespace vjp {
 // ------------------------------------------------------------------ packed look-back ------
 // word = status (bits 62-63) | payload (bits 0-32: value bits 0-31, segment flag bit 32)
 
-constexpr int PK_NT = 256;
 enum : uint64_t { PK_EMPTY = 0, PK_AGG = 1, PK_PREFIX = 2 };
 constexpr uint64_t PK_PAYLOAD = (1ull << 33) - 1;
 
@@ -365,32 +364,54 @@ constexpr int SEG_NT = 512;
 constexpr int SEG_IPT = 8;
 constexpr int SEG_TILE = SEG_NT * SEG_IPT;
 
+// A thread's row of RW consecutive 32-bit words straight from / to global memory with 128-bit accesses: the
+// row is 32 or 64 contiguous bytes, i.e. whole sectors, so nothing is gained by staging the tile through
+// shared memory -- and the barriers around the staging were what these kernels waited on (profiles/r2d:
+// 26 - 37 barrier stall cycles per issue, issue slots 12 - 19 % busy).  `valid` = words of the row that exist.
+template <int RW>
+VJP_DEVINL void load_row(const uint32_t *__restrict__ g, int valid, uint32_t fill, uint32_t (&r)[RW]) {
+    if (valid >= RW) {
+        const uint4 *g4 = reinterpret_cast<const uint4 *>(g);
+#pragma unroll
+        for (int c = 0; c < RW / 4; c++) {
+            const uint4 v = __ldg(g4 + c);
+            r[4 * c] = v.x; r[4 * c + 1] = v.y; r[4 * c + 2] = v.z; r[4 * c + 3] = v.w;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < RW; i++) r[i] = i < valid ? __ldg(g + i) : fill;
+    }
+}
+template <int RW>
+VJP_DEVINL void store_row(uint32_t *__restrict__ g, int valid, const uint32_t (&r)[RW]) {
+    if (valid >= RW) {
+        uint4 *g4 = reinterpret_cast<uint4 *>(g);
+#pragma unroll
+        for (int c = 0; c < RW / 4; c++) g4[c] = make_uint4(r[4 * c], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+    } else {
+#pragma unroll
+        for (int i = 0; i < RW; i++)
+            if (i < valid) g[i] = r[i];
+    }
+}
+
 // G4: ls[j] = fold of the same-key elements before j (neutral at a segment head).
 template <int CODE>
 __global__ void __launch_bounds__(SEG_NT)
 seg_forward_kernel(int64_t n, const uint32_t *__restrict__ keys, const uint2 *__restrict__ pay,
                    float *__restrict__ ls, GenOp<CODE> op, int *ticket, uint64_t *status) {
-    using KS = Stage<SEG_NT, SEG_IPT>;
-    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
-    extern __shared__ uint4 smem[];
-    uint4 *sk = smem;
-    uint4 *sp = smem + KS::SMEM_BYTES / 16;
     __shared__ uint64_t scratch[SEG_NT / 32 + 2];
     __shared__ uint32_t last_key[SEG_NT];
     __shared__ int s_p;
     if (threadIdx.x == 0) s_p = atomicAdd(ticket, 1);
     __syncthreads();
     const int p = s_p;
-    const int64_t base = (int64_t)p * SEG_TILE;
-    const int valid = (int)min((int64_t)SEG_TILE, n - base);
-    const uint32_t fillk[1] = {0xffffffffu};  // a key no element has: the padding is its own segment
-    const uint32_t fillp[1] = {0u};
-    KS::load(sk, keys + base, valid, fillk);
-    PS::load(sp, reinterpret_cast<const uint32_t *>(pay + base), 2 * valid, fillp);
-    __syncthreads();
+    const int64_t base = (int64_t)p * SEG_TILE + threadIdx.x * SEG_IPT;  // this thread's first element
+    const int mine = (int)max((int64_t)0, min((int64_t)SEG_IPT, n - base));  // elements of the row that exist
     uint32_t k[SEG_IPT], pw[2 * SEG_IPT];
-    KS::read_row(sk, threadIdx.x, k);
-    PS::read_row(sp, threadIdx.x, pw);
+    // padding: a key no element has (its own segment), value bits 0
+    load_row<SEG_IPT>(keys + base, mine, 0xffffffffu, k);
+    load_row<2 * SEG_IPT>(reinterpret_cast<const uint32_t *>(pay + base), 2 * mine, 0u, pw);
     last_key[threadIdx.x] = k[SEG_IPT - 1];
     __syncthreads();
     uint32_t prev;
@@ -424,10 +445,7 @@ seg_forward_kernel(int64_t n, const uint32_t *__restrict__ keys, const uint2 *__
         out[j] = __float_as_uint(l);
         run = op.apply(l, v);
     }
-    __syncthreads();  // every thread has read its key row
-    KS::write_row(sk, threadIdx.x, out);
-    __syncthreads();
-    KS::template store<float>(sk, reinterpret_cast<uint32_t *>(ls) + base, valid, false);
+    store_row<SEG_IPT>(reinterpret_cast<uint32_t *>(ls) + base, mine, out);
 }
 
 // G5-G7 fused: reverse segmented exclusive scan, per-element derivative, un-permute.
@@ -437,12 +455,6 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
                        const uint2 *__restrict__ pay, const float *__restrict__ ls,
                        const float *__restrict__ hist_bar, float *__restrict__ vs_bar,
                        GenOp<CODE> op, int num_tiles, int *ticket, uint64_t *status, int accumulate) {
-    using KS = Stage<SEG_NT, SEG_IPT>;
-    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
-    extern __shared__ uint4 smem[];
-    uint4 *sk = smem;
-    uint4 *sl = sk + KS::SMEM_BYTES / 16;
-    uint4 *sp = sl + KS::SMEM_BYTES / 16;
     __shared__ uint64_t scratch[SEG_NT / 32 + 2];
     __shared__ uint32_t first_key[SEG_NT];
     __shared__ int s_p;
@@ -450,24 +462,23 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
     __syncthreads();
     const int p = s_p;
     const int t = num_tiles - 1 - p;
-    const int64_t base = (int64_t)t * SEG_TILE;
-    const int valid = (int)min((int64_t)SEG_TILE, n - base);
-    const uint32_t fillk[1] = {0xffffffffu};
-    const uint32_t fill0[1] = {0u};
-    KS::load(sk, keys + base, valid, fillk);
-    KS::load(sl, reinterpret_cast<const uint32_t *>(ls) + base, valid, fill0);
-    PS::load(sp, reinterpret_cast<const uint32_t *>(pay + base), 2 * valid, fill0);
-    __syncthreads();
+    const int64_t tbase = (int64_t)t * SEG_TILE;
+    const int64_t base = tbase + threadIdx.x * SEG_IPT;
+    const int mine = (int)max((int64_t)0, min((int64_t)SEG_IPT, n - base));  // number of real elements in this row
     uint32_t k[SEG_IPT], lw[SEG_IPT], pw[2 * SEG_IPT];
-    KS::read_row(sk, threadIdx.x, k);
-    KS::read_row(sl, threadIdx.x, lw);
-    PS::read_row(sp, threadIdx.x, pw);
+    load_row<SEG_IPT>(keys + base, mine, 0xffffffffu, k);
+    load_row<SEG_IPT>(reinterpret_cast<const uint32_t *>(ls) + base, mine, 0u, lw);
+    load_row<2 * SEG_IPT>(reinterpret_cast<const uint32_t *>(pay + base), 2 * mine, 0u, pw);
+    // the bin adjoints of the row: issued now, consumed after the scan
+    float hb[SEG_IPT];
+#pragma unroll
+    for (int j = 0; j < SEG_IPT; j++) hb[j] = k[j] < (uint32_t)w ? __ldg(hist_bar + k[j]) : 0.f;
     first_key[threadIdx.x] = k[0];
     __syncthreads();
     uint32_t next;
     bool last_tail = false;
     if (threadIdx.x < SEG_NT - 1) next = first_key[threadIdx.x + 1];
-    else if (base + SEG_TILE < n) next = __ldg(keys + base + SEG_TILE);
+    else if (tbase + SEG_TILE < n) next = __ldg(keys + tbase + SEG_TILE);
     else { next = 0; last_tail = true; }
 
     const SegComb<CODE, true> comb{op};
@@ -487,16 +498,14 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
     }
     __syncthreads();
     float run = __uint_as_float((uint32_t)comb(scratch[SEG_NT / 32 + 1], ex));
-    const int mine = valid - threadIdx.x * SEG_IPT;  // number of real elements in this row
 #pragma unroll
     for (int j = SEG_IPT - 1; j >= 0; j--) {
         const float v = __uint_as_float(pw[2 * j + 1]);
         const float r = tail[j] ? op.neutral() : run;
         run = op.apply(v, r);
         if (j < mine) {
-            float g = 0.f;
-            if (k[j] < (uint32_t)w)  // out-of-range keys were clamped to w: adjoint 0
-                g = op.dfdx(__uint_as_float(lw[j]), v, r) * __ldg(hist_bar + k[j]);
+            // out-of-range keys were clamped to w: adjoint 0 (hb is 0 there)
+            const float g = k[j] < (uint32_t)w ? op.dfdx(__uint_as_float(lw[j]), v, r) * hb[j] : 0.f;
             vs_bar[pw[2 * j]] = accumulate ? vs_bar[pw[2 * j]] + g : g;  // the permutation names every index once
         }
     }
@@ -600,16 +609,9 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
     int buf;
     int rc = run_sort(n, w, is, vs, g, &buf, stream);
     if (rc != VJP_OK) return rc;
-    using KS = Stage<SEG_NT, SEG_IPT>;
-    using PS = Stage<SEG_NT, 2 * SEG_IPT>;
     const GenOp<CODE> op{S};
     const int nt = (int)seg_tiles(n);
-    constexpr size_t FWD_SMEM = KS::SMEM_BYTES + PS::SMEM_BYTES, REV_SMEM = 2 * KS::SMEM_BYTES + PS::SMEM_BYTES;
-    if ((FWD_SMEM > 48 * 1024 &&
-         cudaFuncSetAttribute(seg_forward_kernel<CODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FWD_SMEM) != cudaSuccess) ||
-        (REV_SMEM > 48 * 1024 &&
-         cudaFuncSetAttribute(seg_reverse_vjp_kernel<CODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)REV_SMEM) != cudaSuccess))
-        return VJP_ERR_CUDA;
+    constexpr size_t FWD_SMEM = 0, REV_SMEM = 0;
     if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
     VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, FWD_SMEM, stream>>>(
         n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
