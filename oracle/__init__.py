@@ -163,3 +163,42 @@ def rbi_sort_perm(num_bins, is_):
     _check(_load().orc_rbi_sort_perm(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(sk),
                                      _p(perm)), "rbi_sort_perm")
     return sk, perm
+
+
+# ------------------------------------------------------------------ reduce (section 3) ----
+
+def reduce_forward(op, xs, S: float = 0.0):
+    """y = reduce (.) e xs; the neutral element for an empty array."""
+    op = _opcode(op)
+    xs = _f64(xs)
+    y = ctypes.c_double(0.0)
+    _check(_load().orc_reduce_forward(op, ctypes.c_double(S), ctypes.c_int64(xs.size), _p(xs), ctypes.byref(y)),
+           "reduce_forward")
+    return y.value
+
+
+def vjp_reduce_general(op, xs, y_bar, S: float = 0.0, with_lr: bool = False):
+    """General rule, eq. 2 with the two exclusive scans of Fig. 2.  Returns xs_bar or (xs_bar, ls, rs)."""
+    op = _opcode(op)
+    xs = _f64(xs)
+    n = xs.size
+    xs_bar = np.empty(n, dtype=np.float64)
+    ls = np.empty(n, dtype=np.float64) if with_lr else None
+    rs = np.empty(n, dtype=np.float64) if with_lr else None
+    _check(_load().orc_reduce_vjp_general(op, ctypes.c_double(S), ctypes.c_int64(n), _p(xs),
+                                          ctypes.c_double(float(y_bar)), _p(xs_bar), _p(ls), _p(rs)),
+           "reduce_vjp_general")
+    return (xs_bar, ls, rs) if with_lr else xs_bar
+
+
+def vjp_reduce(op, xs, y_bar):
+    """Specialised rules of section 3.2 ('+', min, max, '*').  Returns (xs_bar, aux_i, aux_v): aux = (k, extremum)
+    for min/max, (number of zeros, product of the non-zeros) for '*', (0, 0.0) for '+'."""
+    op = _opcode(op)
+    xs = _f64(xs)
+    n = xs.size
+    xs_bar = np.empty(n, dtype=np.float64)
+    ai, av = ctypes.c_int64(0), ctypes.c_double(0.0)
+    _check(_load().orc_reduce_vjp(op, ctypes.c_int64(n), _p(xs), ctypes.c_double(float(y_bar)), _p(xs_bar),
+                                  ctypes.byref(ai), ctypes.byref(av)), "reduce_vjp")
+    return xs_bar, ai.value, av.value

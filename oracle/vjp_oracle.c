@@ -18,7 +18,10 @@
  *                       attaining the extremum, '*' as l_i * r_i
  *                        -- the plain definition, no zero-count trick;
  *   - general rule:     eq. 5 literally, l_i / r_i by per-bin forward / backward
- *                       folds (the radix sort of Fig. 4 is only a way to find them).
+ *                       folds (the radix sort of Fig. 4 is only a way to find them);
+ *   - reduce:           the sequential fold, eq. 2 with the two
+ *                       exclusive scans of Fig. 2, and the specialised rules of section 3.2
+ *                       as their plain definitions (added in round 2, before the kernels).
  * Parity pins: tests/test_oracle_pins.py (closed forms, finite differences, brute-force
  * dense Jacobian transposes, dot-product test, PPAD's rule of Fig. 11, hand-worked
  * fixtures under tests/golden/).  No function here is "parity unpinned".
@@ -362,4 +365,92 @@ int orc_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_k
     }
     free(start);
     return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ reduce (section 3) --
+ *
+ * y = reduce (.) e as = a_0 (.) a_1 (.) ... (.) a_{n-1}.  Same operator set as
+ * reduce_by_index ('+', '*', min, max, satadd); a reduce is a reduce_by_index with one bin. */
+
+/* The sequential fold of P:L122-124; the neutral element for n = 0. */
+int orc_reduce_forward(int op, double S, int64_t n, const double *xs, double *y) {
+    if (!rbi_op_ok(op) || n < 0) return ORC_EINVAL;
+    double acc = rbi_neutral(op);
+    for (int64_t i = 0; i < n; i++) acc = rbi_apply(op, S, acc, xs[i]);
+    *y = acc;
+    return ORC_OK;
+}
+
+/* General rule, eq. 2 with Fig. 2:
+ *   ls = scan^exc (.) e as                 (forward exclusive scan)
+ *   rs = reverse (scan^exc (\x y -> y (.) x) e (reverse as))
+ *   as_bar[i] = d(l_i (.) a_i (.) r_i)/d a_i * y_bar
+ * ls_out / rs_out may be NULL. */
+int orc_reduce_vjp_general(int op, double S, int64_t n, const double *xs, double y_bar,
+                           double *xs_bar, double *ls_out, double *rs_out) {
+    if (!rbi_op_ok(op) || n < 0) return ORC_EINVAL;
+    double *l = (double *)malloc((size_t)(n > 0 ? n : 1) * sizeof(double));
+    if (!l) return ORC_ENOMEM;
+    double acc = rbi_neutral(op);
+    for (int64_t i = 0; i < n; i++) { l[i] = acc; acc = rbi_apply(op, S, acc, xs[i]); }
+    acc = rbi_neutral(op);
+    for (int64_t i = n - 1; i >= 0; i--) {
+        double r = acc;
+        xs_bar[i] = general_dfdx(op, S, l[i], xs[i], r) * y_bar;
+        if (ls_out) ls_out[i] = l[i];
+        if (rs_out) rs_out[i] = r;
+        acc = rbi_apply(op, S, xs[i], r); /* y (.) x of P:L148: the element on the left */
+    }
+    free(l);
+    return ORC_OK;
+}
+
+/* Specialised rules of section 3.2, each as its plain definition:
+ *   '+'  as_bar = replicate n y_bar
+ *   min/max  (k, y) = the extremum and the SMALLEST index attaining
+ *           it ("in case of duplicates we choose the smallest index"); as_bar = 0 except
+ *           as_bar[k] = y_bar.  n = 0: k = n, y = +-inf, nothing is written.
+ *   '*'  as_bar[i] = l_i * r_i * y_bar -- no zero counting, no division;
+ *           the lifted primal's (n^{=0}, y^{>0}) of Fig. 3 is computed
+ *           separately for the bit-exact comparison of the count.
+ * aux_i (may be NULL): k for min/max, n^{=0} for '*'.  aux_v (may be NULL): the extremum for
+ * min/max, y^{>0} for '*'. */
+int orc_reduce_vjp(int op, int64_t n, const double *xs, double y_bar, double *xs_bar,
+                   int64_t *aux_i, double *aux_v) {
+    if (n < 0) return ORC_EINVAL;
+    switch (op) {
+    case ORC_ADD:
+        for (int64_t i = 0; i < n; i++) xs_bar[i] = y_bar;
+        return ORC_OK;
+    case ORC_MIN:
+    case ORC_MAX: {
+        int64_t k = n;
+        double e = rbi_neutral(op);
+        for (int64_t i = 0; i < n; i++) {
+            int better = (op == ORC_MIN) ? (xs[i] < e) : (xs[i] > e);
+            if (k == n || better) { k = i; e = xs[i]; } /* min^L((n,inf),(i,v)): P:L184 */
+        }
+        for (int64_t i = 0; i < n; i++) xs_bar[i] = 0.0;
+        if (k < n) xs_bar[k] = y_bar;
+        if (aux_i) *aux_i = k;
+        if (aux_v) *aux_v = e;
+        return ORC_OK;
+    }
+    case ORC_MUL: {
+        double *l = (double *)malloc((size_t)(n > 0 ? n : 1) * sizeof(double));
+        if (!l) return ORC_ENOMEM;
+        double acc = 1.0;
+        for (int64_t i = 0; i < n; i++) { l[i] = acc; acc *= xs[i]; }
+        acc = 1.0;
+        for (int64_t i = n - 1; i >= 0; i--) { xs_bar[i] = (l[i] * acc) * y_bar; acc *= xs[i]; }
+        free(l);
+        int64_t z = 0;
+        double p = 1.0;
+        for (int64_t i = 0; i < n; i++) { if (xs[i] == 0.0) z++; else p *= xs[i]; }
+        if (aux_i) *aux_i = z;
+        if (aux_v) *aux_v = p;
+        return ORC_OK;
+    }
+    default: return ORC_EINVAL;
+    }
 }
