@@ -176,6 +176,37 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
                   int64_t *perm, void *ws, size_t ws_bytes, void *stream);
 
+/* ----------------------------------------------------------------------------- reduce ----- */
+
+/* reduce (section 3 of the paper): y = a_0 (.) a_1 (.) ... (.) a_{n-1}, one scalar.
+ * y, y_bar point to ONE scalar of op.dtype in DEVICE memory (naturally aligned is enough).
+ * Operators: ADD (f32, f64), MIN, MAX, MUL, SATADD (f32).  n < 2^32 - 1. */
+size_t vjp_reduce_workspace_bytes(const vjp_op_t *op, int64_t n);
+
+/* Primal y = reduce (.) e xs; n == 0 gives the neutral element.  Two-level tree
+ * reduction (one partial per CTA, folded in a fixed order: deterministic). */
+int reduce_forward(const vjp_op_t *op, int64_t n, const void *xs, void *y, void *ws, size_t ws_bytes,
+                   void *stream);
+
+/* Input adjoints xs_bar[n] of reduce, given y_bar.
+ *   ADD:     xs_bar = replicate n y_bar; xs may be NULL.
+ *   MIN/MAX: lifted primal (k, y) with the smallest index on ties, then xs_bar = 0 and
+ *            xs_bar[k] = y_bar.  Bit-exact copy.
+ *   MUL:     lifted primal (number of zeros, product of the non-zeros), then the three-way map of
+ *            Fig. 3.
+ *   SATADD or force_general: the general rule, eq. 2 -- forward and reverse exclusive
+ *            scans l_i, r_i (Fig. 2), xs_bar_i = d(l_i (.) x_i (.) r_i)/dx_i * y_bar;
+ *            runs the segmented-scan kernels of the reduce-by-index general rule with one segment.
+ * op.accumulate adds to xs_bar ("as_bar +="). */
+int vjp_reduce(const vjp_op_t *op, int64_t n, const void *xs, const void *y_bar, void *xs_bar,
+               void *ws, size_t ws_bytes, void *stream);
+
+/* Inspection: the lifted primal's integer and value (device scalars), for bit-exact comparison.
+ *   MIN/MAX: *aux_i = k (n for an empty array), *aux_v = the extremum (f32).
+ *   MUL:     *aux_i = number of zeros (IEEE equality, Q7), *aux_v = product of the non-zeros. */
+int reduce_lifted(const vjp_op_t *op, int64_t n, const void *xs, int64_t *aux_i, void *aux_v,
+                  void *ws, size_t ws_bytes, void *stream);
+
 /* ------------------------------------------------------------------ instrumentation ----- */
 
 /* The library's kernels are numbered 0 .. vjp_kernel_count()-1; vjp_kernel_name gives the kernel's

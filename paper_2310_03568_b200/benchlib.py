@@ -161,10 +161,12 @@ C2_CELLS = [(op, w, dist) for op in ("min", "mul") for w in (1 << 10, 1 << 16) f
 VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (roofline table)
     "c1_rbi_add": 12, "c2_rbi_min": 16, "c2_rbi_mul": 28, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 32,
     "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
+    "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
     "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4,
 }
 
 
@@ -228,6 +230,22 @@ class ScanCase:
         return B.scan_forward(self.op, self.xs, out=self.out, ws=self.ws)
 
 
+class ReduceCase:
+    """NEXT row f2: one reduce VJP problem (section 3 of the paper) resident on the device."""
+
+    def __init__(self, op: B.Op, d):
+        self.op, self.n = op, int(d["n"])
+        self.xs, self.yb = to_dev(d["xs"]), to_dev(d["y_bar"])
+        self.out = torch.empty(self.n, dtype=op.torch_dtype, device="cuda")
+        self.ws = torch.empty(max(256, B.vjp_reduce_workspace_bytes(op, self.n)), dtype=torch.uint8, device="cuda")
+
+    def vjp(self):
+        return B.vjp_reduce(self.op, self.xs, self.yb, out=self.out, ws=self.ws)
+
+    def primal(self):
+        return B.reduce_forward(self.op, self.xs, ws=self.ws)
+
+
 def measure_case(key, label, case, reps, peak_gbs):
     """VJP and primal timings of one case (median over reps, CUDA events)."""
     tv = statistics.median(event_time_ms(case.vjp, reps))
@@ -284,6 +302,9 @@ def case_table(scale=1.0):
         ("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
          rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])))),
     ]
+    for opname in ("add", "min", "mul"):  # NEXT row f2 (not a BASELINE config): reduce VJP, n = 2^24
+        t.append(("f2_reduce_" + opname, "f2 reduce %s f32 n=2^24 (NEXT row)" % opname,
+                  lambda opname=opname: ReduceCase(B.Op.of(opname), W.f2_reduce(opname, n=sz(1 << 24)))))
     return t
 
 

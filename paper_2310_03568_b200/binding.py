@@ -28,6 +28,7 @@ EXPORTS = [
     "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_reduce_by_index_workspace_bytes",
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
     "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
+    "vjp_reduce_workspace_bytes", "reduce_forward", "vjp_reduce", "reduce_lifted",
     "vjp_kernel_count", "vjp_kernel_name", "vjp_launch_count", "vjp_profile_enable", "vjp_profile_read",
 ]
 
@@ -97,6 +98,10 @@ def load() -> ctypes.CDLL:
         "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_workspace_bytes": (sz, [opp, i64]),
+        "reduce_forward": (ctypes.c_int, [opp, i64, vp, vp, vp, sz, vp]),
+        "vjp_reduce": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
+        "reduce_lifted": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_kernel_count": (ctypes.c_int, []),
         "vjp_kernel_name": (ctypes.c_char_p, [ctypes.c_int]),
         "vjp_launch_count": (i64, [ctypes.c_int]),
@@ -345,6 +350,56 @@ def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm
+
+
+# ------------------------------------------------------------------ reduce ---------------
+
+def vjp_reduce_workspace_bytes(op: Op, n: int) -> int:
+    o = op.c()
+    return load().vjp_reduce_workspace_bytes(ctypes.byref(o), n)
+
+
+def reduce_forward(op: Op, xs: torch.Tensor, ws=None, stream=None) -> torch.Tensor:
+    """y = reduce (.) e xs as a 1-element device tensor."""
+    xs = _dev(xs, op.torch_dtype, what="xs")
+    n = xs.numel()
+    y = torch.empty(1, dtype=op.torch_dtype, device=xs.device)
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n), xs.device, ws)
+    o = op.c()
+    _check(load().reduce_forward(ctypes.byref(o), n, _ptr(xs), _ptr(y), _ptr(ws), ws.numel(), _stream(stream)),
+           "reduce_forward")
+    return y
+
+
+def vjp_reduce(op: Op, xs, y_bar: torch.Tensor, n=None, out=None, ws=None, stream=None) -> torch.Tensor:
+    """xs_bar of reduce given the 1-element device tensor y_bar (section 3).  xs may be None for '+' (pass n)."""
+    y_bar = _dev(y_bar, op.torch_dtype, 1, "y_bar")
+    if xs is not None:
+        xs = _dev(xs, op.torch_dtype, what="xs")
+        n = xs.numel()
+    if n is None:
+        raise VjpError("n is required when xs is None")
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    xs_bar = _out(out, op.torch_dtype, n, y_bar.device, "xs_bar")
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n), y_bar.device, ws)
+    o = op.c()
+    _check(load().vjp_reduce(ctypes.byref(o), n, _ptr(xs), _ptr(y_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
+                             _stream(stream)), "vjp_reduce")
+    return xs_bar
+
+
+def reduce_lifted(op: Op, xs: torch.Tensor, ws=None, stream=None):
+    """(aux_i, aux_v) of the lifted primal: (k, extremum) for min/max, (zeros, product of non-zeros) for '*'."""
+    xs = _dev(xs, torch.float32, what="xs")
+    n = xs.numel()
+    ai = torch.empty(1, dtype=torch.int64, device=xs.device)
+    av = torch.empty(1, dtype=torch.float32, device=xs.device)
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n), xs.device, ws)
+    o = op.c()
+    _check(load().reduce_lifted(ctypes.byref(o), n, _ptr(xs), _ptr(ai), _ptr(av), _ptr(ws), ws.numel(),
+                                _stream(stream)), "reduce_lifted")
+    return ai, av
 
 
 # ------------------------------------------------------------------ instrumentation ------

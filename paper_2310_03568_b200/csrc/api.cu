@@ -57,7 +57,8 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "rbi_minmax_lifted_kernel", "rbi_minmax_finish_kernel", "rbi_cached_small_kernel", "rbi_cached_big_kernel",
     "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
-    "seg_reverse_vjp_kernel", "sort_export_kernel"};
+    "seg_reverse_vjp_kernel", "sort_export_kernel",
+    "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];
@@ -343,6 +344,75 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
         return VJP_ERR_WORKSPACE;
     return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs), nullptr, nullptr, zeros,
                           static_cast<float *>(prod_nz), ws, 0, as_stream(stream));
+}
+
+// ------------------------------------------------------------------------------ reduce ----
+
+namespace {
+// Which route a reduce operator takes: 0 none, 1 specialised, 2 general (two exclusive scans).
+int reduce_route(const vjp_op_t *op) {
+    const bool f32 = op->dtype == VJP_F32;
+    switch (op->code) {
+    case VJP_OP_ADD: return op->force_general ? (f32 ? 2 : 0) : 1;
+    case VJP_OP_MIN:
+    case VJP_OP_MAX:
+    case VJP_OP_MUL: return f32 ? (op->force_general ? 2 : 1) : 0;
+    case VJP_OP_SATADD: return f32 ? 2 : 0;
+    default: return 0;
+    }
+}
+}  // namespace
+
+size_t vjp_reduce_workspace_bytes(const vjp_op_t *op, int64_t n) {
+    if (!op_ok(op) || n < 0) return 0;
+    switch (reduce_route(op)) {
+    case 1: return reduce_special_workspace_bytes();
+    case 2: {
+        const size_t a = rbi_general_workspace_bytes(n, 1), b = reduce_special_workspace_bytes();
+        return a > b ? a : b;
+    }
+    default: return 0;
+    }
+}
+
+int reduce_forward(const vjp_op_t *op, int64_t n, const void *xs, void *y, void *ws, size_t ws_bytes,
+                   void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (reduce_route(op) == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (!y || !ws || (n > 0 && !xs) || !all_aligned(xs, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < reduce_special_workspace_bytes()) return VJP_ERR_WORKSPACE;
+    // n == 0 runs too (an empty grid-stride loop): y = the neutral element
+    return launch_reduce_forward(op->code, op->dtype, op->param, n, xs, y, nullptr, nullptr, 0, ws, as_stream(stream));
+}
+
+int reduce_lifted(const vjp_op_t *op, int64_t n, const void *xs, int64_t *aux_i, void *aux_v, void *ws,
+                  size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if ((op->code != VJP_OP_MIN && op->code != VJP_OP_MAX && op->code != VJP_OP_MUL) || op->dtype != VJP_F32)
+        return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (!aux_i || !aux_v || !ws || (n > 0 && !xs) || !all_aligned(xs, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < reduce_special_workspace_bytes()) return VJP_ERR_WORKSPACE;
+    return launch_reduce_forward(op->code, op->dtype, op->param, n, xs, nullptr, aux_i, aux_v, 1, ws, as_stream(stream));
+}
+
+int vjp_reduce(const vjp_op_t *op, int64_t n, const void *xs, const void *y_bar, void *xs_bar, void *ws,
+               size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    const int route = reduce_route(op);
+    if (route == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    const bool needs_xs = route == 2 || op->code != VJP_OP_ADD;
+    if (!y_bar || !xs_bar || !ws || (needs_xs && !xs)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(xs, xs_bar, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < vjp_reduce_workspace_bytes(op, n)) return VJP_ERR_WORKSPACE;
+    if (route == 1)
+        return launch_reduce_vjp(op->code, op->dtype, n, xs, y_bar, xs_bar, ws, op->accumulate != 0, as_stream(stream));
+    return launch_reduce_general_vjp(op->code, op->param, n, static_cast<const float *>(xs),
+                                     static_cast<const float *>(y_bar), static_cast<float *>(xs_bar), ws,
+                                     op->accumulate != 0, as_stream(stream));
 }
 
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,

@@ -28,6 +28,7 @@ enum KernelId : int {
     K_RBI_FILL, K_RBI_FORWARD, K_RBI_GATHER,
     K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
+    K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -72,5 +73,15 @@ int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const i
                            int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
                          int64_t *perm, void *ws, cudaStream_t stream);
+
+// ----------------------------------------------------------------------------- reduce ---
+size_t reduce_special_workspace_bytes();
+// primal (lift = 0: y) or lifted primal (lift = 1: aux_i / aux_v of min, max, '*'); n >= 1
+int launch_reduce_forward(int code, int dtype, double param, int64_t n, const void *xs, void *y,
+                          int64_t *aux_i, void *aux_v, int lift, void *ws, cudaStream_t stream);
+int launch_reduce_vjp(int code, int dtype, int64_t n, const void *xs, const void *y_bar, void *xs_bar,
+                      void *ws, int accumulate, cudaStream_t stream);
+int launch_reduce_general_vjp(int code, double param, int64_t n, const float *xs, const float *y_bar,
+                              float *xs_bar, void *ws, int accumulate, cudaStream_t stream);
 
 }  // namespace vjp

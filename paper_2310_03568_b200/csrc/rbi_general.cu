@@ -603,22 +603,56 @@ static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, co
     return last_launch_status();
 }
 
+// G3-G7 on sorted (key, (index, value)) arrays: forward segmented scan, fused reverse scan + derivative + scatter.
+template <int CODE>
+static int run_segscans(float S, int64_t n, int64_t w, const uint32_t *keys, const uint2 *pay,
+                        const float *hist_bar, float *vs_bar, const GenWs &g, int accumulate, cudaStream_t stream) {
+    const GenOp<CODE> op{S};
+    const int nt = (int)seg_tiles(n);
+    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, 0, stream>>>(
+        n, keys, pay, g.ls, op, g.ticket, g.status);
+    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
+    VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, 0, stream>>>(
+        n, w, keys, pay, g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status, accumulate);
+    return last_launch_status();
+}
+
 template <int CODE>
 static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
                        const float *hist_bar, float *vs_bar, const GenWs &g, int accumulate, cudaStream_t stream) {
     int buf;
     int rc = run_sort(n, w, is, vs, g, &buf, stream);
     if (rc != VJP_OK) return rc;
-    const GenOp<CODE> op{S};
-    const int nt = (int)seg_tiles(n);
-    constexpr size_t FWD_SMEM = 0, REV_SMEM = 0;
-    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_SEG_FORWARD, stream) seg_forward_kernel<CODE><<<nt, SEG_NT, FWD_SMEM, stream>>>(
-        n, g.key[buf], g.pay[buf], g.ls, op, g.ticket, g.status);
-    if (cudaMemsetAsync(g.ticket, 0, g.zero_bytes, stream) != cudaSuccess) return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_SEG_REVERSE, stream) seg_reverse_vjp_kernel<CODE><<<nt, SEG_NT, REV_SMEM, stream>>>(
-        n, w, g.key[buf], g.pay[buf], g.ls, hist_bar, vs_bar, op, nt, g.ticket, g.status, accumulate);
-    return last_launch_status();
+    return run_segscans<CODE>(S, n, w, g.key[buf], g.pay[buf], hist_bar, vs_bar, g, accumulate, stream);
+}
+
+// reduce, general rule (eq. 2; Fig. 2): ls = forward exclusive scan, rs = reverse exclusive
+// scan, as_bar_i = d(l_i (.) a_i (.) r_i)/da_i * y_bar -- the segmented-scan pair above with ONE segment
+// (every key 0, the identity permutation as payload index) and no sort; y_bar plays hist_bar[0].
+__global__ void reduce_pack_kernel(int64_t n, const float *__restrict__ xs, uint32_t *__restrict__ keys,
+                                   uint2 *__restrict__ pay) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        keys[i] = 0u;
+        pay[i] = make_uint2((uint32_t)i, __float_as_uint(__ldg(xs + i)));
+    }
+}
+
+int launch_reduce_general_vjp(int code, double param, int64_t n, const float *xs, const float *y_bar,
+                              float *xs_bar, void *ws, int accumulate, cudaStream_t stream) {
+    if (n == 0) return VJP_OK;
+    const GenWs g = gen_carve(ws, n);
+    const float S = (float)param;
+    const int grid = (int)((n + 255) / 256 < 2368 ? (n + 255) / 256 : 2368);
+    VJP_LAUNCH(K_REDUCE_PACK, stream) reduce_pack_kernel<<<grid, 256, 0, stream>>>(n, xs, g.key[0], g.pay[0]);
+    switch (code) {
+    case VJP_OP_ADD: return run_segscans<G_ADD>(S, n, 1, g.key[0], g.pay[0], y_bar, xs_bar, g, accumulate, stream);
+    case VJP_OP_MIN: return run_segscans<G_MIN>(S, n, 1, g.key[0], g.pay[0], y_bar, xs_bar, g, accumulate, stream);
+    case VJP_OP_MAX: return run_segscans<G_MAX>(S, n, 1, g.key[0], g.pay[0], y_bar, xs_bar, g, accumulate, stream);
+    case VJP_OP_MUL: return run_segscans<G_MUL>(S, n, 1, g.key[0], g.pay[0], y_bar, xs_bar, g, accumulate, stream);
+    case VJP_OP_SATADD: return run_segscans<G_SATADD>(S, n, 1, g.key[0], g.pay[0], y_bar, xs_bar, g, accumulate, stream);
+    default: return VJP_ERR_UNSUPPORTED;
+    }
 }
 
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,

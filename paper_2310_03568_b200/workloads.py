@@ -169,3 +169,26 @@ def c5_rbi_satadd(n=FULL["c5"]["n"], w=FULL["c5"]["w"], S=None, seed=0, margin=2
             i = first[k]
             vs[i] = np.float32(vs[i] + 4 * margin) if vs[i] < 0.5 else np.float32(vs[i] - 4 * margin)
     return dict(n=n, w=w, S=float(S), is_=is_, vs=vs, hist_bar=_normal_f32(_rng(seed, 5, 2), w))
+
+
+def f2_reduce(op, n=1 << 24, seed=0):
+    """NEXT row f2 (reduce VJP, section 3): one array per operator, shaped like config 2's values.  '+', min, max:
+    N(0,1) with 1 % duplicated values (ties); '*': U[1-2e-3, 1+2e-3] (the product of 2^24 of them stays inside f32)
+    with exact zeros at rate `1/n` scale chosen by the caller; satadd: U[0,1) with S = n/2 +- a margin."""
+    rng = _rng(seed, 6, {"add": 0, "min": 1, "max": 2, "mul": 3, "satadd": 4}[op])
+    if op == "mul":
+        xs = (1.0 + 2e-3 * (2.0 * rng.random(n) - 1.0)).astype(np.float32)
+    elif op == "satadd":
+        xs = rng.random(n, dtype=np.float32)
+    else:
+        xs = _normal_f32(rng, n)
+        if n >= 2 and op in ("min", "max"):
+            dup = rng.random(n) < 0.01
+            dup[0] = False
+            idx = np.flatnonzero(dup)
+            xs[idx] = xs[idx - 1]
+            ext = np.float32(-9.0 if op == "min" else 9.0)       # the extremum itself is tied (lowest index must win)
+            for pos in (n // 3, n // 2, n - 1):
+                xs[pos] = ext
+    y_bar = np.asarray(_rng(seed, 6, 9).standard_normal(1), dtype=np.float32)
+    return dict(n=n, xs=xs, y_bar=y_bar)
