@@ -259,6 +259,16 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     FS ftotal;
     const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
 
+    // The forward prefixes r_{i-1} of the thread's elements depend only on fpre[t] and fex, not on the reverse
+    // look-back: they are computed BEFORE the barrier that waits for warp 0, so that warps 1 .. N-1 work (and
+    // the fpre load is in flight) while warp 0 walks back.
+    FS rp[WIDE ? 1 : IPT];
+    rp[0] = Op::combine(load_state_cg(fpre + t), fex);
+    if constexpr (!WIDE) {
+#pragma unroll
+        for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
+    }
+
     if (threadIdx.x < 32) {
         RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
         __syncwarp();
@@ -277,19 +287,14 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
             u = Op::adj_mul(rbar, Op::lin_of(Op::from_elem(rx + j * EW)));
             Op::adj_to_elem(rbar, ry + j * EW);
         }
-        FS rp = Op::combine(load_state_cg(fpre + t), fex);
+        FS run = rp[0];
 #pragma unroll 1
         for (int j = 0; j < IPT; j++) {
             const Adj rbar = Op::adj_from_elem(ry + j * EW);
-            Op::xbar(rp, rbar, ry + j * EW);
-            if (j + 1 < IPT) rp = Op::combine(rp, Op::from_elem(rx + j * EW));
+            Op::xbar(run, rbar, ry + j * EW);
+            if (j + 1 < IPT) run = Op::combine(run, Op::from_elem(rx + j * EW));
         }
     } else {
-        // forward prefixes r_{i-1} of the thread's elements
-        FS rp[IPT];
-        rp[0] = Op::combine(load_state_cg(fpre + t), fex);
-#pragma unroll
-        for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
 #pragma unroll
         for (int j = IPT - 1; j >= 0; j--) {
             const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);

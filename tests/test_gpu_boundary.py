@@ -236,3 +236,66 @@ def test_lookback_stress_200_repetitions(name, tiles):
         assert err == err, "NaN left in the output"
         worst = max(worst, err / den)
     assert worst <= 1e-4
+
+
+# ------------------------------------------------------------------ canary guards ------------
+# compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md), so out-of-bounds WRITES are looked
+# for directly: every output and workspace sits between two guard bands filled with a canary pattern, at the
+# exact size the library asked for, and the bands must come back untouched.
+
+GUARD = 4096  # bytes on either side
+
+
+def guarded(nbytes, fill=0xA5):
+    """(payload view, check()) -- a 16-byte aligned payload of nbytes between two canary bands."""
+    pad = (-nbytes) % 16
+    buf = torch.full((GUARD + nbytes + pad + GUARD,), fill, dtype=torch.uint8, device="cuda")
+    payload = buf[GUARD:GUARD + nbytes]
+
+    def check():
+        torch.cuda.synchronize()
+        assert bool((buf[:GUARD] == fill).all()) and bool((buf[GUARD + nbytes:] == fill).all()), "guard band overwritten"
+    return payload, check
+
+
+@pytest.mark.parametrize("n", [1, 4097, 16385, 100003])
+def test_no_write_outside_outputs_and_workspaces(n):
+    rng = np.random.default_rng(n)
+    checks = []
+
+    def out_ws(nbytes_out, nbytes_ws, dtype):
+        o, c1 = guarded(nbytes_out)
+        w, c2 = guarded(max(256, nbytes_ws))
+        checks.extend([c1, c2])
+        return o.view(dtype), w
+
+    # scans
+    for name, dtype, q in SCAN_CASES:
+        d = scan_data(name, n)
+        npdt = np.float64 if dtype == torch.float64 else np.float32
+        op = B.Op.of(name, dtype)
+        xs, yb = dev(d["xs"].astype(npdt)), dev(d["ys_bar"].astype(npdt))
+        out, ws = out_ws(yb.numel() * yb.element_size(), B.vjp_scan_workspace_bytes(op, n), dtype)
+        B.vjp_scan(op, xs, yb, out=out.view(yb.shape), ws=ws)
+        out2, ws2 = out_ws(yb.numel() * yb.element_size(), B.vjp_scan_workspace_bytes(op, n), dtype)
+        B.scan_forward(op, xs, out=out2.view(xs.shape), ws=ws2)
+    # reduce-by-index, narrow and wide histograms
+    for w in (7, 1024, 20000, 70000):
+        is_ = dev(rng.integers(-3, w + 3, size=n, dtype=np.int64))
+        vs = dev(rng.uniform(0.5, 1.5, n).astype(np.float32))
+        hb = dev(rng.standard_normal(w).astype(np.float32))
+        for opname in ("add", "min", "max", "mul", "satadd"):
+            op = B.Op.of(opname, S=0.6 * n / w + 0.37)
+            out, ws = out_ws(n * 4, B.vjp_reduce_by_index_workspace_bytes(op, n, w), torch.float32)
+            B.vjp_reduce_by_index(op, w, is_, vs, hb, out=out, ws=ws)
+            hist, ws2 = out_ws(w * 4, B.vjp_reduce_by_index_workspace_bytes(op, n, w), torch.float32)
+            B.reduce_by_index_forward(op, w, is_, vs, out=hist, ws=ws2)
+    # reduce
+    xs = dev(rng.uniform(0.5, 1.5, n).astype(np.float32))
+    yb1 = torch.ones(1, device="cuda")
+    for opname in ("add", "min", "mul", "satadd"):
+        op = B.Op.of(opname, S=0.3 * n)
+        out, ws = out_ws(n * 4, B.vjp_reduce_workspace_bytes(op, n), torch.float32)
+        B.vjp_reduce(op, xs, yb1, out=out, ws=ws)
+    for c in checks:
+        c()

@@ -10,7 +10,11 @@ from paper_2310_03568_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
+import os
+
 SIZES = [1, 2, 3, 5, 511, 2047, 2049, 4097, 65537, 300007, 1 << 21]
+if os.environ.get("VJP_TEST_MAX_N"):
+    SIZES = [n for n in SIZES if n <= int(os.environ["VJP_TEST_MAX_N"])]
 
 
 def dev(a):
