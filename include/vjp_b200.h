@@ -14,7 +14,7 @@
  *     The *_host entry points are the exception: their data pointers are HOST pointers, they
  *     copy host->device, run the same kernels, copy the result back and synchronise `stream`.
  *   - Scan elements are [n][d] contiguous row-major, d = vjp_scan_arity(op): 1 ('+', '*'),
- *     2 (linear recurrence (a,b)), 4 (2x2 row-major matrix), 25 (5x5 row-major matrix).
+ *     2 (linear recurrence (a,b)), 4 (2x2 row-major matrix), 9 (3x3), 25 (5x5 row-major matrix).
  *   - Bin indices `is` are int64.  An index outside [0, num_bins) -- negative
  *     included -- is ignored by the primal and receives adjoint exactly 0 (P:L335-336,
  *     P:L361-362; Q3).
@@ -62,8 +62,10 @@ typedef enum {
                            config 3).  scan only (not commutative)                   */
     VJP_OP_MATMUL2 = 5, /* 2x2 row-major matrix product R x X, neutral I.  scan only */
     VJP_OP_MATMUL5 = 6, /* 5x5 row-major matrix product.                            scan only */
-    VJP_OP_SATADD = 7   /* min(a+b, S) on non-negative reals, neutral 0 (Q16).
-                           reduce-by-index only; always the general rule (Fig. 4)            */
+    VJP_OP_SATADD = 7,  /* min(a+b, S) on non-negative reals, neutral 0 (Q16).
+                           reduce-by-index / reduce only; always the general rule (Fig. 4)   */
+    VJP_OP_MATMUL3 = 8  /* 3x3 row-major matrix product (the paper's worst
+                           measured overhead).  scan only (round 2, NEXT row f4)              */
 } vjp_opcode_t;
 
 typedef enum { VJP_F32 = 0, VJP_F64 = 1 } vjp_dtype_t;
@@ -92,7 +94,7 @@ size_t vjp_scan_workspace_bytes(const vjp_op_t *op, int64_t n);
 
 /* Primal inclusive scan ys[i] = xs[0] (.) ... (.) xs[i].  Single-pass
  * decoupled-look-back kernel.  Exists for the AD-overhead denominator.
- * Supported: ADD (f32, f64), MUL (f32, f64), LINREC (f32), MATMUL2 (f32), MATMUL5 (f32). */
+ * Supported: ADD (f32, f64), MUL (f32, f64), LINREC (f32), MATMUL2 / MATMUL3 / MATMUL5 (f32). */
 int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
                  void *ws, size_t ws_bytes, void *stream);
 

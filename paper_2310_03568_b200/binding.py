@@ -18,9 +18,9 @@ from . import build as _build
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE, ERR_CUDA = 0, -1, -2, -3, -4
 _STATUS = {-1: "VJP_ERR_INVALID_ARG", -2: "VJP_ERR_UNSUPPORTED", -3: "VJP_ERR_WORKSPACE", -4: "VJP_ERR_CUDA"}
 
-OP_ADD, OP_MIN, OP_MAX, OP_MUL, OP_LINREC, OP_MATMUL2, OP_MATMUL5, OP_SATADD = range(8)
+OP_ADD, OP_MIN, OP_MAX, OP_MUL, OP_LINREC, OP_MATMUL2, OP_MATMUL5, OP_SATADD, OP_MATMUL3 = range(9)
 OPCODES = {"add": OP_ADD, "min": OP_MIN, "max": OP_MAX, "mul": OP_MUL, "linrec": OP_LINREC,
-           "matmul2": OP_MATMUL2, "matmul5": OP_MATMUL5, "satadd": OP_SATADD}
+           "matmul2": OP_MATMUL2, "matmul3": OP_MATMUL3, "matmul5": OP_MATMUL5, "satadd": OP_SATADD}
 F32, F64 = 0, 1
 
 EXPORTS = [

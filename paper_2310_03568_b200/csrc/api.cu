@@ -10,7 +10,7 @@ using namespace vjp;
 namespace {
 
 bool op_ok(const vjp_op_t *op) {
-    return op && op->code >= VJP_OP_ADD && op->code <= VJP_OP_SATADD &&
+    return op && op->code >= VJP_OP_ADD && op->code <= VJP_OP_MATMUL3 &&
            (op->dtype == VJP_F32 || op->dtype == VJP_F64);
 }
 // every data pointer must be 16-byte aligned (128-bit accesses); NULL passes (checked separately)
@@ -25,6 +25,7 @@ bool scan_supported(const vjp_op_t *op) {
     case VJP_OP_MUL: return true;
     case VJP_OP_LINREC:
     case VJP_OP_MATMUL2:
+    case VJP_OP_MATMUL3:
     case VJP_OP_MATMUL5: return op->dtype == VJP_F32;
     default: return false;
     }
@@ -123,6 +124,7 @@ int vjp_scan_arity(const vjp_op_t *op) {
     case VJP_OP_MUL: return 1;
     case VJP_OP_LINREC: return 2;
     case VJP_OP_MATMUL2: return 4;
+    case VJP_OP_MATMUL3: return 9;
     case VJP_OP_MATMUL5: return 25;
     default: return -1;
     }

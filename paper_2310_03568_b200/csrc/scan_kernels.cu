@@ -420,6 +420,7 @@ using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
 using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8>;
+using CfgMat3 = ScanCfg<OpMatMul<3, float, double, float>, 256, 8, 256, 6>;  // f64 forward products, as 2x2 (Q27)
 using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
 
 #define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
@@ -428,6 +429,7 @@ using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;     \
     case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } else { FAIL } break;          \
     case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } else { FAIL } break;           \
+    case VJP_OP_MATMUL3: if (dtype == VJP_F32) { F(CfgMat3) } else { FAIL } break;           \
     case VJP_OP_MATMUL5: if (dtype == VJP_F32) { F(CfgMat5) } else { FAIL } break;           \
     default: FAIL                                                                            \
     }
@@ -442,6 +444,7 @@ size_t scan_workspace_bytes(int code, int dtype, int64_t n) {
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
     case VJP_OP_LINREC: F(CfgLinRec) break;
     case VJP_OP_MATMUL2: F(CfgMat2) break;
+    case VJP_OP_MATMUL3: F(CfgMat3) break;
     case VJP_OP_MATMUL5: F(CfgMat5) break;
     default: return 0;
     }
@@ -471,6 +474,7 @@ int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
     case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } break;
     case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } break;
+    case VJP_OP_MATMUL3: if (dtype == VJP_F32) { F(CfgMat3) } break;
     case VJP_OP_MATMUL5: if (dtype == VJP_F32) { F(CfgMat5) } break;
     default: break;
     }

@@ -27,7 +27,7 @@ def nrel(got, ref):
 # ------------------------------------------------------------------ accumulate ------------
 
 SCAN_CASES = [("add", torch.float32, 0), ("add", torch.float64, 0), ("mul", torch.float64, 0), ("linrec", torch.float32, 0),
-              ("matmul2", torch.float32, 2), ("matmul5", torch.float32, 5)]
+              ("matmul2", torch.float32, 2), ("matmul3", torch.float32, 3), ("matmul5", torch.float32, 5)]
 
 
 def scan_data(name, n):

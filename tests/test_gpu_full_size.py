@@ -79,9 +79,10 @@ def test_c3_scan_linrec_full():
     assert nrel(got, oracle.vjp_scan("linrec", d["xs"], d["ys_bar"])) <= 1e-4
 
 
-@pytest.mark.parametrize("q", [2, 5])
+@pytest.mark.parametrize("q", [2, 3, 5])
 def test_c4_scan_matmul_full(q):
-    d = W.c4_scan_matmul(q)
+    # q = 3 is not a BASELINE config (NEXT row f4): run at the 5x5 size, n = 2^22
+    d = W.c4_scan_matmul(q, n=(1 << 22) if q == 3 else None)
     got = B.vjp_scan(B.Op.of("matmul%d" % q), dev(d["xs"]), dev(d["ys_bar"])).cpu().numpy()
     ref = oracle.vjp_scan("matmul", d["xs"], d["ys_bar"], q=q)
     e = nrel(got, ref)

@@ -66,14 +66,14 @@ def scan_inputs(name, n, seed=0):
     if name == "linrec":
         d = W.c3_scan_linrec(n=n, seed=seed)
         return B.Op.of("linrec"), "linrec", 0, d["xs"], d["ys_bar"]
-    if name in ("matmul2", "matmul5"):
+    if name in ("matmul2", "matmul3", "matmul5"):
         q = int(name[-1])
         d = W.c4_scan_matmul(q, n=n, seed=seed)
         return B.Op.of(name), "matmul", q, d["xs"], d["ys_bar"]
     raise ValueError(name)
 
 
-SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "linrec", "matmul2", "matmul5"]
+SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "linrec", "matmul2", "matmul3", "matmul5"]
 
 
 @pytest.mark.parametrize("n", SIZES)
