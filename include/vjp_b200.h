@@ -55,8 +55,9 @@ typedef enum {
 
 typedef enum {
     VJP_OP_ADD = 0,     /* a + b, neutral 0.                       scan + reduce-by-index   */
-    VJP_OP_MIN = 1,     /* min, neutral +inf, lowest index on ties. rbi only       */
-    VJP_OP_MAX = 2,     /* max, neutral -inf, lowest index on ties (Q4).     rbi only       */
+    VJP_OP_MIN = 1,     /* min, neutral +inf, lowest index on ties.  rbi, reduce, and scan
+                           (f32; the left operand keeps ties: round 2, NEXT row f4)   */
+    VJP_OP_MAX = 2,     /* max, neutral -inf, lowest index on ties (Q4).      as MIN            */
     VJP_OP_MUL = 3,     /* a * b, neutral 1, exact with zeros.     scan + reduce-by-index   */
     VJP_OP_LINREC = 4,  /* (A,B)(+)(a,b) = (a*A, a*B+b), neutral (1,0) (BASELINE
                            config 3).  scan only (not commutative)                   */
@@ -94,13 +95,15 @@ size_t vjp_scan_workspace_bytes(const vjp_op_t *op, int64_t n);
 
 /* Primal inclusive scan ys[i] = xs[0] (.) ... (.) xs[i].  Single-pass
  * decoupled-look-back kernel.  Exists for the AD-overhead denominator.
- * Supported: ADD (f32, f64), MUL (f32, f64), LINREC (f32), MATMUL2 / MATMUL3 / MATMUL5 (f32). */
+ * Supported: ADD (f32, f64), MUL (f32, f64), MIN / MAX (f32), LINREC (f32), MATMUL2 / MATMUL3 / MATMUL5 (f32). */
 int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
                  void *ws, size_t ws_bytes, void *stream);
 
 /* Input adjoints of the inclusive scan: xs_bar = J^T ys_bar (Fig. 7; return sweep
  * P:L553-558).
  *   ADD:   xs_bar = reverse inclusive sum of ys_bar; xs may be NULL.
+ *   MIN/MAX: as `other`, but the 1-by-1 Jacobian [x_{i+1} does not win] depends on the running prefix:
+ *          the reverse kernel rebuilds the forward prefixes of its tile first.
  *   other: forward tile prefixes r_{i-1} are recomputed from xs (no tape), then ONE
  *          fused reverse kernel forms the Jacobians on the fly (never stored), runs
  *          the reverse linear-recurrence scan rbar_i = ys_bar_i + J_i^T rbar_{i+1} with lin_o

@@ -162,12 +162,12 @@ VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (D
     "c1_rbi_add": 12, "c2_rbi_min": 16, "c2_rbi_mul": 28, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 32,
     "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
-    "f4_scan_matmul3": 144,
+    "f4_scan_matmul3": 144, "f4_scan_min": 16,
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
     "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
-    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8,
 }
 
 
@@ -305,6 +305,7 @@ def case_table(scale=1.0):
     ]
     t.append(("f4_scan_matmul3", "f4 scan matmul 3x3 f32 n=2^22 (NEXT row)",
               scan("matmul3", lambda: W.c4_scan_matmul(3, n=sz(1 << 22)))))
+    t.append(("f4_scan_min", "f4 scan min f32 n=2^26 (NEXT row)", scan("min", lambda: W.c3_scan_add(n=n3))))
     for opname in ("add", "min", "mul"):  # NEXT row f2 (not a BASELINE config): reduce VJP, n = 2^24
         t.append(("f2_reduce_" + opname, "f2 reduce %s f32 n=2^24 (NEXT row)" % opname,
                   lambda opname=opname: ReduceCase(B.Op.of(opname), W.f2_reduce(opname, n=sz(1 << 24)))))

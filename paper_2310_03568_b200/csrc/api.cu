@@ -23,6 +23,8 @@ bool scan_supported(const vjp_op_t *op) {
     switch (op->code) {
     case VJP_OP_ADD:
     case VJP_OP_MUL: return true;
+    case VJP_OP_MIN:
+    case VJP_OP_MAX:
     case VJP_OP_LINREC:
     case VJP_OP_MATMUL2:
     case VJP_OP_MATMUL3:
@@ -121,6 +123,8 @@ int vjp_scan_arity(const vjp_op_t *op) {
     if (!op) return -1;
     switch (op->code) {
     case VJP_OP_ADD:
+    case VJP_OP_MIN:
+    case VJP_OP_MAX:
     case VJP_OP_MUL: return 1;
     case VJP_OP_LINREC: return 2;
     case VJP_OP_MATMUL2: return 4;

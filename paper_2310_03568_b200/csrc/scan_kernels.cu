@@ -242,6 +242,46 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
         St::read_row(sy, threadIdx.x, rry);
     }
 
+    if constexpr (Op::PREFIX_DEP) {
+        // The Jacobian of element i depends on the running prefix r_{i-1} (min / max): forward prefixes first.
+        static_assert(!WIDE, "prefix-dependent operators are scalar");
+        FS facc = Op::identity();
+#pragma unroll
+        for (int j = 0; j < IPT; j++) facc = Op::combine(facc, Op::from_elem(rx + j * EW));
+        FS ftotal;
+        const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+        FS rp[IPT];
+        rp[0] = Op::combine(load_state_cg(fpre + t), fex);
+#pragma unroll
+        for (int j = 1; j < IPT; j++) rp[j] = Op::combine(rp[j - 1], Op::from_elem(rx + (j - 1) * EW));
+        // thread-local reverse reduce: u -> (ybar_j + u) * c_j, c_j = d(r_{j-1} (.) x_j)/dr_{j-1}
+        RS racc = RM::identity();
+#pragma unroll
+        for (int j = IPT - 1; j >= 0; j--) {
+            const typename Op::Lin c = Op::lin_at(rp[j], Op::from_elem(rx + j * EW));
+            racc.b = Op::adj_mul(Op::adj_add(Op::adj_from_elem(ry + j * EW), racc.b), c);
+            racc.l = Op::lin_combine(c, racc.l);
+        }
+        RS rtotal;
+        const RS rex = RBS::template exclusive<true>(racc, rtotal, scratch);
+        if (threadIdx.x < 32) {
+            RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
+            __syncwarp();
+            if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
+        }
+        __syncthreads();
+        const Adj ztile = load_state_smem<Adj>(bcast);  // u entering the tile from the right
+        Adj u = Op::adj_add(rex.b, Op::adj_mul(ztile, rex.l));
+        const int64_t first_elem = base + (int64_t)threadIdx.x * IPT;
+#pragma unroll
+        for (int j = IPT - 1; j >= 0; j--) {
+            const FS xj = Op::from_elem(rx + j * EW);
+            const Adj rbar = Op::adj_add(Op::adj_from_elem(ry + j * EW), u);
+            u = Op::adj_mul(rbar, Op::lin_at(rp[j], xj));
+            Op::xbar_at(rp[j], xj, rbar, first_elem + j == 0, ry + j * EW);
+        }
+        St::write_row(sy, threadIdx.x, rry);
+    } else {
     // thread-local reduce, walking the thread's elements from the highest index down
     Adj bacc = Op::adj_zero();
     FS facc = Op::identity();
@@ -303,6 +343,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
         }
         St::write_row(sy, threadIdx.x, rry);
     }
+    }  // !PREFIX_DEP
     __syncthreads();
     St::template store<typename Op::T>(sy, xbar + base * EW, valid * EW, accumulate != 0);
 }
@@ -419,6 +460,8 @@ using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
+using CfgMinF32 = ScanCfg<OpMinMax<float, false>, 512, 32, 512, 16>;
+using CfgMaxF32 = ScanCfg<OpMinMax<float, true>, 512, 32, 512, 16>;
 using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8>;
 using CfgMat3 = ScanCfg<OpMatMul<3, float, double, float>, 256, 8, 256, 6>;  // f64 forward products, as 2x2 (Q27)
 using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
@@ -427,6 +470,8 @@ using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
     switch (code) {                                                                          \
     case VJP_OP_ADD: if (dtype == VJP_F32) { F(CfgAddF32) } else { F(CfgAddF64) } break;     \
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;     \
+    case VJP_OP_MIN: if (dtype == VJP_F32) { F(CfgMinF32) } else { FAIL } break;             \
+    case VJP_OP_MAX: if (dtype == VJP_F32) { F(CfgMaxF32) } else { FAIL } break;             \
     case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } else { FAIL } break;          \
     case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } else { FAIL } break;           \
     case VJP_OP_MATMUL3: if (dtype == VJP_F32) { F(CfgMat3) } else { FAIL } break;           \
@@ -442,6 +487,8 @@ size_t scan_workspace_bytes(int code, int dtype, int64_t n) {
 #define F(C) a = ws_bytes_cfg<C>(n); b = ws_bytes_vjp_cfg<C>(n);
     switch (code) {
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
+    case VJP_OP_MIN: F(CfgMinF32) break;
+    case VJP_OP_MAX: F(CfgMaxF32) break;
     case VJP_OP_LINREC: F(CfgLinRec) break;
     case VJP_OP_MATMUL2: F(CfgMat2) break;
     case VJP_OP_MATMUL3: F(CfgMat3) break;
@@ -472,6 +519,8 @@ int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *
 #define F(C) return run_vjp<C>(n, xs, ys_bar, xs_bar, (char *)ws, accumulate, stream);
     switch (code) {
     case VJP_OP_MUL: if (dtype == VJP_F32) { F(CfgMulF32) } else { F(CfgMulF64) } break;
+    case VJP_OP_MIN: if (dtype == VJP_F32) { F(CfgMinF32) } break;
+    case VJP_OP_MAX: if (dtype == VJP_F32) { F(CfgMaxF32) } break;
     case VJP_OP_LINREC: if (dtype == VJP_F32) { F(CfgLinRec) } break;
     case VJP_OP_MATMUL2: if (dtype == VJP_F32) { F(CfgMat2) } break;
     case VJP_OP_MATMUL3: if (dtype == VJP_F32) { F(CfgMat3) } break;

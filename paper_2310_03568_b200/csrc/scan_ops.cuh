@@ -42,6 +42,7 @@ struct OpAdd {
 template <class T_>
 struct OpMul {
     using T = T_;
+    static constexpr bool PREFIX_DEP = false;
     static constexpr int D = 1;
     static constexpr int EW = WordsOf<T>::value;
     struct Fwd { T v; };
@@ -66,6 +67,42 @@ struct OpMul {
     }
 };
 
+// --------------------------------------------------------------------------- min / max ---
+// r (.) x = min(r, x) with the LEFT (accumulated) operand winning ties (scan with min/max through
+// the general rule with d = 1).  NOT linear in r: the 1-by-1 Jacobian d(r (.) x)/dr = [x does not win] depends
+// on the running prefix r_{i-1} itself (PREFIX_DEP): the reverse kernel builds the forward prefixes first and
+// forms c_i = lin_at(r_{i-1}, x_i) from them; the reverse scan is then that of the scalar recurrence
+// u_i = (ybar_i + u_{i+1}) * c_i, and xbar_i = [x_i wins] * rbar_i (the first element always wins: P:L558).
+template <class T_, bool IS_MAX>
+struct OpMinMax {
+    using T = T_;
+    static constexpr bool PREFIX_DEP = true;
+    static constexpr int D = 1;
+    static constexpr int EW = WordsOf<T>::value;
+    struct Fwd { T v; };
+    struct Lin { T v; };
+    struct Adj { T v; };
+    static VJP_DEVINL T neutral_value() { return IS_MAX ? -__int_as_float(0x7f800000) : __int_as_float(0x7f800000); }
+    static VJP_DEVINL bool wins(T x, T r) { return IS_MAX ? x > r : x < r; }  // strict: the left operand keeps ties
+    static VJP_DEVINL Fwd identity() { return Fwd{neutral_value()}; }
+    static VJP_DEVINL Fwd from_elem(const uint32_t *w) { return Fwd{word_to(w, (T *)nullptr)}; }
+    static VJP_DEVINL void to_elem(const Fwd &f, uint32_t *w) { to_word(f.v, w); }
+    static VJP_DEVINL Fwd combine(const Fwd &l, const Fwd &r) { return Fwd{wins(r.v, l.v) ? r.v : l.v}; }
+    static VJP_DEVINL void identity_words(uint32_t (&w)[EW]) { to_word(neutral_value(), w); }
+
+    static VJP_DEVINL Lin lin_at(const Fwd &rprev, const Fwd &x) { return Lin{wins(x.v, rprev.v) ? T(0) : T(1)}; }
+    static VJP_DEVINL Lin lin_identity() { return Lin{T(1)}; }
+    static VJP_DEVINL Lin lin_combine(const Lin &l, const Lin &r) { return Lin{l.v * r.v}; }
+    static VJP_DEVINL Adj adj_zero() { return Adj{T(0)}; }
+    static VJP_DEVINL Adj adj_from_elem(const uint32_t *w) { return Adj{word_to(w, (T *)nullptr)}; }
+    static VJP_DEVINL Adj adj_add(const Adj &a, const Adj &b) { return Adj{a.v + b.v}; }
+    static VJP_DEVINL Adj adj_mul(const Adj &z, const Lin &l) { return Adj{z.v * l.v}; }
+    // xbar = [x wins against r_{i-1}] * rbar_i; `first`: element 0 of the array takes rbar_0 (xb[0] = rb[0])
+    static VJP_DEVINL void xbar_at(const Fwd &rprev, const Fwd &x, const Adj &rbar, bool first, uint32_t *w) {
+        to_word((first || wins(x.v, rprev.v)) ? rbar.v : T(0), w);
+    }
+};
+
 // ------------------------------------------------------------------- linear recurrence ---
 // (A,B) (+) (a,b) = (a*A, a*B + b)   (BASELINE config 3; the paper's lin_o with c = a).
 // d/d(A,B) = a * I_2 (redundant block-diagonal with a 1x1 block);
@@ -73,6 +110,7 @@ struct OpMul {
 template <class T_>
 struct OpLinRec {
     using T = T_;
+    static constexpr bool PREFIX_DEP = false;
     static constexpr int D = 2;
     static constexpr int EW = 2 * WordsOf<T>::value;
     struct Fwd { T a, b; };
@@ -118,6 +156,7 @@ struct OpLinRec {
 template <int Q, class T_, class AF, class AA>
 struct OpMatMul {
     using T = T_;
+    static constexpr bool PREFIX_DEP = false;
     static constexpr int D = Q * Q;
     static constexpr int EW = D * WordsOf<T>::value;
     struct Fwd { AF m[D]; };

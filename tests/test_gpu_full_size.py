@@ -99,3 +99,15 @@ def test_c5_rbi_satadd_full():
     sk, perm = B.rbi_sort_perm(w, dev(d["is_"]))
     rsk, rperm = oracle.rbi_sort_perm(w, d["is_"])
     assert np.array_equal(sk.cpu().numpy(), rsk) and np.array_equal(perm.cpu().numpy(), rperm)
+
+
+@pytest.mark.parametrize("opname", ["min", "max"])
+def test_f4_scan_minmax_full(opname):
+    """NEXT row f4: scan with min / max at n = 2^26: the adjoint of a record-setting element is the sum of the
+    ys_bar of the run it dominates; all other adjoints are exactly 0."""
+    d = W.c3_scan_add()
+    xs = np.round(d["xs"], 2)
+    got = B.vjp_scan(B.Op.of(opname), dev(xs), dev(d["ys_bar"])).cpu().numpy()
+    ref = oracle.vjp_scan(opname, xs, d["ys_bar"])
+    assert np.array_equal(got != 0, ref != 0)
+    assert nrel(got, ref) <= 1e-4

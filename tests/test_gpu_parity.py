@@ -63,6 +63,12 @@ def scan_inputs(name, n, seed=0):
     if name == "mul_f32":
         d = W.c3_scan_mul(n=n, seed=seed, dtype=np.float32, zero_rate=0.0, lo=0.999, hi=1.001)
         return B.Op.of("mul"), "mul", 0, d["xs"], d["ys_bar"]
+    if name in ("min_f32", "max_f32"):
+        d = W.c3_scan_add(n=n, seed=seed)
+        xs = np.round(d["xs"], 1)                       # rounding forces ties: the left operand keeps them
+        if n > 40:
+            xs[n // 3:n // 3 + 7] = np.float32(-6.0 if name == "min_f32" else 6.0)   # a run of equal record values
+        return B.Op.of(name[:3]), name[:3], 0, xs, d["ys_bar"]
     if name == "linrec":
         d = W.c3_scan_linrec(n=n, seed=seed)
         return B.Op.of("linrec"), "linrec", 0, d["xs"], d["ys_bar"]
@@ -73,7 +79,7 @@ def scan_inputs(name, n, seed=0):
     raise ValueError(name)
 
 
-SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "linrec", "matmul2", "matmul3", "matmul5"]
+SCAN_OPS = ["add_f32", "add_f64", "mul_f64", "mul_f64_nozero", "mul_f32", "min_f32", "max_f32", "linrec", "matmul2", "matmul3", "matmul5"]
 
 
 @pytest.mark.parametrize("n", SIZES)
@@ -86,6 +92,8 @@ def test_scan_vjp_matches_oracle(name, n):
     op, oname, q, xs, ys_bar = scan_inputs(name, n)
     got = B.vjp_scan(op, dev(xs), dev(ys_bar)).cpu().numpy()
     ref = oracle.vjp_scan(oname, xs, ys_bar, q=q)
+    if name in ("min_f32", "max_f32"):   # a selection: every adjoint is a sum of ys_bar entries, order-dependent only in rounding
+        assert np.array_equal(got != 0, ref != 0)
     assert nrel(got, ref) <= TOL[op.torch_dtype]
 
 
