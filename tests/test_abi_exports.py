@@ -38,7 +38,8 @@ def test_header_binding_and_library_export_the_same_entry_points():
 def test_library_loads_and_answers_host_only_queries():
     lib = B.load()
     assert lib.vjp_version().decode().startswith("vjp_b200")
-    assert B.scan_arity(B.Op.of("matmul5")) == 25 and B.scan_arity(B.Op.of("min")) == -1
+    assert B.scan_arity(B.Op.of("matmul5")) == 25 and B.scan_arity(B.Op.of("matmul3")) == 9
+    assert B.scan_arity(B.Op.of("min")) == 1 and B.scan_arity(B.Op.of("satadd")) == -1
     assert B.vjp_scan_workspace_bytes(B.Op.of("linrec"), 1 << 20) > 0
     assert B.vjp_reduce_by_index_workspace_bytes(B.Op.of("mul"), 1 << 20, 1 << 16) > 0
     assert len(B.kernel_names()) == lib.vjp_kernel_count() and all(B.kernel_names())
