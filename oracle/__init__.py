@@ -202,3 +202,38 @@ def vjp_reduce(op, xs, y_bar):
     _check(_load().orc_reduce_vjp(op, ctypes.c_int64(n), _p(xs), ctypes.c_double(float(y_bar)), _p(xs_bar),
                                   ctypes.byref(ai), ctypes.byref(av)), "reduce_vjp")
     return xs_bar, ai.value, av.value
+
+
+# ------------------------------------------------------------------ sumOfProd (sections 3.3, 4.2.4) ----
+
+def sop_apply(a, b):
+    """(p1,s1) sumOfProd (p2,s2) (P:L318)."""
+    a, b, out = _f64(a), _f64(b), np.empty(2)
+    _check(_load().orc_sop_apply(_p(a), _p(b), _p(out)), "sop_apply")
+    return out
+
+
+def sop_inv(z, b):
+    """(p,s) sumOfProd_inv (p2,s2) (P:L319)."""
+    z, b, out = _f64(z), _f64(b), np.empty(2)
+    _check(_load().orc_sop_inv(_p(z), _p(b), _p(out)), "sop_inv")
+    return out
+
+
+def rbi_sop_forward(num_bins, is_, vs):
+    """reduce_by_index with sumOfProd; vs is [n, 2] = (p, s), the result [w, 2]."""
+    is_, vs = _i64(is_), _f64(vs)
+    hist = np.empty((num_bins, 2), dtype=np.float64)
+    _check(_load().orc_rbi_sop_forward(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(vs), _p(hist)),
+           "rbi_sop_forward")
+    return hist
+
+
+def vjp_rbi_sop(num_bins, is_, vs, hist_bar, general: bool = False):
+    """vs_bar [n, 2] by the invertible-operator rule (Fig. 6) or, general=True, by eq. 5 with pair folds."""
+    is_, vs, hist_bar = _i64(is_), _f64(vs), _f64(hist_bar)
+    vs_bar = np.empty((is_.size, 2), dtype=np.float64)
+    fn = _load().orc_rbi_sop_vjp_general if general else _load().orc_rbi_sop_vjp_inv
+    _check(fn(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(vs), _p(hist_bar), _p(vs_bar)),
+           "rbi_sop_vjp")
+    return vs_bar

@@ -21,7 +21,10 @@
  *                       folds (the radix sort of Fig. 4 is only a way to find them);
  *   - reduce:           the sequential fold, eq. 2 with the two
  *                       exclusive scans of Fig. 2, and the specialised rules of section 3.2
- *                       as their plain definitions (added in round 2, before the kernels).
+ *                       as their plain definitions (added in round 2, before the kernels);
+ *   - sumOfProd:        the invertible operator of section 3.3 -- its reduce_by_index loop,
+ *                       Fig. 6 (invertible-operator rule) literally, and eq. 5 with pair folds
+ *                       (added in round 2, before the kernels).
  * Parity pins: tests/test_oracle_pins.py (closed forms, finite differences, brute-force
  * dense Jacobian transposes, dot-product test, PPAD's rule of Fig. 11, hand-worked
  * fixtures under tests/golden/).  No function here is "parity unpinned".
@@ -453,4 +456,92 @@ int orc_reduce_vjp(int op, int64_t n, const double *xs, double y_bar, double *xs
     }
     default: return ORC_EINVAL;
     }
+}
+
+/* ---------------------------------------------- invertible operators: sumOfProd (3.3, 4.2.4) --
+ *
+ * (p1,s1) sumOfProd (p2,s2)     = (p1 + p2 + s1*s2, s1 + s2)            neutral (0,0)   (Fig. 6)
+ * (p,s)   sumOfProd_inv (p2,s2) = (p - p2 - (s - s2)*s2, s - s2)                        (Fig. 6)
+ * Elements are pairs stored [n][2] = (p, s); the histogram is [w][2]. */
+static void sop_apply(const double *a, const double *b, double *out) {
+    double p = a[0] + b[0] + a[1] * b[1], s = a[1] + b[1];
+    out[0] = p; out[1] = s;
+}
+static void sop_inv(const double *z, const double *b, double *out) {
+    double s = z[1] - b[1];
+    out[0] = z[0] - b[0] - s * b[1]; out[1] = s;
+}
+
+/* reduce_by_index with sumOfProd over a neutral-initialised histogram: the loop of P:L335. */
+int orc_rbi_sop_forward(int64_t n, int64_t w, const int64_t *is, const double *vs, double *hist) {
+    if (n < 0 || w < 0) return ORC_EINVAL;
+    for (int64_t k = 0; k < 2 * w; k++) hist[k] = 0.0;
+    for (int64_t i = 0; i < n; i++) {
+        int64_t key = is[i];
+        if (in_range(key, w)) sop_apply(hist + 2 * key, vs + 2 * i, hist + 2 * key);
+    }
+    return ORC_OK;
+}
+
+/* The operator and its inverse on single pairs (for the pins of property (3)). */
+int orc_sop_apply(const double *a, const double *b, double *out) { sop_apply(a, b, out); return ORC_OK; }
+int orc_sop_inv(const double *z, const double *b, double *out) { sop_inv(z, b, out); return ORC_OK; }
+
+/* (d(b (.) x)/dx)^T g  at any x, for y = b sumOfProd x = (bp + xp + bs*xs, bs + xs):
+ *   dyp/dxp = 1, dyp/dxs = bs, dys/dxp = 0, dys/dxs = 1   =>   xbar = (gp, gp*bs + gs). */
+static void sop_vjp_right(const double *b, const double *g, double *xbar) {
+    xbar[0] = g[0];
+    xbar[1] = g[0] * b[1] + g[1];
+}
+
+/* Invertible-operator rule, Fig. 6 literally: xs = the primal histogram;
+ * b_i = xs[k_i] (.)_inv v_i;  vs_bar_i = (d(b_i (.) x)/dx)^T xs_bar[k_i];  0 out of range. */
+int orc_rbi_sop_vjp_inv(int64_t n, int64_t w, const int64_t *is, const double *vs,
+                        const double *hist_bar, double *vs_bar) {
+    if (n < 0 || w < 0) return ORC_EINVAL;
+    double *xs = (double *)malloc((size_t)(w > 0 ? 2 * w : 2) * sizeof(double));
+    if (!xs) return ORC_ENOMEM;
+    orc_rbi_sop_forward(n, w, is, vs, xs);
+    for (int64_t i = 0; i < n; i++) {
+        int64_t key = is[i];
+        if (!in_range(key, w)) { vs_bar[2 * i] = vs_bar[2 * i + 1] = 0.0; continue; }
+        double b[2];
+        sop_inv(xs + 2 * key, vs + 2 * i, b);
+        sop_vjp_right(b, hist_bar + 2 * key, vs_bar + 2 * i);
+    }
+    free(xs);
+    return ORC_OK;
+}
+
+/* General-case rule, eq. 5 with pairs: l_i / r_i = sumOfProd-fold of the same-bin elements before /
+ * after i;  y = l (.) x (.) r = (lp + xp + ls*xs + rp + (ls + xs)*rs, ls + xs + rs):
+ *   dyp/dxp = 1, dyp/dxs = ls + rs, dys/dxs = 1   =>   xbar = (gp, gp*(ls + rs) + gs). */
+int orc_rbi_sop_vjp_general(int64_t n, int64_t w, const int64_t *is, const double *vs,
+                            const double *hist_bar, double *vs_bar) {
+    if (n < 0 || w < 0) return ORC_EINVAL;
+    size_t wn = (size_t)(w > 0 ? w : 1), nn = (size_t)(n > 0 ? n : 1);
+    double *acc = (double *)malloc(2 * wn * sizeof(double));
+    double *l = (double *)malloc(2 * nn * sizeof(double));
+    if (!acc || !l) { free(acc); free(l); return ORC_ENOMEM; }
+    for (int64_t k = 0; k < 2 * w; k++) acc[k] = 0.0;
+    for (int64_t i = 0; i < n; i++) {
+        int64_t key = is[i];
+        if (!in_range(key, w)) continue;
+        l[2 * i] = acc[2 * key]; l[2 * i + 1] = acc[2 * key + 1];
+        sop_apply(acc + 2 * key, vs + 2 * i, acc + 2 * key);
+    }
+    for (int64_t k = 0; k < 2 * w; k++) acc[k] = 0.0;
+    for (int64_t i = n - 1; i >= 0; i--) {
+        int64_t key = is[i];
+        if (!in_range(key, w)) { vs_bar[2 * i] = vs_bar[2 * i + 1] = 0.0; continue; }
+        const double *r = acc + 2 * key, *g = hist_bar + 2 * key;
+        vs_bar[2 * i] = g[0];
+        vs_bar[2 * i + 1] = g[0] * (l[2 * i + 1] + r[1]) + g[1];
+        double t[2];
+        sop_apply(vs + 2 * i, r, t); /* r of the previous same-bin element = v_i (.) r_i */
+        acc[2 * key] = t[0]; acc[2 * key + 1] = t[1];
+    }
+    free(acc);
+    free(l);
+    return ORC_OK;
 }
