@@ -181,6 +181,28 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
                   int64_t *perm, void *ws, size_t ws_bytes, void *stream);
 
+/* -------------------------------------------------------------------------- sumOfProd ----- */
+
+/* reduce_by_index with the invertible operator sumOfProd (sections 3.3 and 4.2.4 of the paper):
+ *   (p1,s1) sumOfProd (p2,s2) = (p1 + p2 + s1*s2, s1 + s2), neutral (0,0)
+ * Elements are f32 pairs: vs [n][2] = (p, s), hist / hist_bar [num_bins][2], vs_bar [n][2].
+ * Primal: the fold of a bin has the closed form P = sum p + ((sum s)^2 - sum s^2) / 2, S = sum s, so the
+ * histogram is three float atomicAdd histograms and a finish pass. */
+size_t rbi_sumofprod_workspace_bytes(int64_t n, int64_t num_bins, int use_general);
+int rbi_sumofprod_forward(int64_t n, int64_t num_bins, const int64_t *is, const float *vs, float *hist,
+                          void *ws, size_t ws_bytes, void *stream);
+
+/* Input adjoints vs_bar of the above.
+ *   use_general == 0: the invertible-operator rule of Fig. 6: xs = the primal histogram,
+ *                     b_i = xs[k_i] sumOfProd_inv v_i, vs_bar_i = (d(b_i (.) x)/dx)^T hist_bar[k_i]
+ *                     -- a histogram and a map.
+ *   use_general != 0: the general rule of Fig. 4 (sort by bin, forward and reverse segmented scans, eq. 5)
+ *                     for the same operator -- the paper's 8 - 92x against 1.1 - 2.1x contrast.
+ * accumulate != 0 adds to vs_bar.  Keys outside [0, num_bins) get (0, 0). */
+int vjp_rbi_sumofprod(int64_t n, int64_t num_bins, const int64_t *is, const float *vs,
+                      const float *hist_bar, float *vs_bar, int use_general, int accumulate,
+                      void *ws, size_t ws_bytes, void *stream);
+
 /* ----------------------------------------------------------------------------- reduce ----- */
 
 /* reduce (section 3 of the paper): y = a_0 (.) a_1 (.) ... (.) a_{n-1}, one scalar.

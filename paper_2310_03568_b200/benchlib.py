@@ -163,11 +163,12 @@ VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (D
     "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
     "f4_scan_matmul3": 144, "f4_scan_min": 16,
+    "f1_sop_inv": 40, "f1_sop_general": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
     "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
-    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16,
 }
 
 
@@ -229,6 +230,23 @@ class ScanCase:
 
     def primal(self):
         return B.scan_forward(self.op, self.xs, out=self.out, ws=self.ws)
+
+
+class SopCase:
+    """NEXT row f1: reduce-by-index with sumOfProd, by the invertible-operator rule or the general rule."""
+
+    def __init__(self, d, general):
+        self.n, self.w, self.general = int(d["n"]), int(d["w"]), general
+        self.is_, self.vs, self.hb = to_dev(d["is_"]), to_dev(d["vs"]), to_dev(d["hist_bar"])
+        self.out = torch.empty(2 * self.n, dtype=torch.float32, device="cuda")
+        self.hist = torch.empty(2 * self.w, dtype=torch.float32, device="cuda")
+        self.ws = torch.empty(max(256, B.rbi_sumofprod_workspace_bytes(self.n, self.w, True)), dtype=torch.uint8, device="cuda")
+
+    def vjp(self):
+        return B.vjp_rbi_sumofprod(self.w, self.is_, self.vs, self.hb, general=self.general, out=self.out, ws=self.ws)
+
+    def primal(self):
+        return B.rbi_sumofprod_forward(self.w, self.is_, self.vs, out=self.hist, ws=self.ws)
 
 
 class ReduceCase:
@@ -303,6 +321,10 @@ def case_table(scale=1.0):
         ("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
          rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])))),
     ]
+    for general in (False, True):  # NEXT row f1: the same data through both rules
+        t.append(("f1_sop_general" if general else "f1_sop_inv",
+                  "f1 rbi sumOfProd w=1024 uniform, %s (NEXT row)" % ("general rule" if general else "invertible rule"),
+                  lambda general=general: SopCase(W.f1_rbi_sumofprod(n=sz(1 << 24)), general)))
     t.append(("f4_scan_matmul3", "f4 scan matmul 3x3 f32 n=2^22 (NEXT row)",
               scan("matmul3", lambda: W.c4_scan_matmul(3, n=sz(1 << 22)))))
     t.append(("f4_scan_min", "f4 scan min f32 n=2^26 (NEXT row)", scan("min", lambda: W.c3_scan_add(n=n3))))

@@ -29,6 +29,7 @@ EXPORTS = [
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
     "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
     "vjp_reduce_workspace_bytes", "reduce_forward", "vjp_reduce", "reduce_lifted",
+    "rbi_sumofprod_workspace_bytes", "rbi_sumofprod_forward", "vjp_rbi_sumofprod",
     "vjp_kernel_count", "vjp_kernel_name", "vjp_launch_count", "vjp_profile_enable", "vjp_profile_read",
 ]
 
@@ -98,6 +99,9 @@ def load() -> ctypes.CDLL:
         "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+        "rbi_sumofprod_workspace_bytes": (sz, [i64, i64, ctypes.c_int]),
+        "rbi_sumofprod_forward": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_rbi_sumofprod": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp, sz, vp]),
         "vjp_reduce_workspace_bytes": (sz, [opp, i64]),
         "reduce_forward": (ctypes.c_int, [opp, i64, vp, vp, vp, sz, vp]),
         "vjp_reduce": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
@@ -350,6 +354,40 @@ def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm
+
+
+# ------------------------------------------------------------------ sumOfProd ------------
+
+def rbi_sumofprod_workspace_bytes(n: int, num_bins: int, general: bool = False) -> int:
+    return load().rbi_sumofprod_workspace_bytes(n, num_bins, int(general))
+
+
+def rbi_sumofprod_forward(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, out=None, ws=None, stream=None):
+    """reduce_by_index with sumOfProd (P:L318): vs [n, 2] = (p, s) -> hist [num_bins, 2]."""
+    is_ = _dev(is_, torch.int64, what="is")
+    n = is_.numel()
+    vs = _dev(vs, torch.float32, 2 * n, "vs")
+    hist = _out(out, torch.float32, 2 * num_bins, is_.device, "hist")
+    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins), is_.device, ws)
+    _check(load().rbi_sumofprod_forward(n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist), _ptr(ws), ws.numel(),
+                                        _stream(stream)), "rbi_sumofprod_forward")
+    return hist.view(num_bins, 2)
+
+
+def vjp_rbi_sumofprod(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, hist_bar: torch.Tensor, general: bool = False,
+                      accumulate: bool = False, out=None, ws=None, stream=None):
+    """vs_bar [n, 2] by the invertible-operator rule (Fig. 6) or, general=True, by sort + segmented scans (Fig. 4)."""
+    is_ = _dev(is_, torch.int64, what="is")
+    n = is_.numel()
+    vs = _dev(vs, torch.float32, 2 * n, "vs")
+    hist_bar = _dev(hist_bar, torch.float32, 2 * num_bins, "hist_bar")
+    if out is None and accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    vs_bar = _out(out, torch.float32, 2 * n, is_.device, "vs_bar")
+    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins, general), is_.device, ws)
+    _check(load().vjp_rbi_sumofprod(n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar), _ptr(vs_bar), int(general),
+                                    int(accumulate), _ptr(ws), ws.numel(), _stream(stream)), "vjp_rbi_sumofprod")
+    return vs_bar.view(n, 2)
 
 
 # ------------------------------------------------------------------ reduce ---------------

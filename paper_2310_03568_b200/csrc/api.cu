@@ -61,7 +61,8 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "rbi_cached_fold_kernel", "rbi_mul_finish_kernel", "rbi_mul_sweep_kernel",
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel",
-    "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel"};
+    "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel",
+    "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];
@@ -350,6 +351,36 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
         return VJP_ERR_WORKSPACE;
     return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs), nullptr, nullptr, zeros,
                           static_cast<float *>(prod_nz), ws, 0, as_stream(stream));
+}
+
+// --------------------------------------------------------------------------- sumOfProd ----
+
+size_t rbi_sumofprod_workspace_bytes(int64_t n, int64_t num_bins, int use_general) {
+    if (n < 0 || num_bins < 0) return 0;
+    return use_general ? rbi_general_workspace_bytes(n, num_bins) : rbi_sop_workspace_bytes(num_bins);
+}
+
+int rbi_sumofprod_forward(int64_t n, int64_t num_bins, const int64_t *is, const float *vs, float *hist,
+                          void *ws, size_t ws_bytes, void *stream) {
+    if (n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if ((num_bins > 0 && (!hist || !ws)) || (n > 0 && (!is || !vs)) || !all_aligned(is, vs, hist, ws))
+        return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < rbi_sop_workspace_bytes(num_bins)) return VJP_ERR_WORKSPACE;
+    return launch_rbi_sop_forward(n, num_bins, is, vs, hist, ws, as_stream(stream));
+}
+
+int vjp_rbi_sumofprod(int64_t n, int64_t num_bins, const int64_t *is, const float *vs, const float *hist_bar,
+                      float *vs_bar, int use_general, int accumulate, void *ws, size_t ws_bytes, void *stream) {
+    if (n < 0 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!is || !vs || !vs_bar || !ws || (num_bins > 0 && !hist_bar) || !all_aligned(is, vs, hist_bar, vs_bar, ws))
+        return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < rbi_sumofprod_workspace_bytes(n, num_bins, use_general)) return VJP_ERR_WORKSPACE;
+    if (use_general)
+        return launch_rbi_sop_general_vjp(n, num_bins, is, vs, hist_bar, vs_bar, ws, accumulate != 0, as_stream(stream));
+    return launch_rbi_sop_vjp_inv(n, num_bins, is, vs, hist_bar, vs_bar, ws, accumulate != 0, as_stream(stream));
 }
 
 // ------------------------------------------------------------------------------ reduce ----

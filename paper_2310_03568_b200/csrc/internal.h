@@ -29,6 +29,7 @@ enum KernelId : int {
     K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
+    K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -73,6 +74,15 @@ int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const i
                            int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
                          int64_t *perm, void *ws, cudaStream_t stream);
+
+// -------------------------------------------------------------------------- sumOfProd ---
+size_t rbi_sop_workspace_bytes(int64_t w);
+int launch_rbi_sop_forward(int64_t n, int64_t w, const int64_t *is, const float *vs, float *hist, void *ws,
+                           cudaStream_t stream);
+int launch_rbi_sop_vjp_inv(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
+                           float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
+int launch_rbi_sop_general_vjp(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
+                               float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
 
 // ----------------------------------------------------------------------------- reduce ---
 size_t reduce_special_workspace_bytes();

@@ -220,7 +220,7 @@ constexpr size_t SORT_SCATTER_SMEM = (size_t)SORT_TILE * 12;
 template <bool FIRST>
 __global__ void __launch_bounds__(SORT_NT)
 sort_scatter_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
-                    const float *__restrict__ vs, const uint32_t *__restrict__ kin,
+                    const float *__restrict__ vs, int vstride, const uint32_t *__restrict__ kin,
                     const uint2 *__restrict__ pin, int shift, int radix, int num_tiles,
                     const uint32_t *__restrict__ offsets, uint32_t *__restrict__ kout,
                     uint2 *__restrict__ pout) {
@@ -295,7 +295,7 @@ sort_scatter_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             const uint32_t d = (key[j] >> shift) & mask;
             const uint32_t lp = dstart[d] + cnt[warp][d] + rank[j];
             skey[lp] = key[j];
-            spay[lp] = FIRST ? make_uint2((uint32_t)i, vs ? __float_as_uint(__ldg(vs + i)) : 0u)
+            spay[lp] = FIRST ? make_uint2((uint32_t)i, vs ? __float_as_uint(__ldg(vs + i * vstride)) : 0u)
                              : __ldg(pin + i);
         }
     }
@@ -311,7 +311,9 @@ sort_scatter_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 
 // ------------------------------------------------------------------ operators -------------
 
-enum : int { G_ADD = 0, G_MIN = 1, G_MAX = 2, G_MUL = 3, G_SATADD = 4 };
+// G_SOP: sumOfProd.  Of l (.) x (.) r only the s components enter the derivative with respect to x
+// (d yp / d xs = ls + rs), so the segmented scans carry s alone, under '+'; the output is a pair.
+enum : int { G_ADD = 0, G_MIN = 1, G_MAX = 2, G_MUL = 3, G_SATADD = 4, G_SOP = 5 };
 
 // The operator, its neutral element, and d/dx of (l (.) x) (.) r at x = v (eq. 5).
 template <int CODE>
@@ -323,6 +325,7 @@ struct GenOp {
     VJP_DEVINL float apply(float a, float b) const {
         switch (CODE) {
         case G_ADD: return a + b;
+        case G_SOP: return a + b;
         case G_MUL: return a * b;
         case G_MIN: return b < a ? b : a;
         case G_MAX: return b > a ? b : a;
@@ -334,6 +337,7 @@ struct GenOp {
     VJP_DEVINL float dfdx(float l, float v, float r) const {
         switch (CODE) {
         case G_ADD: return 1.f;
+        case G_SOP: return l + r;
         case G_MUL: return l * r;
         case G_MIN: return (v < l && !(r < v)) ? 1.f : 0.f;
         case G_MAX: return (v > l && !(r > v)) ? 1.f : 0.f;
@@ -470,9 +474,17 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
     load_row<SEG_IPT>(reinterpret_cast<const uint32_t *>(ls) + base, mine, 0u, lw);
     load_row<2 * SEG_IPT>(reinterpret_cast<const uint32_t *>(pay + base), 2 * mine, 0u, pw);
     // the bin adjoints of the row: issued now, consumed after the scan
-    float hb[SEG_IPT];
+    float hb[SEG_IPT], hb2[CODE == G_SOP ? SEG_IPT : 1];  // G_SOP: hist_bar is [w][2] = (Pbar, Sbar)
 #pragma unroll
-    for (int j = 0; j < SEG_IPT; j++) hb[j] = k[j] < (uint32_t)w ? __ldg(hist_bar + k[j]) : 0.f;
+    for (int j = 0; j < SEG_IPT; j++) {
+        if constexpr (CODE == G_SOP) {
+            const float2 h = k[j] < (uint32_t)w ? __ldg(reinterpret_cast<const float2 *>(hist_bar) + k[j]) : make_float2(0.f, 0.f);
+            hb[j] = h.x;
+            hb2[j] = h.y;
+        } else {
+            hb[j] = k[j] < (uint32_t)w ? __ldg(hist_bar + k[j]) : 0.f;
+        }
+    }
     first_key[threadIdx.x] = k[0];
     __syncthreads();
     uint32_t next;
@@ -506,7 +518,18 @@ seg_reverse_vjp_kernel(int64_t n, int64_t w, const uint32_t *__restrict__ keys,
         if (j < mine) {
             // out-of-range keys were clamped to w: adjoint 0 (hb is 0 there)
             const float g = k[j] < (uint32_t)w ? op.dfdx(__uint_as_float(lw[j]), v, r) * hb[j] : 0.f;
-            vs_bar[pw[2 * j]] = accumulate ? vs_bar[pw[2 * j]] + g : g;  // the permutation names every index once
+            if constexpr (CODE == G_SOP) {  // vs_bar_i = (Pbar, Pbar * (ls + rs) + Sbar)
+                float2 *dst = reinterpret_cast<float2 *>(vs_bar) + pw[2 * j];
+                float2 o = make_float2(hb[j], g + hb2[j]);
+                if (accumulate) {
+                    const float2 pr = *dst;
+                    o.x += pr.x;
+                    o.y += pr.y;
+                }
+                *dst = o;
+            } else {
+                vs_bar[pw[2 * j]] = accumulate ? vs_bar[pw[2 * j]] + g : g;  // the permutation names every index once
+            }
         }
     }
 }
@@ -563,7 +586,7 @@ size_t rbi_general_workspace_bytes(int64_t n, int64_t) { return gen_carve(nullpt
 
 // Sorts (clamped key, (index, value)); returns the buffer index holding the result in *out_buf.
 static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, const GenWs &g,
-                    int *out_buf, cudaStream_t stream) {
+                    int *out_buf, cudaStream_t stream, int vstride = 1) {
     if (cudaFuncSetAttribute(sort_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)SORT_SCATTER_SMEM) != cudaSuccess ||
         cudaFuncSetAttribute(sort_scatter_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -590,10 +613,10 @@ static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, co
         const int sb = (int)((m + US_NT * US_IPT - 1) / (US_NT * US_IPT));
         VJP_LAUNCH(K_U32_SCAN, stream) u32_exclusive_scan_kernel<<<sb, US_NT, 0, stream>>>(g.counts, m, g.ticket, g.status);
         if (ps == 0)
-            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<true><<<nt, SORT_NT, SORT_SCATTER_SMEM, stream>>>(n, w, is, vs, nullptr, nullptr, shift, radix,
+            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<true><<<nt, SORT_NT, SORT_SCATTER_SMEM, stream>>>(n, w, is, vs, vstride, nullptr, nullptr, shift, radix,
                                                                   nt, g.counts, g.key[dst], g.pay[dst]);
         else
-            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<false><<<nt, SORT_NT, SORT_SCATTER_SMEM, stream>>>(n, w, nullptr, nullptr, g.key[src],
+            VJP_LAUNCH(K_SORT_SCATTER, stream) sort_scatter_kernel<false><<<nt, SORT_NT, SORT_SCATTER_SMEM, stream>>>(n, w, nullptr, nullptr, 1, g.key[src],
                                                                    g.pay[src], shift, radix, nt, g.counts,
                                                                    g.key[dst], g.pay[dst]);
         src = dst;
@@ -625,6 +648,18 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
     int rc = run_sort(n, w, is, vs, g, &buf, stream);
     if (rc != VJP_OK) return rc;
     return run_segscans<CODE>(S, n, w, g.key[buf], g.pay[buf], hist_bar, vs_bar, g, accumulate, stream);
+}
+
+// sumOfProd through the general rule (Fig. 4): sort by bin with the s component as payload, segmented exclusive
+// '+' scans of s forwards and backwards, vs_bar_i = (Pbar, Pbar * (ls_i + rs_i) + Sbar).
+int launch_rbi_sop_general_vjp(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
+                               float *vs_bar, void *ws, int accumulate, cudaStream_t stream) {
+    if (n == 0) return VJP_OK;
+    const GenWs g = gen_carve(ws, n);
+    int buf;
+    const int rc = run_sort(n, w, is, vs + 1, g, &buf, stream, 2);
+    if (rc != VJP_OK) return rc;
+    return run_segscans<G_SOP>(0.f, n, w, g.key[buf], g.pay[buf], hist_bar, vs_bar, g, accumulate, stream);
 }
 
 // reduce, general rule (eq. 2; Fig. 2): ls = forward exclusive scan, rs = reverse exclusive

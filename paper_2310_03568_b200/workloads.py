@@ -192,3 +192,14 @@ def f2_reduce(op, n=1 << 24, seed=0):
                 xs[pos] = ext
     y_bar = np.asarray(_rng(seed, 6, 9).standard_normal(1), dtype=np.float32)
     return dict(n=n, xs=xs, y_bar=y_bar)
+
+
+def f1_rbi_sumofprod(n=1 << 24, w=1 << 10, dist="uniform", seed=0):
+    """NEXT row f1 (invertible operator sumOfProd, sections 3.3 / 4.2.4): pairs (p, s) ~ N(0,1)^2 as [n, 2] f32, keys as
+    in config 2 (uniform or Zipf(1.1)) with 3 % out of range on both sides, bin adjoints (Pbar, Sbar) ~ N(0,1)^2."""
+    cell = {"uniform": 0, "zipf": 1}[dist] + 2 * int(np.log2(w))
+    is_ = _keys(dist, _rng(seed, 7, 10 + cell), n, w)
+    oob = _rng(seed, 7, 40 + cell).random(n) < 0.03
+    is_[oob] = np.where(np.arange(n)[oob] % 2 == 0, -1 - (is_[oob] % 5), w + (is_[oob] % 7))
+    vs = _normal_f32(_rng(seed, 7, 70 + cell), (n, 2))
+    return dict(n=n, w=w, is_=is_, vs=vs, hist_bar=_normal_f32(_rng(seed, 7, 100 + cell), (w, 2)))
