@@ -237,3 +237,37 @@ def vjp_rbi_sop(num_bins, is_, vs, hist_bar, general: bool = False):
     _check(fn(ctypes.c_int64(is_.size), ctypes.c_int64(num_bins), _p(is_), _p(vs), _p(hist_bar), _p(vs_bar)),
            "rbi_sop_vjp")
     return vs_bar
+
+
+# ------------------------------------------------------------------ vectorised operators (3.2.4, 4.2.5) ----
+# reduce_by_index / scan with the operator `map2 (.)` on rows of d scalars.  By IRWIM / ISWIM (eq. 3 P:L252-263,
+# P:L464-466) the combinator moves inside the map: column c of the result depends on column c of the
+# input only, so the plain definition is the scalar definition applied to every column.
+
+def rbi_forward_vec(op, num_bins, is_, vss, S: float = 0.0):
+    """hist[k, :] = fold over i with is[i] = k of vss[i, :] under map2 (.); vss is [n, d]."""
+    vss = _f64(vss)
+    return np.stack([reduce_by_index_forward(op, num_bins, is_, vss[:, c], S=S) for c in range(vss.shape[1])], axis=1)
+
+
+def vjp_rbi_vec(op, num_bins, is_, vss, hist_bar, S: float = 0.0):
+    """vss_bar [n, d] of the vectorised reduce_by_index given hist_bar [w, d]: the scalar rule per column."""
+    vss, hist_bar = _f64(vss), _f64(hist_bar)
+    name = op if isinstance(op, str) else {v: k for k, v in OPS.items()}[op]
+    cols = []
+    for c in range(vss.shape[1]):
+        if name == "add":
+            cols.append(vjp_rbi_add(num_bins, is_, hist_bar[:, c]))
+        elif name in ("min", "max"):
+            cols.append(vjp_rbi_minmax(name, num_bins, is_, vss[:, c], hist_bar[:, c])[0])
+        elif name == "mul":
+            cols.append(vjp_rbi_mul(num_bins, is_, vss[:, c], hist_bar[:, c])[0])
+        else:
+            cols.append(vjp_rbi_general(name, num_bins, is_, vss[:, c], hist_bar[:, c], S=S))
+    return np.stack(cols, axis=1)
+
+
+def vjp_scan_vec(op, xss, yss_bar):
+    """xss_bar [n, d] of the inclusive scan with map2 (.) over rows of d scalars: the scalar rule per column."""
+    xss, yss_bar = _f64(xss), _f64(yss_bar)
+    return np.stack([vjp_scan(op, xss[:, c], yss_bar[:, c]) for c in range(xss.shape[1])], axis=1)
