@@ -181,6 +181,23 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
 int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorted_keys,
                   int64_t *perm, void *ws, size_t ws_bytes, void *stream);
 
+/* ---------------------------------------------------------------- vectorised operators ----- */
+
+/* reduce_by_index and scan with the vectorised operator `map2 (.)` on rows of d f32 scalars
+ * (sections 3.2.4 / 4.2.5): vss, vss_bar are [n][d], hist_bar is [num_bins][d]; xss, yss_bar, xss_bar are [n][d].
+ * The rule is the INTERCHANGE of the combinator with the inner map (IRWIM eq. 3 P:L252-263 and its
+ * reduce-by-index form P:L464-466; ISWIM P:L655-657): the arrays are transposed, the scalar rule runs on each of
+ * the d columns (any scalar operator the scalar entry point accepts in f32: ADD, MIN, MAX, MUL, SATADD for
+ * reduce_by_index; ADD, MUL, MIN, MAX for scan), and the result is transposed back (op.accumulate fused there).
+ * d <= 4096. */
+size_t vjp_reduce_by_index_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins);
+int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins, const int64_t *is,
+                            const void *vss, const void *hist_bar, void *vss_bar,
+                            void *ws, size_t ws_bytes, void *stream);
+size_t vjp_scan_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d);
+int vjp_scan_vec(const vjp_op_t *op, int64_t n, int64_t d, const void *xss, const void *yss_bar,
+                 void *xss_bar, void *ws, size_t ws_bytes, void *stream);
+
 /* -------------------------------------------------------------------------- sumOfProd ----- */
 
 /* reduce_by_index with the invertible operator sumOfProd (sections 3.3 and 4.2.4 of the paper):

@@ -163,12 +163,13 @@ VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (D
     "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
     "f4_scan_matmul3": 144, "f4_scan_min": 16,
+    "f3_rbi_vec_mul": 16 + 28 * 4,   # per ROW of d = 4: two transposes (read + write 4 d each way) + d scalar '*' VJPs at 28 B
     "f1_sop_inv": 40, "f1_sop_general": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
     "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
-    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16, "f3_rbi_vec_mul": 8 + 4 * 4,
 }
 
 
@@ -249,6 +250,29 @@ class SopCase:
         return B.rbi_sumofprod_forward(self.w, self.is_, self.vs, out=self.hist, ws=self.ws)
 
 
+class VecCase:
+    """NEXT row f3: reduce-by-index with map2 (*) on rows of d scalars; the primal column = d scalar primal calls."""
+
+    def __init__(self, d):
+        self.n, self.d, self.w = int(d["n"]), int(d["d"]), int(d["w"])
+        self.op = B.Op.of("mul")
+        self.is_, self.vss, self.hb = to_dev(d["is_"]), to_dev(d["vss"]), to_dev(d["hist_bar"])
+        self.cols = self.vss.t().contiguous()
+        self.out = torch.empty(self.n * self.d, dtype=torch.float32, device="cuda")
+        self.hist = torch.empty(self.w, dtype=torch.float32, device="cuda")
+        o = self.op.c()
+        import ctypes
+        self.ws = torch.empty(B.load().vjp_reduce_by_index_vec_workspace_bytes(ctypes.byref(o), self.n, self.d, self.w),
+                              dtype=torch.uint8, device="cuda")
+
+    def vjp(self):
+        return B.vjp_reduce_by_index_vec(self.op, self.w, self.is_, self.vss, self.hb, out=self.out, ws=self.ws)
+
+    def primal(self):  # the interchanged primal: d scalar histograms on the columns (transposed once, outside the timing)
+        for c in range(self.d):
+            B.reduce_by_index_forward(self.op, self.w, self.is_, self.cols[c], out=self.hist, ws=self.ws)
+
+
 class ReduceCase:
     """NEXT row f2: one reduce VJP problem (section 3 of the paper) resident on the device."""
 
@@ -321,6 +345,7 @@ def case_table(scale=1.0):
         ("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
          rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])))),
     ]
+    t.append(("f3_rbi_vec_mul", "f3 rbi map2(*) d=4 n=2^22 rows w=1024 (NEXT row)", lambda: VecCase(W.f3_rbi_vec("mul", n=sz(1 << 22)))))
     for general in (False, True):  # NEXT row f1: the same data through both rules
         t.append(("f1_sop_general" if general else "f1_sop_inv",
                   "f1 rbi sumOfProd w=1024 uniform, %s (NEXT row)" % ("general rule" if general else "invertible rule"),

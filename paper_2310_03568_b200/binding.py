@@ -30,6 +30,7 @@ EXPORTS = [
     "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
     "vjp_reduce_workspace_bytes", "reduce_forward", "vjp_reduce", "reduce_lifted",
     "rbi_sumofprod_workspace_bytes", "rbi_sumofprod_forward", "vjp_rbi_sumofprod",
+    "vjp_reduce_by_index_vec_workspace_bytes", "vjp_reduce_by_index_vec", "vjp_scan_vec_workspace_bytes", "vjp_scan_vec",
     "vjp_kernel_count", "vjp_kernel_name", "vjp_launch_count", "vjp_profile_enable", "vjp_profile_read",
 ]
 
@@ -99,6 +100,10 @@ def load() -> ctypes.CDLL:
         "rbi_argext": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_zero_prod": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
         "rbi_sort_perm": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_reduce_by_index_vec_workspace_bytes": (sz, [opp, i64, i64, i64]),
+        "vjp_reduce_by_index_vec": (ctypes.c_int, [opp, i64, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
+        "vjp_scan_vec_workspace_bytes": (sz, [opp, i64, i64]),
+        "vjp_scan_vec": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, sz, vp]),
         "rbi_sumofprod_workspace_bytes": (sz, [i64, i64, ctypes.c_int]),
         "rbi_sumofprod_forward": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_rbi_sumofprod": (ctypes.c_int, [i64, i64, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, vp, sz, vp]),
@@ -354,6 +359,45 @@ def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm
+
+
+# ------------------------------------------------------------------ vectorised operators --
+
+def vjp_reduce_by_index_vec(op: Op, num_bins: int, is_: torch.Tensor, vss, hist_bar: torch.Tensor, out=None, ws=None,
+                            stream=None) -> torch.Tensor:
+    """vss_bar [n, d] of reduce_by_index with map2 (.) on rows of d scalars (eq. 3); hist_bar is [w, d]."""
+    is_ = _dev(is_, torch.int64, what="is")
+    n, d = is_.numel(), hist_bar.shape[-1]
+    hist_bar = _dev(hist_bar, torch.float32, num_bins * d, "hist_bar")
+    if vss is not None:
+        vss = _dev(vss, torch.float32, n * d, "vss")
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    vss_bar = _out(out, torch.float32, n * d, is_.device, "vss_bar")
+    o = op.c()
+    need = load().vjp_reduce_by_index_vec_workspace_bytes(ctypes.byref(o), n, d, num_bins)
+    ws = _workspace(need, is_.device, ws)
+    _check(load().vjp_reduce_by_index_vec(ctypes.byref(o), n, d, num_bins, _ptr(is_), _ptr(vss), _ptr(hist_bar),
+                                          _ptr(vss_bar), _ptr(ws), ws.numel(), _stream(stream)), "vjp_reduce_by_index_vec")
+    return vss_bar.view(n, d)
+
+
+def vjp_scan_vec(op: Op, xss, yss_bar: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
+    """xss_bar [n, d] of the inclusive scan with map2 (.) on rows of d scalars (ISWIM)."""
+    if yss_bar.dim() != 2:
+        raise VjpError("yss_bar must be [n, d]")
+    n, d = yss_bar.shape
+    yss_bar = _dev(yss_bar, torch.float32, n * d, "yss_bar")
+    if xss is not None:
+        xss = _dev(xss, torch.float32, n * d, "xss")
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    xss_bar = _out(out, torch.float32, n * d, yss_bar.device, "xss_bar")
+    o = op.c()
+    ws = _workspace(load().vjp_scan_vec_workspace_bytes(ctypes.byref(o), n, d), yss_bar.device, ws)
+    _check(load().vjp_scan_vec(ctypes.byref(o), n, d, _ptr(xss), _ptr(yss_bar), _ptr(xss_bar), _ptr(ws), ws.numel(),
+                               _stream(stream)), "vjp_scan_vec")
+    return xss_bar.view(n, d)
 
 
 # ------------------------------------------------------------------ sumOfProd ------------

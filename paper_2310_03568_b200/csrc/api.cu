@@ -62,7 +62,7 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel",
     "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel",
-    "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel"};
+    "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel", "rows_to_cols / cols_to_rows"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];
@@ -351,6 +351,96 @@ int rbi_zero_prod(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t
         return VJP_ERR_WORKSPACE;
     return launch_rbi_mul(n, num_bins, is, static_cast<const float *>(vs), nullptr, nullptr, zeros,
                           static_cast<float *>(prod_nz), ws, 0, as_stream(stream));
+}
+
+// ----------------------------------------------------------------- vectorised operators ----
+
+namespace {
+struct VecWs {
+    float *cols, *outs, *hbs;
+    char *inner;
+    int64_t ncol, wcol;
+    size_t total;
+};
+// columns are padded to a multiple of 4 floats so that every column start is 16-byte aligned
+VecWs vec_carve(void *ws, int64_t n, int64_t d, int64_t w, size_t inner_bytes) {
+    VecWs v;
+    v.ncol = (n + 3) / 4 * 4;
+    v.wcol = (w + 3) / 4 * 4;
+    char *p = static_cast<char *>(ws);
+    auto take = [&](size_t bytes) { char *r = p; p += align_up(bytes < 16 ? 16 : bytes, 256); return r; };
+    v.cols = reinterpret_cast<float *>(take((size_t)v.ncol * d * 4));
+    v.outs = reinterpret_cast<float *>(take((size_t)v.ncol * d * 4));
+    v.hbs = reinterpret_cast<float *>(take((size_t)v.wcol * d * 4));
+    v.inner = take(inner_bytes);
+    v.total = (size_t)(p - static_cast<char *>(ws));
+    return v;
+}
+bool vec_op_ok(const vjp_op_t *op) { return op_ok(op) && op->dtype == VJP_F32; }
+}  // namespace
+
+size_t vjp_reduce_by_index_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins) {
+    if (!vec_op_ok(op) || n < 0 || d < 1 || num_bins < 0) return 0;
+    const size_t inner = vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
+    return inner ? vec_carve(nullptr, n, d, num_bins, inner).total : 0;
+}
+
+int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins, const int64_t *is,
+                            const void *vss, const void *hist_bar, void *vss_bar, void *ws, size_t ws_bytes,
+                            void *stream) {
+    if (!op_ok(op) || n < 0 || d < 1 || num_bins < 0) return VJP_ERR_INVALID_ARG;
+    if (!vec_op_ok(op) || rbi_route(op) == 0) return VJP_ERR_UNSUPPORTED;
+    if (n >= RBI_MAX_N || num_bins >= RBI_MAX_N || d > 4096) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    const bool needs_vs = rbi_route(op) != 1;
+    if (!is || !vss_bar || !ws || (num_bins > 0 && !hist_bar) || (needs_vs && !vss)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(is, vss, hist_bar, vss_bar, ws)) return VJP_ERR_INVALID_ARG;
+    const size_t inner = vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
+    const VecWs v = vec_carve(ws, n, d, num_bins, inner);
+    if (ws_bytes < v.total) return VJP_ERR_WORKSPACE;
+    cudaStream_t s = as_stream(stream);
+    int rc;
+    if (needs_vs && (rc = launch_rows_to_cols(n, d, v.ncol, static_cast<const float *>(vss), v.cols, s)) != VJP_OK) return rc;
+    if ((rc = launch_rows_to_cols(num_bins, d, v.wcol, static_cast<const float *>(hist_bar), v.hbs, s)) != VJP_OK) return rc;
+    vjp_op_t col = *op;
+    col.accumulate = 0;  // the "+=" is fused into the transpose back
+    for (int64_t c = 0; c < d; c++) {  // the scalar rule on every column (eq. 3: map (reduce ...) (transpose ...))
+        rc = vjp_reduce_by_index(&col, n, num_bins, is, needs_vs ? v.cols + c * v.ncol : nullptr, v.hbs + c * v.wcol,
+                                 v.outs + c * v.ncol, v.inner, inner, stream);
+        if (rc != VJP_OK) return rc;
+    }
+    return launch_cols_to_rows(n, d, v.ncol, v.outs, static_cast<float *>(vss_bar), op->accumulate != 0, s);
+}
+
+size_t vjp_scan_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d) {
+    if (!vec_op_ok(op) || n < 0 || d < 1 || vjp_scan_arity(op) != 1) return 0;
+    const size_t inner = vjp_scan_workspace_bytes(op, n);
+    return inner ? vec_carve(nullptr, n, d, n, inner).total : 0;  // hbs holds the transposed output adjoints
+}
+
+int vjp_scan_vec(const vjp_op_t *op, int64_t n, int64_t d, const void *xss, const void *yss_bar, void *xss_bar,
+                 void *ws, size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0 || d < 1) return VJP_ERR_INVALID_ARG;
+    if (!vec_op_ok(op) || !scan_supported(op) || vjp_scan_arity(op) != 1 || d > 4096) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    const bool needs_xs = op->code != VJP_OP_ADD;
+    if (!yss_bar || !xss_bar || !ws || (needs_xs && !xss)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(xss, yss_bar, xss_bar, ws)) return VJP_ERR_INVALID_ARG;
+    const size_t inner = vjp_scan_workspace_bytes(op, n);
+    const VecWs v = vec_carve(ws, n, d, n, inner);  // hbs holds the transposed output adjoints
+    if (ws_bytes < v.total) return VJP_ERR_WORKSPACE;
+    cudaStream_t s = as_stream(stream);
+    int rc;
+    if (needs_xs && (rc = launch_rows_to_cols(n, d, v.ncol, static_cast<const float *>(xss), v.cols, s)) != VJP_OK) return rc;
+    if ((rc = launch_rows_to_cols(n, d, v.wcol, static_cast<const float *>(yss_bar), v.hbs, s)) != VJP_OK) return rc;
+    vjp_op_t col = *op;
+    col.accumulate = 0;
+    for (int64_t c = 0; c < d; c++) {  // ISWIM: scan (map2 (.)) = map (scan (.)) on the transpose
+        rc = vjp_scan(&col, n, needs_xs ? v.cols + c * v.ncol : nullptr, v.hbs + c * v.wcol, v.outs + c * v.ncol,
+                      v.inner, inner, stream);
+        if (rc != VJP_OK) return rc;
+    }
+    return launch_cols_to_rows(n, d, v.ncol, v.outs, static_cast<float *>(xss_bar), op->accumulate != 0, s);
 }
 
 // --------------------------------------------------------------------------- sumOfProd ----

@@ -29,7 +29,7 @@ enum KernelId : int {
     K_MINMAX_LIFTED, K_MINMAX_FINISH, K_CACHED_SMALL, K_CACHED_BIG, K_CACHED_FOLD, K_MUL_FINISH, K_MUL_SWEEP,
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
-    K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP,
+    K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP, K_VEC_TRANSPOSE,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -74,6 +74,11 @@ int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const i
                            int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
                          int64_t *perm, void *ws, cudaStream_t stream);
+
+// ---------------------------------------------------------------- vectorised operators ---
+int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream);
+int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, int accumulate,
+                        cudaStream_t stream);
 
 // -------------------------------------------------------------------------- sumOfProd ---
 size_t rbi_sop_workspace_bytes(int64_t w);

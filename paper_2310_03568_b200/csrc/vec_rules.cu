@@ -1,0 +1,55 @@
+// vec_rules.cu -- vectorised operators `map2 (.)` (sections 3.2.4 and 4.2.5 of the paper).
+//
+// reduce / reduce_by_index / scan whose operator acts element-wise on rows of d scalars are differentiated
+// by INTERCHANGE (IRWIM for reduce, eq. 3; its reduce-by-index form; ISWIM for scan,
+// P:L655-657): the combinator moves inside the map, i.e. the [n][d] array is transposed and the scalar rule
+// is applied to each of the d rows of the transpose.  This file holds the two transposes; the host loop over
+// the columns is in api.cu and calls the scalar entry points of the library.
+#include "common.cuh"
+#include "internal.h"
+
+namespace vjp {
+
+constexpr int TR_NT = 256;
+
+// out[c * cstride + r] = in[r * d + c]   ([n][d] -> d columns of stride cstride); flat over the input, so the
+// reads are coalesced and a warp writes d runs of 32 / d consecutive floats
+__global__ void __launch_bounds__(TR_NT)
+rows_to_cols_kernel(int64_t n, int64_t d, int64_t cstride, const float *__restrict__ in, float *__restrict__ out) {
+    const int64_t total = n * d, stride = (int64_t)gridDim.x * TR_NT;
+    for (int64_t e = blockIdx.x * (int64_t)TR_NT + threadIdx.x; e < total; e += stride) {
+        const int64_t r = e / d, c = e - r * d;
+        out[c * cstride + r] = __ldg(in + e);
+    }
+}
+
+// out[r * d + c] (+)= in[c * cstride + r]; flat over the output: coalesced writes
+__global__ void __launch_bounds__(TR_NT)
+cols_to_rows_kernel(int64_t n, int64_t d, int64_t cstride, const float *__restrict__ in, float *__restrict__ out,
+                    int accumulate) {
+    const int64_t total = n * d, stride = (int64_t)gridDim.x * TR_NT;
+    for (int64_t e = blockIdx.x * (int64_t)TR_NT + threadIdx.x; e < total; e += stride) {
+        const int64_t r = e / d, c = e - r * d;
+        const float v = __ldg(in + c * cstride + r);
+        out[e] = accumulate ? out[e] + v : v;
+    }
+}
+
+static int tr_grid(int64_t total) {
+    const int64_t need = (total + TR_NT - 1) / TR_NT, cap = (int64_t)NUM_SMS_B200 * 8;
+    return (int)(need < 1 ? 1 : (need < cap ? need : cap));
+}
+
+int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream) {
+    if (n * d == 0) return VJP_OK;
+    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) rows_to_cols_kernel<<<tr_grid(n * d), TR_NT, 0, stream>>>(n, d, cstride, in, out);
+    return last_launch_status();
+}
+int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, int accumulate,
+                        cudaStream_t stream) {
+    if (n * d == 0) return VJP_OK;
+    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) cols_to_rows_kernel<<<tr_grid(n * d), TR_NT, 0, stream>>>(n, d, cstride, in, out, accumulate);
+    return last_launch_status();
+}
+
+}  // namespace vjp

@@ -203,3 +203,19 @@ def f1_rbi_sumofprod(n=1 << 24, w=1 << 10, dist="uniform", seed=0):
     is_[oob] = np.where(np.arange(n)[oob] % 2 == 0, -1 - (is_[oob] % 5), w + (is_[oob] % 7))
     vs = _normal_f32(_rng(seed, 7, 70 + cell), (n, 2))
     return dict(n=n, w=w, is_=is_, vs=vs, hist_bar=_normal_f32(_rng(seed, 7, 100 + cell), (w, 2)))
+
+
+def f3_rbi_vec(op, n=1 << 22, d=4, w=1 << 10, seed=0, zero_rate=1e-3):
+    """NEXT row f3 (vectorised operators map2 (.), sections 3.2.4 / 4.2.5): rows of d scalars, uniform keys with 3 % out of
+    range, values per column as in config 2 ('*': U[0.9,1.1] with exact zeros; min/max/+: N(0,1) rounded to 2 decimals for
+    ties; satadd: U[0,1))."""
+    rng = _rng(seed, 8, d)
+    is_ = rng.integers(-w // 64 - 1, w + w // 64 + 1, size=n, dtype=np.int64)
+    if op == "mul":
+        vss = (0.9 + 0.2 * rng.random((n, d))).astype(np.float32)
+        vss[rng.random((n, d)) < zero_rate] = 0.0
+    elif op == "satadd":
+        vss = rng.random((n, d), dtype=np.float32)
+    else:
+        vss = np.round(_normal_f32(rng, (n, d)), 2)
+    return dict(n=n, d=d, w=w, is_=is_, vss=vss, hist_bar=_normal_f32(_rng(seed, 8, 100 + d), (w, d)))
