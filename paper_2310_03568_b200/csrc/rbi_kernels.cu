@@ -1069,32 +1069,35 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
 // 8 chains are combined in a fixed order through shared memory (deterministic).  Returns the result
 // in the threads with y == 0.  One thread per bin walking all G tables was latency-bound (10 % of
 // the bench step in the launch list of profiles/r1g).
-constexpr int FOLD_NT = 256;
-template <int ACC>
+// CH chains per bin (CTA of 32 * CH threads): 8, or 32 when there are hundreds of tables to fold (narrow histograms
+// written by every CTA of a full grid: 592 tables at w <= 1024), where 8 chains of 74 dependent loads were the
+// kernel's whole duration; at w = 2^16 (74 tables) 32 chains are slower (+13 us, round 1).
+template <int ACC, int CH>
 VJP_DEVINL float fold_partials(int64_t w, int G, const float *__restrict__ part, int64_t k, float S) {
-    __shared__ float sm[8][32];
+    __shared__ float sm[CH][32];
     const int x = threadIdx.x & 31, y = threadIdx.x >> 5;
     float p = CachedOp<ACC>::neutral();
     if (k < w) {
 #pragma unroll 4
-        for (int g = y; g < G; g += 8) p = CachedOp<ACC>::comb(p, __ldg(part + (size_t)g * (size_t)w + k), S);
+        for (int g = y; g < G; g += CH) p = CachedOp<ACC>::comb(p, __ldg(part + (size_t)g * (size_t)w + k), S);
     }
     sm[y][x] = p;
     __syncthreads();
     if (y == 0) {
 #pragma unroll
-        for (int i = 1; i < 8; i++) p = CachedOp<ACC>::comb(p, sm[i][x], S);
+        for (int i = 1; i < CH; i++) p = CachedOp<ACC>::comb(p, sm[i][x], S);
     }
     return p;
 }
+static int fold_chains(int G) { return G >= 256 ? 32 : 8; }
 static int fold_grid(int64_t w) { return (int)((w + 31) / 32); }
 
 // out[k] = fold over the G partial tables.
-template <int ACC>
-__global__ void __launch_bounds__(FOLD_NT)
+template <int ACC, int CH>
+__global__ void __launch_bounds__(32 * CH)
 rbi_cached_fold_kernel(int64_t w, int G, const float *__restrict__ part, float *__restrict__ out, float S) {
     const int64_t k = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
-    const float p = fold_partials<ACC>(w, G, part, k, S);
+    const float p = fold_partials<ACC, CH>(w, G, part, k, S);
     if (threadIdx.x < 32 && k < w) out[k] = p;
 }
 
@@ -1152,10 +1155,14 @@ static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *i
                        ? run_cached<ACC_MUL, false>(n, w, is, vs, part, nullptr, S, &G, stream)
                        : run_cached<ACC_SATADD, false>(n, w, is, vs, part, nullptr, S, &G, stream);
     if (rc != VJP_OK) return rc;
-    if (code == VJP_OP_MUL)
-        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL><<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, part, hist, S);
-    else
-        VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD><<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, part, hist, S);
+    const bool wide = fold_chains(G) == 32;
+    if (code == VJP_OP_MUL) {
+        if (wide) VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL, 32><<<fold_grid(w), 1024, 0, stream>>>(w, G, part, hist, S);
+        else VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_MUL, 8><<<fold_grid(w), 256, 0, stream>>>(w, G, part, hist, S);
+    } else {
+        if (wide) VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD, 32><<<fold_grid(w), 1024, 0, stream>>>(w, G, part, hist, S);
+        else VJP_LAUNCH(K_CACHED_FOLD, stream) rbi_cached_fold_kernel<ACC_SATADD, 8><<<fold_grid(w), 256, 0, stream>>>(w, G, part, hist, S);
+    }
     return last_launch_status();
 }
 
@@ -1167,12 +1174,13 @@ static int launch_cached_primal(int code, int64_t n, int64_t w, const int64_t *i
 // Per bin: fold the G partial products (fixed order: deterministic), expose (zeros, prod_nz), and
 // prepare the return sweep's coefficient c_k = prod_nz_k * hist_bar_k with the zero count clamped
 // to {0, 1, 2}.
-__global__ void __launch_bounds__(FOLD_NT)
+template <int CH>
+__global__ void __launch_bounds__(32 * CH)
 rbi_mul_finish_kernel(int64_t w, int G, const float *__restrict__ part,
                       const unsigned *__restrict__ zeros_u, const float *__restrict__ hist_bar,
                       int64_t *zeros, float *prod_nz, float2 *coef) {
     const int64_t k = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
-    const float p = fold_partials<ACC_MUL>(w, G, part, k, 0.f);
+    const float p = fold_partials<ACC_MUL, CH>(w, G, part, k, 0.f);
     if (threadIdx.x < 32 && k < w) {
         const unsigned z = zeros_u[k];
         if (zeros) zeros[k] = (int64_t)z;
@@ -1251,8 +1259,12 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     int G = 0;
     const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream);
     if (rc != VJP_OK) return rc;
-    VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<<<fold_grid(w), FOLD_NT, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
-                                                  vs_bar ? m.coef : nullptr);
+    if (fold_chains(G) == 32)
+        VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<32><<<fold_grid(w), 1024, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
+                                                                                              vs_bar ? m.coef : nullptr);
+    else
+        VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<8><<<fold_grid(w), 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
+                                                                                            vs_bar ? m.coef : nullptr);
     if (vs_bar && n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         const size_t bytes = (size_t)w * sizeof(float2);
