@@ -234,6 +234,25 @@ VJP_DEVINL typename M::State lookback_warp(const TileSlots<typename M::State> &t
     return acc;
 }
 
+// L2 prefetch of the tile that will be processed `dist` tiles later (dist = the number of co-resident CTAs, i.e. the
+// tile this CTA's successor on the same SM will get from the ticket counter).  With one or two CTAs per SM a tile's load,
+// scan, look-back and store phases do not overlap; the prefetch keeps HBM busy during the other phases and turns the
+// next load into L2 hits.  One bulk instruction per warp (UBLKPF takes a warp-uniform address); `bytes` of the tile
+// starting at `tile_ptr` (16-byte aligned) are split evenly over the NW warps.
+template <int NW>
+VJP_DEVINL void prefetch_tile_l2(const void *tile_ptr, int64_t bytes) {
+    const int warp = threadIdx.x >> 5;
+    const int64_t chunk = ((bytes + NW - 1) / NW + 15) & ~(int64_t)15;
+    const int64_t off = warp * chunk;
+    int64_t len = bytes - off;
+    if (len > chunk) len = chunk;
+    len &= ~(int64_t)15;
+    if ((threadIdx.x & 31) == 0 && len > 0)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(static_cast<const char *>(tile_ptr) + off),
+                     "r"((uint32_t)len)
+                     : "memory");
+}
+
 // 16 bytes of T plus 16 bytes of T (the "+=" of an accumulating VJP call, fused into the final store)
 template <class T>
 VJP_DEVINL uint4 chunk_add(const uint4 &a, const uint4 &b);

@@ -72,7 +72,7 @@ template <class Op, int NT, int IPT, bool REV, int MODE>
 __global__ void __launch_bounds__(NT)
 scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out, int64_t n,
                      int num_tiles, LookbackWs<typename Op::Fwd> ws,
-                     typename Op::Fwd *__restrict__ fpre, int accumulate) {
+                     typename Op::Fwd *__restrict__ fpre, int accumulate, int pf_dist) {
     using M = FwdMonoid<Op>;
     using S = typename Op::Fwd;
     constexpr int EW = Op::EW, RW = IPT * EW;
@@ -91,6 +91,10 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
     const int t = REV ? num_tiles - 1 - p : p;
     const int64_t base = (int64_t)t * (NT * IPT);
     const int valid = (int)min((int64_t)(NT * IPT), n - base);
+    if (pf_dist > 0 && p + pf_dist < num_tiles) {
+        const int64_t b2 = (int64_t)(REV ? t - pf_dist : t + pf_dist) * (NT * IPT);
+        prefetch_tile_l2<NT / 32>(in + b2 * EW, min((int64_t)(NT * IPT), n - b2) * EW * 4);
+    }
 
     uint32_t fill[EW];
     Op::identity_words(fill);
@@ -200,7 +204,7 @@ __global__ void __launch_bounds__(NT, (Op::EW <= 4 ? 1024 / NT : 1))
 scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
                         uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
                         const typename Op::Fwd *__restrict__ fpre,
-                        LookbackWs<typename RevMonoid<Op>::State> ws, int accumulate) {
+                        LookbackWs<typename RevMonoid<Op>::State> ws, int accumulate, int pf_dist) {
     using RM = RevMonoid<Op>;
     using RS = typename RM::State;
     using FM = FwdMonoid<Op>;
@@ -225,6 +229,11 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     const int64_t base = (int64_t)t * (NT * IPT);
     const int valid = (int)min((int64_t)(NT * IPT), n - base);
 
+    if (pf_dist > 0 && p + pf_dist < num_tiles) {
+        const int64_t b2 = (int64_t)(t - pf_dist) * (NT * IPT);  // a full tile: only the last one (t = num_tiles - 1) is ragged
+        prefetch_tile_l2<NT / 32>(xs + b2 * EW, (int64_t)(NT * IPT) * EW * 4);
+        prefetch_tile_l2<NT / 32>(ybar + b2 * EW, (int64_t)(NT * IPT) * EW * 4);
+    }
     uint32_t fillx[EW];
     Op::identity_words(fillx);  // identity element: u passes through unchanged
     const uint32_t filly[1] = {0u};
@@ -350,11 +359,15 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
 
 // ------------------------------------------------------------------ host side ------------
 
-template <class Op, int NT_, int IPT_, int VNT_, int VIPT_>
+template <class Op, int NT_, int IPT_, int VNT_, int VIPT_, bool PF_ = false>
 struct ScanCfg {
     using op = Op;
     static constexpr int NT = NT_, IPT = IPT_;     // plain scans
     static constexpr int VNT = VNT_, VIPT = VIPT_; // VJP: forward tile prefixes + fused reverse
+    // L2 prefetch of the tile the CTA's successor will take (prefetch_tile_l2): helps where a tile spends a long time
+    // away from HBM (matrix operators, min / max: -3 to -5 %), costs 2 % on the scalar operators that are closest to
+    // the HBM roofline ('*' f64, linrec), is neutral for '+'
+    static constexpr bool PF = PF_;
 };
 
 template <class Op, int NT, int IPT>
@@ -374,7 +387,15 @@ static size_t vjp_smem_bytes() {
 
 static int64_t tiles_of(int64_t n, int tile) { return (n + tile - 1) / tile; }
 
-template <class Op, int NT, int IPT, bool REV, int MODE>
+// Number of CTAs of `kern` that are resident on the whole GPU = the distance (in tiles) of the L2 prefetch.
+template <class K>
+static int resident_ctas(K kern, int nt, size_t smem) {
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, nt, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    return per_sm * NUM_SMS_B200;
+}
+
+template <class Op, int NT, int IPT, bool REV, int MODE, bool PF = false>
 static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre, char *ws,
                     int accumulate, cudaStream_t stream) {
     using S = typename Op::Fwd;
@@ -387,9 +408,11 @@ static int run_scan(int64_t n, const void *in, void *out, typename Op::Fwd *fpre
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
+    static const int resident = resident_ctas(kern, NT, smem);
     VJP_LAUNCH(MODE == MODE_SCAN ? K_SCAN_LOOKBACK : K_SCAN_TILEAGG, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(in),
-                                             static_cast<uint32_t *>(out), n, (int)nt, lw, fpre, accumulate);
+                                             static_cast<uint32_t *>(out), n, (int)nt, lw, fpre, accumulate,
+                                             PF ? resident : 0);
     return last_launch_status();
 }
 
@@ -415,13 +438,14 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     using FS = typename Op::Fwd;
     using RS = typename RevMonoid<Op>::State;
     constexpr int NT = Cfg::VNT, IPT = Cfg::VIPT;
+    constexpr bool PF = Cfg::PF;
     const int64_t nt = tiles_of(n, NT * IPT);
     char *ws_fwd = ws;
     char *ws_rev = ws_fwd + lookback_bytes<FS>(nt);
     FS *fpre = reinterpret_cast<FS *>(ws_rev + lookback_bytes<RS>(nt));
     // (A) forward tile prefixes: streaming per-tile aggregates, then their exclusive scan by one cluster
     int rc;
-    rc = run_scan<Op, NT, IPT, false, MODE_TILEAGG>(n, xs, nullptr, fpre, ws_fwd, 0, stream);
+    rc = run_scan<Op, NT, IPT, false, MODE_TILEAGG, Cfg::PF>(n, xs, nullptr, fpre, ws_fwd, 0, stream);
     if (rc != VJP_OK) return rc;
     constexpr int XNT = sizeof(FS) > 32 ? 128 : 512;
     cudaLaunchConfig_t cfg = {};
@@ -447,10 +471,11 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
     if (smem > 48 * 1024 &&
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return VJP_ERR_CUDA;
+    static const int resident = resident_ctas(kern, NT, smem);
     VJP_LAUNCH(K_SCAN_VJP_REVERSE, stream)
     kern<<<(unsigned)nt, NT, smem, stream>>>(static_cast<const uint32_t *>(xs),
                                              static_cast<const uint32_t *>(ys_bar),
-                                             static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw, accumulate);
+                                             static_cast<uint32_t *>(xs_bar), n, (int)nt, fpre, lw, accumulate, PF ? resident : 0);
     return last_launch_status();
 }
 
@@ -460,11 +485,11 @@ using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
-using CfgMinF32 = ScanCfg<OpMinMax<float, false>, 512, 32, 512, 16>;
-using CfgMaxF32 = ScanCfg<OpMinMax<float, true>, 512, 32, 512, 16>;
-using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8>;
-using CfgMat3 = ScanCfg<OpMatMul<3, float, double, float>, 256, 8, 256, 6>;  // f64 forward products, as 2x2 (Q27)
-using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3>;
+using CfgMinF32 = ScanCfg<OpMinMax<float, false>, 512, 32, 512, 16, true>;
+using CfgMaxF32 = ScanCfg<OpMinMax<float, true>, 512, 32, 512, 16, true>;
+using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8, true>;
+using CfgMat3 = ScanCfg<OpMatMul<3, float, double, float>, 256, 8, 256, 6, true>;  // f64 forward products, as 2x2 (Q27)
+using CfgMat5 = ScanCfg<OpMatMul<5, float, float, float>, 128, 5, 256, 3, true>;
 
 #define VJP_SCAN_DISPATCH(code, dtype, F, FAIL)                                              \
     switch (code) {                                                                          \
@@ -501,7 +526,7 @@ size_t scan_workspace_bytes(int code, int dtype, int64_t n) {
 
 int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys, void *ws,
                         cudaStream_t stream) {
-#define F(C) return run_scan<typename C::op, C::NT, C::IPT, false, MODE_SCAN>(n, xs, ys, nullptr, (char *)ws, 0, stream);
+#define F(C) return run_scan<typename C::op, C::NT, C::IPT, false, MODE_SCAN, C::PF>(n, xs, ys, nullptr, (char *)ws, 0, stream);
     VJP_SCAN_DISPATCH(code, dtype, F, return VJP_ERR_UNSUPPORTED;)
 #undef F
     return VJP_ERR_UNSUPPORTED;
