@@ -77,8 +77,11 @@ typedef struct {
     int32_t dtype;         /* vjp_dtype_t of xs / vs and of every real-valued output          */
     double param;          /* S for VJP_OP_SATADD, ignored otherwise                          */
     int32_t force_general; /* reduce-by-index only: != 0 routes '+', '*', min, max through the
-                              general rule (sort + segmented scans, Fig. 4) instead
-                              of their specialisation                            */
+                              general rule (eq. 5) instead of their specialisation
+                              (P:L412-416).  1: the library picks how l_i and r_i are computed
+                              (see vjp_reduce_by_index); 2: Fig. 4 as written: sort
+                              + segmented scans.  SATADD always takes the general rule; for it
+                              0 and 1 mean the same                                           */
     int32_t accumulate;    /* VJP calls only: != 0 adds the contribution to the output instead of
                               overwriting it               */
 } vjp_op_t;
@@ -139,9 +142,16 @@ int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, con
  *   MUL:      lifted primal (zero count, product of non-zeros) (Fig. 3),
  *             then the three-way map of P:L208-219 / P:L243-246.  num_bins <= 2^20, else
  *             VJP_ERR_UNSUPPORTED (force_general handles any num_bins).
- *   SATADD or force_general: stable radix sort by clamped bin, forward and reverse segmented
- *             exclusive scans, per-element derivative of l (.) x (.) r, un-permute
- *             (Fig. 4, eq. 5).
+ *   SATADD or force_general: the general rule, eq. 5:
+ *             vs_bar_i = d(l_i (.) x (.) r_i)/dx at vs_i * hist_bar[is_i], l_i / r_i = the fold of the
+ *             same-bin values before / after i.  Two routes to l and r, same results:
+ *             - num_bins <= 4096 and force_general != 2: no sort.  Two in-order walks over the input,
+ *               each warp with a running per-bin table in shared memory (forward: l, backward: r),
+ *               per-chunk carries scanned in between; every array is read and written in its
+ *               original order (36 bytes per element).
+ *             - otherwise (or force_general == 2): Fig. 4 as written: stable radix sort
+ *               by clamped bin, forward and reverse segmented exclusive scans, derivative, un-permute.
+ *             min / max give the adjoint of tied extrema to the lowest index on both routes.
  * n must be < 2^32 - 1 (packed 32-bit positions). */
 int vjp_reduce_by_index(const vjp_op_t *op, int64_t n, int64_t num_bins, const int64_t *is,
                         const void *vs, const void *hist_bar, void *vs_bar,
@@ -213,8 +223,9 @@ int rbi_sumofprod_forward(int64_t n, int64_t num_bins, const int64_t *is, const 
  *   use_general == 0: the invertible-operator rule of Fig. 6: xs = the primal histogram,
  *                     b_i = xs[k_i] sumOfProd_inv v_i, vs_bar_i = (d(b_i (.) x)/dx)^T hist_bar[k_i]
  *                     -- a histogram and a map.
- *   use_general != 0: the general rule of Fig. 4 (sort by bin, forward and reverse segmented scans, eq. 5)
- *                     for the same operator -- the paper's 8 - 92x against 1.1 - 2.1x contrast.
+ *   use_general != 0: the general rule (eq. 5) for the same operator -- the paper's 8 - 92x against
+ *                     1.1 - 2.1x contrast.  1: route picked as in vjp_reduce_by_index (no sort
+ *                     for num_bins <= 4096); 2: Fig. 4 as written (sort by bin + segmented scans).
  * accumulate != 0 adds to vs_bar.  Keys outside [0, num_bins) get (0, 0). */
 int vjp_rbi_sumofprod(int64_t n, int64_t num_bins, const int64_t *is, const float *vs,
                       const float *hist_bar, float *vs_bar, int use_general, int accumulate,

@@ -160,16 +160,19 @@ def to_pinned(a):
 C2_CELLS = [(op, w, dist) for op in ("min", "mul") for w in (1 << 10, 1 << 16) for dist in ("uniform", "zipf")]
 VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (roofline table)
     "c1_rbi_add": 12, "c2_rbi_min": 16, "c2_rbi_mul": 28, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 32,
-    "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400, "c5_rbi_satadd": 88,
+    "c3_scan_linrec_f32": 32, "c4_scan_matmul2": 64, "c4_scan_matmul5": 400,
+    # general rule: sort-free walks = forward (is 8 + vs 4 read, l 4 written) + backward (is 8 + vs 4 + l 4 read, 4 written);
+    # sort-based (Fig. 4 as written) = the budget of SURVEY.md 8(d)
+    "c5_rbi_satadd": 36, "c5_rbi_satadd_sorted": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
     "f4_scan_matmul3": 144, "f4_scan_min": 16,
     "f3_rbi_vec_mul": 16 + 28 * 4,   # per ROW of d = 4: two transposes (read + write 4 d each way) + d scalar '*' VJPs at 28 B
-    "f1_sop_inv": 40, "f1_sop_general": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
+    "f1_sop_inv": 40, "f1_sop_general": 40, "f1_sop_general_sorted": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
-    "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12,
-    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16, "f3_rbi_vec_mul": 8 + 4 * 4,
+    "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12, "c5_rbi_satadd_sorted": 12,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16, "f1_sop_general_sorted": 16, "f3_rbi_vec_mul": 8 + 4 * 4,
 }
 
 
@@ -316,7 +319,7 @@ def case_table(scale=1.0):
     def rbi(opname, gen, **kw):
         def make():
             d = gen()
-            return RbiCase(B.Op.of(opname, **({"S": d["S"]} if opname == "satadd" else {})), d)
+            return RbiCase(B.Op.of(opname, **({"S": d["S"]} if opname == "satadd" else {}), **kw), d)
         return make
 
     def scan(opname, gen, dtype=None):
@@ -342,13 +345,16 @@ def case_table(scale=1.0):
          scan("matmul2", lambda: W.c4_scan_matmul(2, n=sz(W.FULL["c4"]["n2"])))),
         ("c4_scan_matmul5", "c4 scan matmul 5x5 f32",
          scan("matmul5", lambda: W.c4_scan_matmul(5, n=sz(W.FULL["c4"]["n5"])))),
-        ("c5_rbi_satadd", "c5 rbi satadd (general rule) f32 w=4096",
+        ("c5_rbi_satadd", "c5 rbi satadd (general rule, sort-free walks) f32 w=4096",
          rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])))),
+        ("c5_rbi_satadd_sorted", "c5 rbi satadd (general rule as Fig. 4: sort + segmented scans) f32 w=4096",
+         rbi("satadd", lambda: W.c5_rbi_satadd(n=sz(W.FULL["c5"]["n"])), force_general=2)),
     ]
     t.append(("f3_rbi_vec_mul", "f3 rbi map2(*) d=4 n=2^22 rows w=1024 (NEXT row)", lambda: VecCase(W.f3_rbi_vec("mul", n=sz(1 << 22)))))
-    for general in (False, True):  # NEXT row f1: the same data through both rules
-        t.append(("f1_sop_general" if general else "f1_sop_inv",
-                  "f1 rbi sumOfProd w=1024 uniform, %s (NEXT row)" % ("general rule" if general else "invertible rule"),
+    for general in (0, 1, 2):  # NEXT row f1: the same data through both rules
+        t.append((("f1_sop_inv", "f1_sop_general", "f1_sop_general_sorted")[general],
+                  "f1 rbi sumOfProd w=1024 uniform, %s (NEXT row)" % (
+                      "invertible rule", "general rule, sort-free walks", "general rule as Fig. 4 (sort)")[general],
                   lambda general=general: SopCase(W.f1_rbi_sumofprod(n=sz(1 << 24)), general)))
     t.append(("f4_scan_matmul3", "f4 scan matmul 3x3 f32 n=2^22 (NEXT row)",
               scan("matmul3", lambda: W.c4_scan_matmul(3, n=sz(1 << 22)))))

@@ -50,13 +50,13 @@ class Op:
     code: int
     dtype: int = F32
     param: float = 0.0
-    force_general: bool = False
+    force_general: int = 0     # 1: the general rule (eq. 5), route chosen by the library; 2: its sort-based form (Fig. 4)
     accumulate: bool = False   # VJP calls: out += contribution (the paper's "+=") instead of out = contribution
 
     @staticmethod
-    def of(name: str, dtype=torch.float32, S: float = 0.0, force_general: bool = False,
+    def of(name: str, dtype=torch.float32, S: float = 0.0, force_general: int = 0,
            accumulate: bool = False) -> "Op":
-        return Op(OPCODES[name], F64 if dtype in (torch.float64, F64) else F32, float(S), bool(force_general),
+        return Op(OPCODES[name], F64 if dtype in (torch.float64, F64) else F32, float(S), int(force_general),
                   bool(accumulate))
 
     def c(self) -> _OpStruct:
@@ -418,9 +418,11 @@ def rbi_sumofprod_forward(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ou
     return hist.view(num_bins, 2)
 
 
-def vjp_rbi_sumofprod(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, hist_bar: torch.Tensor, general: bool = False,
+def vjp_rbi_sumofprod(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, hist_bar: torch.Tensor, general: int = 0,
                       accumulate: bool = False, out=None, ws=None, stream=None):
-    """vs_bar [n, 2] by the invertible-operator rule (Fig. 6) or, general=True, by sort + segmented scans (Fig. 4)."""
+    """vs_bar [n, 2] by the invertible-operator rule (Fig. 6) or by the general rule (eq. 5): general=1 lets the
+    library choose the route (sort-free when the bin table fits a warp's shared memory), general=2 is Fig. 4 as
+    written (sort + segmented scans)."""
     is_ = _dev(is_, torch.int64, what="is")
     n = is_.numel()
     vs = _dev(vs, torch.float32, 2 * n, "vs")

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libvjp_b200.so")
-SOURCES = ["api.cu", "scan_kernels.cu", "rbi_kernels.cu", "rbi_general.cu", "reduce_kernels.cu", "rbi_sumofprod.cu", "vec_rules.cu"]
+SOURCES = ["api.cu", "scan_kernels.cu", "rbi_kernels.cu", "rbi_general.cu", "rbi_multiscan.cu", "reduce_kernels.cu", "rbi_sumofprod.cu", "vec_rules.cu"]
 # no --use_fast_math: flush-to-zero would change the v == 0 test of the '*' rule (Q7)
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]

@@ -62,7 +62,8 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "sort_hist_kernel", "u32_exclusive_scan_kernel", "sort_scatter_kernel", "seg_forward_kernel",
     "seg_reverse_vjp_kernel", "sort_export_kernel",
     "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel",
-    "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel", "rows_to_cols / cols_to_rows"};
+    "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel", "rows_to_cols / cols_to_rows",
+    "ms_forward_kernel", "ms_seg_agg / ms_carry_kernel", "ms_backward_kernel"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];
@@ -258,7 +259,7 @@ int vjp_reduce_by_index(const vjp_op_t *op, int64_t n, int64_t num_bins, const i
         return launch_rbi_general_vjp(op->code, op->param, n, num_bins, is,
                                       static_cast<const float *>(vs),
                                       static_cast<const float *>(hist_bar),
-                                      static_cast<float *>(vs_bar), ws, acc, s);
+                                      static_cast<float *>(vs_bar), ws, acc, op->force_general == 2, s);
     }
 }
 
@@ -469,7 +470,7 @@ int vjp_rbi_sumofprod(int64_t n, int64_t num_bins, const int64_t *is, const floa
         return VJP_ERR_INVALID_ARG;
     if (ws_bytes < rbi_sumofprod_workspace_bytes(n, num_bins, use_general)) return VJP_ERR_WORKSPACE;
     if (use_general)
-        return launch_rbi_sop_general_vjp(n, num_bins, is, vs, hist_bar, vs_bar, ws, accumulate != 0, as_stream(stream));
+        return launch_rbi_sop_general_vjp(n, num_bins, is, vs, hist_bar, vs_bar, ws, accumulate != 0, use_general == 2, as_stream(stream));
     return launch_rbi_sop_vjp_inv(n, num_bins, is, vs, hist_bar, vs_bar, ws, accumulate != 0, as_stream(stream));
 }
 

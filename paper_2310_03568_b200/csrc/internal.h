@@ -30,6 +30,7 @@ enum KernelId : int {
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
     K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP, K_VEC_TRANSPOSE,
+    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -71,7 +72,12 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
 size_t rbi_general_workspace_bytes(int64_t n, int64_t w);
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
                            const float *vs, const float *hist_bar, float *vs_bar, void *ws,
-                           int accumulate, cudaStream_t stream);
+                           int accumulate, int sorted, cudaStream_t stream);
+// the sort-free route (rbi_multiscan.cu); gcode = G_ADD ... G_SOP of gen_ops.cuh
+bool rbi_multiscan_fits(int64_t w);
+size_t rbi_multiscan_workspace_bytes(int64_t n, int64_t w);
+int launch_rbi_multiscan_vjp(int gcode, double param, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                             const float *hist_bar, float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,
                          int64_t *perm, void *ws, cudaStream_t stream);
 
@@ -87,7 +93,7 @@ int launch_rbi_sop_forward(int64_t n, int64_t w, const int64_t *is, const float 
 int launch_rbi_sop_vjp_inv(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
                            float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
 int launch_rbi_sop_general_vjp(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
-                               float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
+                               float *vs_bar, void *ws, int accumulate, int sorted, cudaStream_t stream);
 
 // ----------------------------------------------------------------------------- reduce ---
 size_t reduce_special_workspace_bytes();

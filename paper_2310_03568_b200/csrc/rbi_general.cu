@@ -17,6 +17,7 @@
 #include <math_constants.h>
 
 #include "common.cuh"
+#include "gen_ops.cuh"
 #include "internal.h"
 
 namespace vjp {
@@ -309,45 +310,7 @@ sort_scatter_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
 }
 
-// ------------------------------------------------------------------ operators -------------
-
-// G_SOP: sumOfProd.  Of l (.) x (.) r only the s components enter the derivative with respect to x
-// (d yp / d xs = ls + rs), so the segmented scans carry s alone, under '+'; the output is a pair.
-enum : int { G_ADD = 0, G_MIN = 1, G_MAX = 2, G_MUL = 3, G_SATADD = 4, G_SOP = 5 };
-
-// The operator, its neutral element, and d/dx of (l (.) x) (.) r at x = v (eq. 5).
-template <int CODE>
-struct GenOp {
-    float S;
-    VJP_DEVINL float neutral() const {
-        return CODE == G_MUL ? 1.f : CODE == G_MIN ? CUDART_INF_F : CODE == G_MAX ? -CUDART_INF_F : 0.f;
-    }
-    VJP_DEVINL float apply(float a, float b) const {
-        switch (CODE) {
-        case G_ADD: return a + b;
-        case G_SOP: return a + b;
-        case G_MUL: return a * b;
-        case G_MIN: return b < a ? b : a;
-        case G_MAX: return b > a ? b : a;
-        default: return fminf(a + b, S);
-        }
-    }
-    // min / max: the accumulated (left) operand wins ties, so among equal extrema the lowest index
-    // gets the adjoint, as with min^L.  satadd: slope 1 strictly below S (Q17).
-    VJP_DEVINL float dfdx(float l, float v, float r) const {
-        switch (CODE) {
-        case G_ADD: return 1.f;
-        case G_SOP: return l + r;
-        case G_MUL: return l * r;
-        case G_MIN: return (v < l && !(r < v)) ? 1.f : 0.f;
-        case G_MAX: return (v > l && !(r > v)) ? 1.f : 0.f;
-        default: {
-            const float s = l + v;
-            return (s < S && s + r < S) ? 1.f : 0.f;
-        }
-        }
-    }
-};
+// ------------------------------------------------------------------ operators: gen_ops.cuh
 
 // Segmented-scan combine on payloads (flag << 32 | value bits).  REV: "earlier" holds the HIGHER
 // indices, and the fold keeps index order: value = later (.) earlier.
@@ -582,7 +545,11 @@ static GenWs gen_carve(void *ws, int64_t n) {
     return g;
 }
 
-size_t rbi_general_workspace_bytes(int64_t n, int64_t) { return gen_carve(nullptr, n).total; }
+// one query serves both routes of the general rule (sort-based: here; sort-free: rbi_multiscan.cu)
+size_t rbi_general_workspace_bytes(int64_t n, int64_t w) {
+    const size_t a = gen_carve(nullptr, n).total, b = rbi_multiscan_workspace_bytes(n, w);
+    return a > b ? a : b;
+}
 
 // Sorts (clamped key, (index, value)); returns the buffer index holding the result in *out_buf.
 static int run_sort(int64_t n, int64_t w, const int64_t *is, const float *vs, const GenWs &g,
@@ -653,8 +620,10 @@ static int run_general(float S, int64_t n, int64_t w, const int64_t *is, const f
 // sumOfProd through the general rule (Fig. 4): sort by bin with the s component as payload, segmented exclusive
 // '+' scans of s forwards and backwards, vs_bar_i = (Pbar, Pbar * (ls_i + rs_i) + Sbar).
 int launch_rbi_sop_general_vjp(int64_t n, int64_t w, const int64_t *is, const float *vs, const float *hist_bar,
-                               float *vs_bar, void *ws, int accumulate, cudaStream_t stream) {
+                               float *vs_bar, void *ws, int accumulate, int sorted, cudaStream_t stream) {
     if (n == 0) return VJP_OK;
+    if (!sorted && rbi_multiscan_fits(w))
+        return launch_rbi_multiscan_vjp(G_SOP, 0.0, n, w, is, vs, hist_bar, vs_bar, ws, accumulate, stream);
     const GenWs g = gen_carve(ws, n);
     int buf;
     const int rc = run_sort(n, w, is, vs + 1, g, &buf, stream, 2);
@@ -690,10 +659,24 @@ int launch_reduce_general_vjp(int code, double param, int64_t n, const float *xs
     }
 }
 
+// sorted != 0: Fig. 4 as written (sort + segmented scans); else the sort-free walks of rbi_multiscan.cu when a bin
+// table fits a warp's shared memory (w <= 4096), the sort-based route otherwise.
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
                            const float *vs, const float *hist_bar, float *vs_bar, void *ws,
-                           int accumulate, cudaStream_t stream) {
+                           int accumulate, int sorted, cudaStream_t stream) {
     if (n == 0) return VJP_OK;
+    if (!sorted && rbi_multiscan_fits(w)) {
+        int gc;
+        switch (code) {
+        case VJP_OP_ADD: gc = G_ADD; break;
+        case VJP_OP_MIN: gc = G_MIN; break;
+        case VJP_OP_MAX: gc = G_MAX; break;
+        case VJP_OP_MUL: gc = G_MUL; break;
+        case VJP_OP_SATADD: gc = G_SATADD; break;
+        default: return VJP_ERR_UNSUPPORTED;
+        }
+        return launch_rbi_multiscan_vjp(gc, param, n, w, is, vs, hist_bar, vs_bar, ws, accumulate, stream);
+    }
     const GenWs g = gen_carve(ws, n);
     const float S = (float)param;
     switch (code) {

@@ -1,0 +1,415 @@
+// rbi_multiscan.cu -- the general-case rule for reduce-by-index (eq. 5) WITHOUT the sort:
+//
+//   vs_bar_i = d(l_i (.) x (.) r_i)/dx at x = vs_i  *  hist_bar[is_i],
+//   l_i = fold of the same-bin values BEFORE i,   r_i = fold of the same-bin values AFTER i
+//
+// Fig. 4 gets l and r by sorting (key, iota) and running two segmented scans over the sorted values:
+// six passes over n-sized arrays, two of them scatters, and a random un-permute at the end (rbi_general.cu; the paper
+// itself reports that the sort dominates).  The sort is only a means: what eq. 5 needs is, per element,
+// the per-bin exclusive folds in index order.  When a bin table fits a warp's share of shared memory (w <= 4096 f32
+// states = 16 KB: the C5 workload) they come from two in-order walks with a RUNNING per-bin table, with no data movement
+// at all -- every array is read and written in its original order, fully coalesced:
+//
+//   forward   each warp owns a contiguous chunk of the input and a private table tab[w] (neutral-initialised).  Per row
+//             of 32 consecutive elements: lanes holding the same bin are found with match.any; an exclusive fold along
+//             each such group in lane (= index) order by pointer jumping; l_local_i = tab[bin] (.) that fold; the last
+//             lane of the group stores the group's inclusive fold back.  l_local -> global (4 B / element); at the end of
+//             the chunk the table IS the chunk's per-bin aggregate -> agg[chunk][w].
+//   carry     per bin, exclusive prefix L[chunk][bin] and exclusive suffix R[chunk][bin] of agg over the chunks (a
+//             few thousand chunks x w bins; two-level: segments of <= 32 chunks held in registers).
+//   backward  the same walk from the end of the chunk towards its start, table initialised with R[chunk][.]: gives
+//             r_i directly; l_i = L[chunk][bin] (.) l_local_i; then the derivative and the store of vs_bar_i in place
+//             (original order: no scatter).  Out-of-range keys take no part and get 0.
+//             The operator is commutative, so d(l (.) x (.) r)/dx depends on l and r only through l (.) r:
+//             for every operator but min / max the table starts as L[chunk][.] (.) R[chunk][.] and l_local stands
+//             for l -- no per-element gather of L (16 M random L2 reads cost 158 us at w = 4096, more than the rest
+//             of the kernel).  min / max break ties by index ("v < l" strict, "r < v" not), so they keep the gather.
+//             hist_bar sits in shared memory next to the tables (its gather from L1 / L2 cost another 48 us).
+//
+// Index order matters beyond associativity only for min / max, whose ties give the adjoint to the lowest index
+// (P:L425-428): rows are 32 CONSECUTIVE elements and chunks are contiguous, so "before" is always the true index order.
+// Traffic: forward 12 B read + 4 B written per element, backward 16 B read + 4 B written: 36 B / element against
+// ~90 B for the sort-based route.
+#include "gen_ops.cuh"
+#include "internal.h"
+
+namespace vjp {
+
+constexpr size_t MS_SMEM_BUDGET = 224 * 1024;  // warp tables of one CTA
+constexpr int MS_W_MAX = 4096;                 // bins (one f32 state each) a warp-private table may hold
+constexpr int MS_SEG = 32;                     // chunks per carry segment (held in registers)
+constexpr int MS_MIN_ROWS = 8;                 // do not split the input finer than this many rows per warp
+
+bool rbi_multiscan_fits(int64_t w) { return w >= 1 && w <= MS_W_MAX; }
+
+// shared memory of a CTA: hist_bar (hw words per bin: 2 for the pairs of sumOfProd) + one table of w floats per warp
+static int ms_warps_per_cta(int64_t w, int hw) {
+    const int fit = (int)((MS_SMEM_BUDGET - (size_t)w * 4 * hw) / ((size_t)w * 4));
+    return fit > 32 ? 32 : fit;
+}
+
+struct MsShape {
+    int wpc, grid;
+    int64_t G, R, segs;  // chunks (warps), rows per chunk, carry segments
+};
+static MsShape ms_shape(int64_t n, int64_t w, int hw) {
+    MsShape s;
+    s.wpc = ms_warps_per_cta(w, hw);
+    const int64_t rows = (n + 31) / 32;
+    int64_t want = (rows + MS_MIN_ROWS - 1) / MS_MIN_ROWS;
+    const int64_t cap = (int64_t)NUM_SMS_B200 * s.wpc;
+    if (want > cap) want = cap;
+    if (want < 1) want = 1;
+    s.grid = (int)((want + s.wpc - 1) / s.wpc);
+    s.G = (int64_t)s.grid * s.wpc;
+    s.R = (rows + s.G - 1) / s.G;
+    if (s.R < 1) s.R = 1;
+    s.segs = (s.G + MS_SEG - 1) / MS_SEG;
+    return s;
+}
+
+// A cell of a warp's table doubles as its claim word while a row is in flight: NaN-boxed lane id (no operator result is
+// a NaN for NaN-free input; NaN input is undefined, include/vjp_b200.h).
+constexpr uint32_t MS_CLAIM = 0xfff00000u;
+
+// One row of the forward walk.  Returns l_local (table (.) earlier same-bin lanes) and updates the table.
+// match.any runs on the ADU pipe at ~75 cycles per warp instruction (profiles/r2c_multiscan.txt: that pipe 91 % busy
+// when every row used it), so the row first finds out through the table itself whether any two lanes share a bin:
+// every lane reads its cell, then stores its claim, then reads it back; if nobody lost, each lane is alone in its bin
+// and the row is a plain read-modify-write (89 % of the rows at w = 4096 with uniform keys).  Otherwise the lanes of
+// a bin are grouped with match.any and folded in lane order by pointer jumping.
+template <int CODE>
+VJP_DEVINL float ms_row_forward(const GenOp<CODE> &op, float *tab, int64_t k, float x, int64_t w, int lane) {
+    const bool inr = (uint64_t)k < (uint64_t)w;
+    const uint32_t key = inr ? (uint32_t)k : (0x80000000u | (uint32_t)lane);  // out of range: a group of its own
+    uint32_t *tabu = reinterpret_cast<uint32_t *>(tab);
+    const float t = inr ? tab[key] : op.neutral();
+    __syncwarp();  // every lane has read its cell
+    if (inr) tabu[key] = MS_CLAIM | (uint32_t)lane;
+    __syncwarp();
+    const bool lost = inr && tabu[key] != (MS_CLAIM | (uint32_t)lane);
+    if (!__any_sync(FULL_MASK, lost)) {
+        if (inr) tab[key] = op.apply(t, x);
+        __syncwarp();
+        return t;
+    }
+    const uint32_t m = __match_any_sync(FULL_MASK, key);
+    const uint32_t lower = m & ((1u << lane) - 1u);
+    const int prev0 = lower ? 31 - __clz(lower) : -1;
+    float inc = x;  // fold over (pj, lane] along the group's list
+    int pj = prev0;
+    while (__any_sync(FULL_MASK, pj >= 0)) {
+        const int src = pj < 0 ? lane : pj;
+        const float pv = __shfl_sync(FULL_MASK, inc, src);
+        const int pp = __shfl_sync(FULL_MASK, pj, src);
+        if (pj >= 0) {
+            inc = op.apply(pv, inc);
+            pj = pp;
+        }
+    }
+    const float exv = __shfl_sync(FULL_MASK, inc, prev0 < 0 ? lane : prev0);
+    const float l = prev0 < 0 ? t : op.apply(t, exv);
+    const bool last = (m & (0xfffffffeu << lane)) == 0u;
+    if (inr & last) tab[key] = op.apply(t, inc);  // replaces the claim: every bin of the row has one last lane
+    __syncwarp();
+    return l;
+}
+
+// One row of the backward walk.  Returns r (later same-bin lanes (.) table) and updates the table.
+template <int CODE>
+VJP_DEVINL float ms_row_backward(const GenOp<CODE> &op, float *tab, int64_t k, float x, int64_t w, int lane) {
+    const bool inr = (uint64_t)k < (uint64_t)w;
+    const uint32_t key = inr ? (uint32_t)k : (0x80000000u | (uint32_t)lane);
+    uint32_t *tabu = reinterpret_cast<uint32_t *>(tab);
+    const float t = inr ? tab[key] : op.neutral();
+    __syncwarp();
+    if (inr) tabu[key] = MS_CLAIM | (uint32_t)lane;
+    __syncwarp();
+    const bool lost = inr && tabu[key] != (MS_CLAIM | (uint32_t)lane);
+    if (!__any_sync(FULL_MASK, lost)) {
+        if (inr) tab[key] = op.apply(x, t);
+        __syncwarp();
+        return t;
+    }
+    const uint32_t m = __match_any_sync(FULL_MASK, key);
+    const uint32_t higher = m & (0xfffffffeu << lane);
+    const int next0 = higher ? __ffs(higher) - 1 : -1;
+    float suf = x;  // fold over [lane, nj) along the group's list
+    int nj = next0;
+    while (__any_sync(FULL_MASK, nj >= 0)) {
+        const int src = nj < 0 ? lane : nj;
+        const float sv = __shfl_sync(FULL_MASK, suf, src);
+        const int nn = __shfl_sync(FULL_MASK, nj, src);
+        if (nj >= 0) {
+            suf = op.apply(suf, sv);
+            nj = nn;
+        }
+    }
+    const float exv = __shfl_sync(FULL_MASK, suf, next0 < 0 ? lane : next0);
+    const float r = next0 < 0 ? t : op.apply(exv, t);
+    const bool first = (m & ((1u << lane) - 1u)) == 0u;
+    if (inr & first) tab[key] = op.apply(suf, t);
+    __syncwarp();
+    return r;
+}
+
+// WMAX = warps per CTA the kernel is compiled for (register budget), D = rows of loads in flight per warp.
+template <int CODE, int WMAX, int D>
+__global__ void __launch_bounds__(WMAX * 32, 1)
+ms_forward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs, int vstride,
+                  float *__restrict__ ls, float *__restrict__ agg, int64_t R, GenOp<CODE> op) {
+    extern __shared__ float ms_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    float *tab = ms_smem + (size_t)warp * (size_t)w;
+    for (int i = lane; i < (int)w; i += 32) tab[i] = op.neutral();
+    __syncwarp();
+    const int64_t g = (int64_t)blockIdx.x * wpc + warp;
+    const int64_t rows = (n + 31) >> 5;
+    const int64_t r0 = min(g * R, rows), r1 = min(r0 + R, rows);
+    int64_t kn[D];
+    float vn[D];
+    auto fetch = [&](int64_t rb) {
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            const int64_t idx = (rb + d) * 32 + lane;
+            const bool ok = (rb + d < r1) & (idx < n);
+            kn[d] = ok ? __ldg(is + idx) : (int64_t)-1;
+            vn[d] = ok ? __ldg(vs + idx * vstride) : 0.f;
+        }
+    };
+    fetch(r0);
+    for (int64_t rb = r0; rb < r1; rb += D) {
+        int64_t k[D];
+        float v[D];
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            k[d] = kn[d];
+            v[d] = vn[d];
+        }
+        fetch(rb + D);  // the next block's loads fly while this one is walked
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            if (rb + d < r1) {  // warp-uniform
+                const float l = ms_row_forward<CODE>(op, tab, k[d], v[d], w, lane);
+                const int64_t idx = (rb + d) * 32 + lane;
+                if (idx < n) ls[idx] = l;
+            }
+        }
+    }
+    __syncwarp();
+    for (int i = lane; i < (int)w; i += 32) agg[g * w + i] = tab[i];
+}
+
+template <int CODE, int WMAX, int D>
+__global__ void __launch_bounds__(WMAX * 32, 1)
+ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs, int vstride,
+                   const float *__restrict__ ls, const float *__restrict__ Lc, const float *__restrict__ Rc,
+                   const float *__restrict__ hist_bar, float *__restrict__ vs_bar, int64_t R, GenOp<CODE> op,
+                   int accumulate) {
+    extern __shared__ float ms_smem[];
+    constexpr bool SYM = CODE != G_MIN && CODE != G_MAX;  // see the header: L folded into the table
+    constexpr int HW = CODE == G_SOP ? 2 : 1;             // words of hist_bar per bin
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    float *hs = ms_smem;                                  // [w][HW]
+    float *tab = ms_smem + (size_t)w * HW + (size_t)warp * (size_t)w;
+    const int64_t g = (int64_t)blockIdx.x * wpc + warp;
+    for (int i = threadIdx.x; i < (int)w * HW; i += blockDim.x) hs[i] = hist_bar[i];
+    for (int i = lane; i < (int)w; i += 32) {
+        const float rc = Rc[g * w + i];  // what lies to the right of the chunk
+        tab[i] = SYM ? op.apply(Lc[g * w + i], rc) : rc;
+    }
+    __syncthreads();
+    const float *Lg = Lc + g * w;
+    const int64_t rows = (n + 31) >> 5;
+    const int64_t r0 = min(g * R, rows), r1 = min(r0 + R, rows);
+    // rows are walked from r1 - 1 down to r0, D at a time: block b covers rows r1 - 1 - b*D - d
+    int64_t kn[D];
+    float vn[D], ln[D];
+    auto fetch = [&](int64_t top) {  // top = highest row of the block
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            const int64_t row = top - d;
+            const int64_t idx = row * 32 + lane;
+            const bool ok = (row >= r0) & (idx < n);
+            kn[d] = ok ? __ldg(is + idx) : (int64_t)-1;
+            vn[d] = ok ? __ldg(vs + idx * vstride) : 0.f;
+            ln[d] = ok ? __ldg(ls + idx) : 0.f;
+        }
+    };
+    fetch(r1 - 1);
+    for (int64_t top = r1 - 1; top >= r0; top -= D) {
+        int64_t k[D];
+        float v[D], ll[D], lc[SYM ? 1 : D];
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            k[d] = kn[d];
+            v[d] = vn[d];
+            ll[d] = ln[d];
+        }
+        fetch(top - D);
+        if constexpr (!SYM) {
+#pragma unroll
+            for (int d = 0; d < D; d++)  // the gathers of the whole block are issued before the walk
+                lc[d] = (uint64_t)k[d] < (uint64_t)w ? __ldg(Lg + k[d]) : op.neutral();
+        }
+        // the table walk of the whole block first (shared-memory latencies only), then the outputs: by then the
+        // gathers have arrived, and a wait on them no longer sits between two rows of the (in-order) walk
+        float rr[D];
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            rr[d] = op.neutral();
+            if (top - d >= r0) rr[d] = ms_row_backward<CODE>(op, tab, k[d], v[d], w, lane);  // warp-uniform
+        }
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            const int64_t row = top - d;
+            const int64_t idx = row * 32 + lane;
+            if (row >= r0 && idx < n) {
+                const bool inr = (uint64_t)k[d] < (uint64_t)w;
+                const float l = SYM ? ll[d] : op.apply(lc[d], ll[d]);
+                const float h0 = inr ? hs[(uint32_t)k[d] * HW] : 0.f;
+                const float gq = inr ? op.dfdx(l, v[d], rr[d]) * h0 : 0.f;  // 0 out of range
+                if constexpr (CODE == G_SOP) {  // vs_bar_i = (Pbar, Pbar * (ls + rs) + Sbar)
+                    float2 *dst = reinterpret_cast<float2 *>(vs_bar) + idx;
+                    float2 o = make_float2(h0, gq + (inr ? hs[(uint32_t)k[d] * 2 + 1] : 0.f));
+                    if (accumulate) {
+                        const float2 pr = *dst;
+                        o.x += pr.x;
+                        o.y += pr.y;
+                    }
+                    *dst = o;
+                } else {
+                    vs_bar[idx] = accumulate ? vs_bar[idx] + gq : gq;
+                }
+            }
+        }
+    }
+}
+
+// Carry, level 1: segagg[seg][b] = fold of agg[g][b] over the chunks g of segment seg (in order).
+template <int CODE>
+__global__ void ms_seg_agg_kernel(int64_t w, int64_t G, const float *__restrict__ agg, float *__restrict__ segagg,
+                                  GenOp<CODE> op) {
+    const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t seg = blockIdx.y;
+    if (b >= w) return;
+    const int64_t g0 = seg * MS_SEG, g1 = min(g0 + MS_SEG, G);
+    float a[MS_SEG];
+#pragma unroll
+    for (int j = 0; j < MS_SEG; j++) a[j] = g0 + j < g1 ? __ldg(agg + (g0 + j) * w + b) : op.neutral();
+    float acc = op.neutral();
+#pragma unroll
+    for (int j = 0; j < MS_SEG; j++) acc = op.apply(acc, a[j]);
+    segagg[seg * w + b] = acc;
+}
+
+// Carry, level 2: L[g][b] (in place of agg) and R[g][b] for the chunks of one segment.
+template <int CODE>
+__global__ void ms_carry_kernel(int64_t w, int64_t G, int64_t segs, float *__restrict__ aggL, float *__restrict__ Rc,
+                                const float *__restrict__ segagg, GenOp<CODE> op) {
+    const int64_t b = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t seg = blockIdx.y;
+    if (b >= w) return;
+    const int64_t g0 = seg * MS_SEG, g1 = min(g0 + MS_SEG, G);
+    float a[MS_SEG];
+#pragma unroll
+    for (int j = 0; j < MS_SEG; j++) a[j] = g0 + j < g1 ? aggL[(g0 + j) * w + b] : op.neutral();
+    // the segments before / after this one: loads in batches of 16 (independent), folds in order
+    float pre = op.neutral(), suf = op.neutral();
+    for (int64_t s0 = 0; s0 < seg; s0 += 16) {
+        float q[16];
+#pragma unroll
+        for (int j = 0; j < 16; j++) q[j] = s0 + j < seg ? __ldg(segagg + (s0 + j) * w + b) : op.neutral();
+#pragma unroll
+        for (int j = 0; j < 16; j++) pre = op.apply(pre, q[j]);
+    }
+    for (int64_t s0 = segs - 1; s0 > seg; s0 -= 16) {
+        float q[16];
+#pragma unroll
+        for (int j = 0; j < 16; j++) q[j] = s0 - j > seg ? __ldg(segagg + (s0 - j) * w + b) : op.neutral();
+#pragma unroll
+        for (int j = 0; j < 16; j++) suf = op.apply(q[j], suf);
+    }
+#pragma unroll
+    for (int j = 0; j < MS_SEG; j++) {
+        if (g0 + j < g1) aggL[(g0 + j) * w + b] = pre;
+        pre = op.apply(pre, a[j]);
+    }
+#pragma unroll
+    for (int j = MS_SEG - 1; j >= 0; j--) {
+        if (g0 + j < g1) Rc[(g0 + j) * w + b] = suf;
+        suf = op.apply(a[j], suf);
+    }
+}
+
+// ------------------------------------------------------------------ host side -------------
+
+struct MsWs {
+    float *ls, *aggL, *Rc, *segagg;
+    size_t total;
+};
+static MsWs ms_carve(void *ws, int64_t n, int64_t w) {
+    const MsShape s = ms_shape(n < 1 ? 1 : n, w < 1 ? 1 : w, 1);  // hw = 1: the most chunks any operator uses
+    MsWs m;
+    char *p = static_cast<char *>(ws);
+    auto take = [&](size_t bytes) { char *r = p; p += align_up(bytes, 256); return r; };
+    m.ls = reinterpret_cast<float *>(take((size_t)(n < 1 ? 1 : n) * 4));
+    m.aggL = reinterpret_cast<float *>(take((size_t)s.G * (size_t)w * 4));
+    m.Rc = reinterpret_cast<float *>(take((size_t)s.G * (size_t)w * 4));
+    m.segagg = reinterpret_cast<float *>(take((size_t)s.segs * (size_t)w * 4));
+    m.total = (size_t)(p - static_cast<char *>(ws));
+    return m;
+}
+
+size_t rbi_multiscan_workspace_bytes(int64_t n, int64_t w) {
+    if (!rbi_multiscan_fits(w)) return 0;
+    return ms_carve(nullptr, n, w).total;
+}
+
+template <int CODE, int WMAX, int D>
+static int ms_run(float S, int64_t n, int64_t w, const int64_t *is, const float *vs, int vstride,
+                  const float *hist_bar, float *vs_bar, const MsWs &m, const MsShape &s, int accumulate,
+                  cudaStream_t stream) {
+    const GenOp<CODE> op{S};
+    const size_t smem = (size_t)w * 4 * (CODE == G_SOP ? 2 : 1) + (size_t)s.wpc * (size_t)w * 4;
+    auto kf = ms_forward_kernel<CODE, WMAX, D>;
+    auto kb = ms_backward_kernel<CODE, WMAX, D>;
+    if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess ||
+        cudaFuncSetAttribute(kb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess)
+        return VJP_ERR_CUDA;
+    VJP_LAUNCH(K_MS_FORWARD, stream) kf<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, vstride, m.ls, m.aggL, s.R, op);
+    const dim3 cg((unsigned)((w + 127) / 128), (unsigned)s.segs);
+    VJP_LAUNCH(K_MS_CARRY, stream) ms_seg_agg_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.G, m.aggL, m.segagg, op);
+    VJP_LAUNCH(K_MS_CARRY, stream) ms_carry_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.G, s.segs, m.aggL, m.Rc, m.segagg, op);
+    VJP_LAUNCH(K_MS_BACKWARD, stream) kb<<<s.grid, s.wpc * 32, smem, stream>>>(
+        n, w, is, vs, vstride, m.ls, m.aggL, m.Rc, hist_bar, vs_bar, s.R, op, accumulate);
+    return last_launch_status();
+}
+
+template <int CODE>
+static int ms_dispatch(float S, int64_t n, int64_t w, const int64_t *is, const float *vs, int vstride,
+                       const float *hist_bar, float *vs_bar, void *ws, int accumulate, cudaStream_t stream) {
+    const MsShape s = ms_shape(n, w, CODE == G_SOP ? 2 : 1);
+    const MsWs m = ms_carve(ws, n, w);
+    if (s.wpc <= 16) return ms_run<CODE, 16, 8>(S, n, w, is, vs, vstride, hist_bar, vs_bar, m, s, accumulate, stream);
+    return ms_run<CODE, 32, 2>(S, n, w, is, vs, vstride, hist_bar, vs_bar, m, s, accumulate, stream);
+}
+
+// gcode: G_ADD ... G_SOP (gen_ops.cuh).  vs: values (G_SOP: the pairs, the s component is read with stride 2).
+int launch_rbi_multiscan_vjp(int gcode, double param, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                             const float *hist_bar, float *vs_bar, void *ws, int accumulate, cudaStream_t stream) {
+    if (n == 0) return VJP_OK;
+    if (!rbi_multiscan_fits(w)) return VJP_ERR_UNSUPPORTED;
+    const float S = (float)param;
+    switch (gcode) {
+    case G_ADD: return ms_dispatch<G_ADD>(S, n, w, is, vs, 1, hist_bar, vs_bar, ws, accumulate, stream);
+    case G_MIN: return ms_dispatch<G_MIN>(S, n, w, is, vs, 1, hist_bar, vs_bar, ws, accumulate, stream);
+    case G_MAX: return ms_dispatch<G_MAX>(S, n, w, is, vs, 1, hist_bar, vs_bar, ws, accumulate, stream);
+    case G_MUL: return ms_dispatch<G_MUL>(S, n, w, is, vs, 1, hist_bar, vs_bar, ws, accumulate, stream);
+    case G_SATADD: return ms_dispatch<G_SATADD>(S, n, w, is, vs, 1, hist_bar, vs_bar, ws, accumulate, stream);
+    case G_SOP: return ms_dispatch<G_SOP>(0.f, n, w, is, vs + 1, 2, hist_bar, vs_bar, ws, accumulate, stream);
+    default: return VJP_ERR_UNSUPPORTED;
+    }
+}
+
+}  // namespace vjp

@@ -260,8 +260,9 @@ def test_rbi_sort_perm_bit_exact(n, w):
     assert np.array_equal(perm.cpu().numpy(), rperm)
 
 
+@pytest.mark.parametrize("route", [1, 2])  # 1: the library's choice (sort-free walks for w <= 4096), 2: Fig. 4 as written
 @pytest.mark.parametrize("n,w", RBI_SHAPES)
-def test_rbi_general_satadd(n, w):
+def test_rbi_general_satadd(n, w, route):
     d = W.c5_rbi_satadd(n=n, w=w)
     is_ = d["is_"].copy()
     is_[::53] = w + 2
@@ -272,21 +273,24 @@ def test_rbi_general_satadd(n, w):
         S += 2.0 ** -5
     S = float(np.float32(S))
     assert not np.any(np.abs(tot - S) < 2.0 ** -7)
-    got = B.vjp_reduce_by_index(B.Op.of("satadd", S=S), w, dev(is_), dev(d["vs"]), dev(d["hist_bar"]))
+    got = B.vjp_reduce_by_index(B.Op.of("satadd", S=S, force_general=route), w, dev(is_), dev(d["vs"]), dev(d["hist_bar"]))
     ref = oracle.vjp_rbi_general("satadd", w, is_, d["vs"], d["hist_bar"], S=S)
     assert np.array_equal(got.cpu().numpy().astype(np.float64), ref)  # every adjoint is a copy or 0
 
 
-@pytest.mark.parametrize("n,w", [(5, 3), (4097, 7), (100003, 1024), (100003, 20000)])
+@pytest.mark.parametrize("route", [1, 2])
+@pytest.mark.parametrize("n,w", [(5, 3), (4097, 7), (100003, 1024), (100003, 4096), (100003, 20000), (1 << 21, 1)])
 @pytest.mark.parametrize("opname", ["add", "min", "max", "mul"])
-def test_general_rule_with_specialisable_operators(opname, n, w):
+def test_general_rule_with_specialisable_operators(opname, n, w, route):
     """the specialised rules are instances of eq. 5; force_general must agree."""
+    if opname == "mul" and w == 1:
+        pytest.skip("2^21 factors in one bin: the product underflows f64")
     if opname == "mul":
         d = W.c2_rbi_mul(n=n, w=w, zero_rate=min(0.3, 0.7 * w / n))
     else:
         d = W.c2_rbi_min(n=n, w=w)
     is_, vs, hb = d["is_"], d["vs"], d["hist_bar"]
-    op = B.Op.of(opname, force_general=True)
+    op = B.Op.of(opname, force_general=route)
     got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
     ref = oracle.vjp_rbi_general(opname, w, is_, vs, hb)
     if opname == "mul":
