@@ -288,33 +288,45 @@ ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const f
         }
         // the table walk of the whole block first (shared-memory latencies only), then the outputs: by then the
         // gathers have arrived, and a wait on them no longer sits between two rows of the (in-order) walk
-        float rr[D];
-#pragma unroll
-        for (int d = 0; d < D; d++) {
-            rr[d] = op.neutral();
-            if (top - d >= r0) rr[d] = ms_row_backward<CODE>(op, tab, k[d], v[d], w, lane);  // warp-uniform
-        }
-#pragma unroll
-        for (int d = 0; d < D; d++) {
-            const int64_t row = top - d;
-            const int64_t idx = row * 32 + lane;
-            if (row >= r0 && idx < n) {
-                const bool inr = (uint64_t)k[d] < (uint64_t)w;
-                const float l = SYM ? ll[d] : op.apply(lc[d], ll[d]);
-                const float h0 = inr ? hs[(uint32_t)k[d] * HW] : 0.f;
-                const float gq = inr ? op.dfdx(l, v[d], rr[d]) * h0 : 0.f;  // 0 out of range
-                if constexpr (CODE == G_SOP) {  // vs_bar_i = (Pbar, Pbar * (ls + rs) + Sbar)
-                    float2 *dst = reinterpret_cast<float2 *>(vs_bar) + idx;
-                    float2 o = make_float2(h0, gq + (inr ? hs[(uint32_t)k[d] * 2 + 1] : 0.f));
-                    if (accumulate) {
-                        const float2 pr = *dst;
-                        o.x += pr.x;
-                        o.y += pr.y;
-                    }
-                    *dst = o;
-                } else {
-                    vs_bar[idx] = accumulate ? vs_bar[idx] + gq : gq;
+        const bool fullb = (top - (D - 1) >= r0) & (top < nfull);  // D whole rows inside the chunk (warp-uniform)
+        // one element's output; `o1` points at vs_bar[idx] (pairs for sumOfProd)
+        auto emit = [&](int d, float r, float *o1) {
+            const bool inr = (uint64_t)k[d] < (uint64_t)w;
+            float l = ll[d];
+            if constexpr (!SYM) l = op.apply(lc[d], l);
+            const float h0 = inr ? hs[(uint32_t)k[d] * HW] : 0.f;
+            const float gq = inr ? op.dfdx(l, v[d], r) * h0 : 0.f;  // 0 out of range
+            if constexpr (CODE == G_SOP) {  // vs_bar_i = (Pbar, Pbar * (ls + rs) + Sbar)
+                float2 *dst = reinterpret_cast<float2 *>(o1);
+                float2 o = make_float2(h0, gq + (inr ? hs[(uint32_t)k[d] * 2 + 1] : 0.f));
+                if (accumulate) {
+                    const float2 pr = *dst;
+                    o.x += pr.x;
+                    o.y += pr.y;
                 }
+                *dst = o;
+            } else {
+                *o1 = accumulate ? *o1 + gq : gq;
+            }
+        };
+        float rr[D];
+        if (fullb) {
+#pragma unroll
+            for (int d = 0; d < D; d++) rr[d] = ms_row_backward<CODE>(op, tab, k[d], v[d], w, lane);
+            float *op1 = vs_bar + (top * 32 + lane) * HW;
+#pragma unroll
+            for (int d = 0; d < D; d++) emit(d, rr[d], op1 - d * 32 * HW);
+        } else {
+#pragma unroll
+            for (int d = 0; d < D; d++) {
+                rr[d] = op.neutral();
+                if (top - d >= r0) rr[d] = ms_row_backward<CODE>(op, tab, k[d], v[d], w, lane);  // warp-uniform
+            }
+#pragma unroll
+            for (int d = 0; d < D; d++) {
+                const int64_t row = top - d;
+                const int64_t idx = row * 32 + lane;
+                if (row >= r0 && idx < n) emit(d, rr[d], vs_bar + idx * HW);
             }
         }
     }
