@@ -145,7 +145,7 @@ int reduce_by_index_forward(const vjp_op_t *op, int64_t n, int64_t num_bins, con
  *   SATADD or force_general: the general rule, eq. 5:
  *             vs_bar_i = d(l_i (.) x (.) r_i)/dx at vs_i * hist_bar[is_i], l_i / r_i = the fold of the
  *             same-bin values before / after i.  Two routes to l and r, same results:
- *             - num_bins <= 4096 and force_general != 2: no sort.  Two in-order walks over the input,
+ *             - num_bins <= 12288 and force_general != 2: no sort.  Two in-order walks over the input,
  *               each warp with a running per-bin table in shared memory (forward: l, backward: r),
  *               per-chunk carries scanned in between; every array is read and written in its
  *               original order (36 bytes per element).
@@ -225,7 +225,7 @@ int rbi_sumofprod_forward(int64_t n, int64_t num_bins, const int64_t *is, const 
  *                     -- a histogram and a map.
  *   use_general != 0: the general rule (eq. 5) for the same operator -- the paper's 8 - 92x against
  *                     1.1 - 2.1x contrast.  1: route picked as in vjp_reduce_by_index (no sort
- *                     for num_bins <= 4096); 2: Fig. 4 as written (sort by bin + segmented scans).
+ *                     for num_bins <= 12288); 2: Fig. 4 as written (sort by bin + segmented scans).
  * accumulate != 0 adds to vs_bar.  Keys outside [0, num_bins) get (0, 0). */
 int vjp_rbi_sumofprod(int64_t n, int64_t num_bins, const int64_t *is, const float *vs,
                       const float *hist_bar, float *vs_bar, int use_general, int accumulate,

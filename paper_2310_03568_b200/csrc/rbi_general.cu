@@ -660,7 +660,7 @@ int launch_reduce_general_vjp(int code, double param, int64_t n, const float *xs
 }
 
 // sorted != 0: Fig. 4 as written (sort + segmented scans); else the sort-free walks of rbi_multiscan.cu when a bin
-// table fits a warp's shared memory (w <= 4096), the sort-based route otherwise.
+// table fits a warp's share of shared memory (w <= 12 288), the sort-based route otherwise.
 int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const int64_t *is,
                            const float *vs, const float *hist_bar, float *vs_bar, void *ws,
                            int accumulate, int sorted, cudaStream_t stream) {

@@ -1,7 +1,7 @@
 """GPU parity of the SORT-FREE route of the general reduce-by-index rule (eq. 5; csrc/rbi_multiscan.cu)
 against the f64 CPU oracle of eq. 5, on the cases that route has of its own: chunk boundaries, rows whose lanes share
 bins (the match.any path) and rows whose lanes do not (the claim path), ties of min / max across chunks (the lowest
-index must win), keys out of range, the hand-over to the sort-based route above w = 4096, accumulate.
+index must win), keys out of range, the hand-over to the sort-based route above w = 12 288, accumulate.
 Integer-valued results (copies of hist_bar or 0) are compared bit-exactly, products normwise at 1e-4."""
 import numpy as np
 import pytest
@@ -103,8 +103,8 @@ def test_all_keys_out_of_range_and_empty_bins():
     assert np.array_equal(got, np.full(n, hb[5], dtype=np.float32))
 
 
-@pytest.mark.parametrize("w", [4096, 4097, 5000])
-def test_handover_to_the_sort_based_route_above_4096_bins(w):
+@pytest.mark.parametrize("w", [4097, 8192, 12288, 12289, 20000])   # 6, 3 warps per SM; then the sort-based route
+def test_handover_to_the_sort_based_route_above_12288_bins(w):
     n = 150001
     d = W.c2_rbi_min(n=n, w=w)
     ref = oracle.vjp_rbi_general("min", w, d["is_"], d["vs"], d["hist_bar"])

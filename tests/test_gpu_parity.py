@@ -260,7 +260,7 @@ def test_rbi_sort_perm_bit_exact(n, w):
     assert np.array_equal(perm.cpu().numpy(), rperm)
 
 
-@pytest.mark.parametrize("route", [1, 2])  # 1: the library's choice (sort-free walks for w <= 4096), 2: Fig. 4 as written
+@pytest.mark.parametrize("route", [1, 2])  # 1: the library's choice (sort-free walks for w <= 12 288), 2: Fig. 4 as written
 @pytest.mark.parametrize("n,w", RBI_SHAPES)
 def test_rbi_general_satadd(n, w, route):
     d = W.c5_rbi_satadd(n=n, w=w)
