@@ -16,8 +16,9 @@
 //             each such group in lane (= index) order by pointer jumping; l_local_i = tab[bin] (.) that fold; the last
 //             lane of the group stores the group's inclusive fold back.  l_local -> global (4 B / element); at the end of
 //             the chunk the table IS the chunk's per-bin aggregate -> agg[chunk][w].
-//   carry     per bin, exclusive prefix L[chunk][bin] and exclusive suffix R[chunk][bin] of agg over the chunks (a
-//             few thousand chunks x w bins; two-level: segments of <= 32 chunks held in registers).
+//   carry     per bin, exclusive prefix L[chunk][bin] and exclusive suffix R[chunk][bin] of agg over the chunks, in two
+//             levels: among the chunks of one CTA in the forward kernel's epilogue (the tables are still in shared
+//             memory), among the CTAs by two small kernels over the 148 CTA aggregates.
 //   backward  the same walk from the end of the chunk towards its start, table initialised with R[chunk][.]: gives
 //             r_i directly; l_i = L[chunk][bin] (.) l_local_i; then the derivative and the store of vs_bar_i in place
 //             (original order: no scatter).  Out-of-range keys take no part and get 0.
@@ -51,7 +52,7 @@ static int ms_warps_per_cta(int64_t w, int hw) {
 
 struct MsShape {
     int wpc, grid;
-    int64_t G, R, segs;  // chunks (warps), rows per chunk, carry segments
+    int64_t G, R, segs;  // chunks (warps), rows per chunk, carry segments (of MS_SEG CTAs)
 };
 static MsShape ms_shape(int64_t n, int64_t w, int hw) {
     MsShape s;
@@ -65,7 +66,7 @@ static MsShape ms_shape(int64_t n, int64_t w, int hw) {
     s.G = (int64_t)s.grid * s.wpc;
     s.R = (rows + s.G - 1) / s.G;
     if (s.R < 1) s.R = 1;
-    s.segs = (s.G + MS_SEG - 1) / MS_SEG;
+    s.segs = (s.grid + MS_SEG - 1) / MS_SEG;  // the carry kernels scan the CTA aggregates
     return s;
 }
 
@@ -158,8 +159,10 @@ VJP_DEVINL float ms_row_backward(const GenOp<CODE> &op, float *tab, int64_t k, f
 template <int CODE, int WMAX, int D>
 __global__ void __launch_bounds__(WMAX * 32, 1)
 ms_forward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs, int vstride,
-                  float *__restrict__ ls, float *__restrict__ agg, int64_t R, GenOp<CODE> op) {
+                  float *__restrict__ ls, float *__restrict__ intraA, float *__restrict__ intraB,
+                  float *__restrict__ ctaagg, int64_t R, GenOp<CODE> op) {
     extern __shared__ float ms_smem[];
+    constexpr bool SYM = CODE != G_MIN && CODE != G_MAX;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
     float *tab = ms_smem + (size_t)warp * (size_t)w;
     for (int i = lane; i < (int)w; i += 32) tab[i] = op.neutral();
@@ -217,14 +220,43 @@ ms_forward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const fl
             }
         }
     }
-    __syncwarp();
-    for (int i = lane; i < (int)w; i += 32) agg[g * w + i] = tab[i];
+    // Epilogue: the tables of the CTA's warps are the aggregates of wpc CONSECUTIVE chunks.  Per bin, what the other
+    // chunks of this CTA contribute to chunk j -- the fold of the warps before it (P_j) and after it (S_j) -- is formed
+    // here, from shared memory; only the CTA totals go through the carry kernels (148 rows instead of ~1900).
+    //   SYM operators:  intraA[g][b] = P_j (.) S_j          (L and R are only ever used as L (.) R, see the header)
+    //   min / max:      intraA[g][b] = P_j,  intraB[g][b] = S_j
+    __syncthreads();
+    const int64_t g0 = (int64_t)blockIdx.x * wpc;
+    for (int b = threadIdx.x; b < (int)w; b += blockDim.x) {
+        float sfx[WMAX];
+        float suf = op.neutral();
+#pragma unroll
+        for (int j = WMAX - 1; j >= 0; j--) {
+            sfx[j] = suf;
+            if (j < wpc) suf = op.apply(ms_smem[(size_t)j * w + b], suf);
+        }
+        float pre = op.neutral();
+#pragma unroll
+        for (int j = 0; j < WMAX; j++) {
+            if (j < wpc) {
+                if constexpr (SYM) {
+                    intraA[(g0 + j) * w + b] = op.apply(pre, sfx[j]);
+                } else {
+                    intraA[(g0 + j) * w + b] = pre;
+                    intraB[(g0 + j) * w + b] = sfx[j];
+                }
+                pre = op.apply(pre, ms_smem[(size_t)j * w + b]);
+            }
+        }
+        ctaagg[(int64_t)blockIdx.x * w + b] = pre;
+    }
 }
 
 template <int CODE, int WMAX, int D>
 __global__ void __launch_bounds__(WMAX * 32, 1)
 ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs, int vstride,
-                   const float *__restrict__ ls, const float *__restrict__ Lc, const float *__restrict__ Rc,
+                   const float *__restrict__ ls, float *intraA, const float *__restrict__ intraB,
+                   const float *__restrict__ ctaL, const float *__restrict__ ctaR,
                    const float *__restrict__ hist_bar, float *__restrict__ vs_bar, int64_t R, GenOp<CODE> op,
                    int accumulate) {
     extern __shared__ float ms_smem[];
@@ -235,12 +267,20 @@ ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const f
     float *tab = ms_smem + (size_t)w * HW + (size_t)warp * (size_t)w;
     const int64_t g = (int64_t)blockIdx.x * wpc + warp;
     for (int i = threadIdx.x; i < (int)w * HW; i += blockDim.x) hs[i] = hist_bar[i];
+    // what lies outside the chunk: the other chunks of this CTA (forward kernel's epilogue) and the other CTAs (carry
+    // kernels).  SYM: all of it on the r side.  min / max: the right part in the table, the left part L[g][.] written
+    // back over intraA for the per-element gather.
+    float *Lg = intraA + g * w;
+    const float *cl = ctaL + (int64_t)blockIdx.x * w, *cr = ctaR + (int64_t)blockIdx.x * w;
     for (int i = lane; i < (int)w; i += 32) {
-        const float rc = Rc[g * w + i];  // what lies to the right of the chunk
-        tab[i] = SYM ? op.apply(Lc[g * w + i], rc) : rc;
+        if constexpr (SYM) {
+            tab[i] = op.apply(op.apply(cl[i], Lg[i]), cr[i]);
+        } else {
+            tab[i] = op.apply(intraB[g * w + i], cr[i]);
+            Lg[i] = op.apply(cl[i], Lg[i]);
+        }
     }
     __syncthreads();
-    const float *Lg = Lc + g * w;
     const int64_t rows = (n + 31) >> 5;
     const int64_t r0 = min(g * R, rows), r1 = min(r0 + R, rows);
     // rows are walked from r1 - 1 down to r0, D at a time: block b covers rows r1 - 1 - b*D - d
@@ -285,7 +325,7 @@ ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const f
         if constexpr (!SYM) {
 #pragma unroll
             for (int d = 0; d < D; d++)  // the gathers of the whole block are issued before the walk
-                lc[d] = (uint64_t)k[d] < (uint64_t)w ? __ldg(Lg + k[d]) : op.neutral();
+                lc[d] = (uint64_t)k[d] < (uint64_t)w ? Lg[k[d]] : op.neutral();  // written above by this warp: no __ldg
         }
         // the table walk of the whole block first (shared-memory latencies only), then the outputs: by then the
         // gathers have arrived, and a wait on them no longer sits between two rows of the (in-order) walk
@@ -392,18 +432,24 @@ __global__ void ms_carry_kernel(int64_t w, int64_t G, int64_t segs, float *__res
 // ------------------------------------------------------------------ host side -------------
 
 struct MsWs {
-    float *ls, *aggL, *Rc, *segagg;
+    float *ls, *intraA, *intraB, *ctaL, *ctaR, *segagg;
     size_t total;
 };
 static MsWs ms_carve(void *ws, int64_t n, int64_t w) {
-    const MsShape s = ms_shape(n < 1 ? 1 : n, w < 1 ? 1 : w, 1);  // hw = 1: the most chunks any operator uses
+    // the workspace query does not know the operator: rows for whichever of the two table shapes (hist_bar of 1 or 2
+    // words per bin) has more chunks / more CTAs at this (n, w)
+    const MsShape s1 = ms_shape(n < 1 ? 1 : n, w < 1 ? 1 : w, 1), s2 = ms_shape(n < 1 ? 1 : n, w < 1 ? 1 : w, 2);
+    const size_t G = (size_t)(s1.G > s2.G ? s1.G : s2.G), grid = (size_t)(s1.grid > s2.grid ? s1.grid : s2.grid);
+    const size_t segs = (size_t)(s1.segs > s2.segs ? s1.segs : s2.segs);
     MsWs m;
     char *p = static_cast<char *>(ws);
     auto take = [&](size_t bytes) { char *r = p; p += align_up(bytes, 256); return r; };
     m.ls = reinterpret_cast<float *>(take((size_t)(n < 1 ? 1 : n) * 4));
-    m.aggL = reinterpret_cast<float *>(take((size_t)s.G * (size_t)w * 4));
-    m.Rc = reinterpret_cast<float *>(take((size_t)s.G * (size_t)w * 4));
-    m.segagg = reinterpret_cast<float *>(take((size_t)s.segs * (size_t)w * 4));
+    m.intraA = reinterpret_cast<float *>(take(G * (size_t)w * 4));
+    m.intraB = reinterpret_cast<float *>(take(G * (size_t)w * 4));  // min / max only
+    m.ctaL = reinterpret_cast<float *>(take(grid * (size_t)w * 4));   // CTA aggregates, then their prefixes
+    m.ctaR = reinterpret_cast<float *>(take(grid * (size_t)w * 4));
+    m.segagg = reinterpret_cast<float *>(take(segs * (size_t)w * 4));
     m.total = (size_t)(p - static_cast<char *>(ws));
     return m;
 }
@@ -424,12 +470,14 @@ static int ms_run(float S, int64_t n, int64_t w, const int64_t *is, const float 
     if (cudaFuncSetAttribute(kf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess ||
         cudaFuncSetAttribute(kb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess)
         return VJP_ERR_CUDA;
-    VJP_LAUNCH(K_MS_FORWARD, stream) kf<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, vstride, m.ls, m.aggL, s.R, op);
+    VJP_LAUNCH(K_MS_FORWARD, stream) kf<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, vstride, m.ls, m.intraA, m.intraB,
+                                                                              m.ctaL, s.R, op);
+    // exclusive prefix (in place) and suffix of the CTA aggregates over the CTAs
     const dim3 cg((unsigned)((w + 127) / 128), (unsigned)s.segs);
-    VJP_LAUNCH(K_MS_CARRY, stream) ms_seg_agg_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.G, m.aggL, m.segagg, op);
-    VJP_LAUNCH(K_MS_CARRY, stream) ms_carry_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.G, s.segs, m.aggL, m.Rc, m.segagg, op);
+    VJP_LAUNCH(K_MS_CARRY, stream) ms_seg_agg_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.grid, m.ctaL, m.segagg, op);
+    VJP_LAUNCH(K_MS_CARRY, stream) ms_carry_kernel<CODE><<<cg, 128, 0, stream>>>(w, s.grid, s.segs, m.ctaL, m.ctaR, m.segagg, op);
     VJP_LAUNCH(K_MS_BACKWARD, stream) kb<<<s.grid, s.wpc * 32, smem, stream>>>(
-        n, w, is, vs, vstride, m.ls, m.aggL, m.Rc, hist_bar, vs_bar, s.R, op, accumulate);
+        n, w, is, vs, vstride, m.ls, m.intraA, m.intraB, m.ctaL, m.ctaR, hist_bar, vs_bar, s.R, op, accumulate);
     return last_launch_status();
 }
 
