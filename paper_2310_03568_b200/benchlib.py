@@ -46,6 +46,8 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
         "sort_scatter_kernel": 24,                   # read 12, write 12
         "seg_forward_kernel": 12 + 4,
         "seg_reverse_vjp_kernel": 16 + 4,
+        "ms_forward_kernel": 8 + 4 + 4,              # is + vs, l written
+        "ms_backward_kernel": 8 + 4 + 4 + 4,         # is + vs + l, vs_bar written
     }
     return float(table.get(name, 0.0))
 
