@@ -30,7 +30,7 @@ enum KernelId : int {
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
     K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP, K_VEC_TRANSPOSE,
-    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD,
+    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD, K_MS_HIST,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -76,6 +76,10 @@ int launch_rbi_general_vjp(int code, double param, int64_t n, int64_t w, const i
 // the sort-free route (rbi_multiscan.cu); gcode = G_ADD ... G_SOP of gen_ops.cuh
 bool rbi_multiscan_fits(int64_t w);
 size_t rbi_multiscan_workspace_bytes(int64_t n, int64_t w);
+// the same walk as a plain histogram for '*' / satadd (rbi_kernels.cu uses it for 1024 < w <= 12288)
+int rbi_ms_hist_tables(int64_t n, int64_t w);
+int launch_ms_hist(int mul, int count_zeros, float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                   float *part, unsigned *zeros, cudaStream_t stream);
 int launch_rbi_multiscan_vjp(int gcode, double param, int64_t n, int64_t w, const int64_t *is, const float *vs,
                              const float *hist_bar, float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,

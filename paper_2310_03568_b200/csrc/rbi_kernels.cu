@@ -1116,8 +1116,11 @@ static int cached_grid(int64_t n, int64_t w) {
     if (groups > cap) groups = cap;
     return (int)(groups << c);
 }
+// 1024 < w <= 12288: the in-order walk of rbi_multiscan.cu as a histogram (warp-private tables, no CTA-wide rounds)
+static bool cached_walk(int64_t w) { return w > CS_SLOTS && rbi_multiscan_fits(w); }
 // number of partial tables the accumulation kernel writes
 static int cached_tables(int64_t n, int64_t w) {
+    if (cached_walk(w)) return rbi_ms_hist_tables(n, w);
     return w <= CS_SLOTS ? cached_grid(n, w) : cached_grid(n, w) >> cached_split_log2(w);
 }
 static size_t cached_part_bytes(int64_t n, int64_t w) {
@@ -1131,6 +1134,8 @@ static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, 
                       unsigned *zeros, float S, int *G_out, cudaStream_t stream) {
     const int G = cached_grid(n, w);
     *G_out = cached_tables(n, w);
+    if (cached_walk(w))
+        return launch_ms_hist(ACC == ACC_MUL, COUNT_ZEROS, S, n, w, is, vs, part, zeros, stream);
     if (w <= CS_SLOTS) {
         auto kern = rbi_cached_small_kernel<ACC, COUNT_ZEROS>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CS_SMEM) != cudaSuccess)

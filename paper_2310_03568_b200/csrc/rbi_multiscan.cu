@@ -373,6 +373,76 @@ ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const f
     }
 }
 
+// The same walk as a plain HISTOGRAM for the operators with no hardware atomic ('*', satadd; H0 / H4 for
+// 1024 < w <= MS_W_MAX, where rbi_cached_big_kernel needs CTA-wide claim rounds between barriers): no l is stored, the
+// epilogue folds the CTA's warp tables in warp order into ONE partial table per CTA (deterministic), which the fold
+// kernels of rbi_kernels.cu combine.  COUNT_ZEROS (the lifted '*' of P:L460): an exact zero is counted in zeros[bin]
+// and takes no part in the product.
+template <int CODE, int WMAX, int D, bool COUNT_ZEROS>
+__global__ void __launch_bounds__(WMAX * 32, 1)
+ms_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs,
+               float *__restrict__ part, unsigned *zeros, int64_t R, GenOp<CODE> op) {
+    extern __shared__ float ms_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
+    float *tab = ms_smem + (size_t)warp * (size_t)w;
+    for (int i = lane; i < (int)w; i += 32) tab[i] = op.neutral();
+    __syncwarp();
+    const int64_t g = (int64_t)blockIdx.x * wpc + warp;
+    const int64_t rows = (n + 31) >> 5;
+    const int64_t r0 = min(g * R, rows), r1 = min(r0 + R, rows);
+    const int64_t rfull = min(r1, n >> 5);
+    int64_t kn[D];
+    float vn[D];
+    auto fetch = [&](int64_t rb) {
+        if (rb + D <= rfull) {
+            const int64_t *kp = is + rb * 32 + lane;
+            const float *vp = vs + rb * 32 + lane;
+#pragma unroll
+            for (int d = 0; d < D; d++) {
+                kn[d] = __ldg(kp + d * 32);
+                vn[d] = __ldg(vp + d * 32);
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < D; d++) {
+                const int64_t idx = (rb + d) * 32 + lane;
+                const bool ok = (rb + d < r1) & (idx < n);
+                kn[d] = ok ? __ldg(is + idx) : (int64_t)-1;
+                vn[d] = ok ? __ldg(vs + idx) : 1.f;
+            }
+        }
+    };
+    fetch(r0);
+    for (int64_t rb = r0; rb < r1; rb += D) {
+        int64_t k[D];
+        float v[D];
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            k[d] = kn[d];
+            v[d] = vn[d];
+        }
+        fetch(rb + D);
+#pragma unroll
+        for (int d = 0; d < D; d++) {
+            if (rb + d < r1) {  // warp-uniform
+                if (COUNT_ZEROS) {
+                    if ((uint64_t)k[d] < (uint64_t)w && v[d] == 0.f) {  // IEEE equality: +-0 only (Q7)
+                        atomicAdd(zeros + k[d], 1u);
+                        k[d] = -1;
+                    }
+                }
+                ms_row_forward<CODE>(op, tab, k[d], v[d], w, lane);
+            }
+        }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < (int)w; b += blockDim.x) {
+        float acc = ms_smem[b];
+        for (int j = 1; j < wpc; j++) acc = op.apply(acc, ms_smem[(size_t)j * w + b]);
+        part[(int64_t)blockIdx.x * w + b] = acc;
+    }
+}
+
 // Carry, level 1: segagg[seg][b] = fold of agg[g][b] over the chunks g of segment seg (in order).
 template <int CODE>
 __global__ void ms_seg_agg_kernel(int64_t w, int64_t G, const float *__restrict__ agg, float *__restrict__ segagg,
@@ -505,6 +575,41 @@ int launch_rbi_multiscan_vjp(int gcode, double param, int64_t n, int64_t w, cons
     case G_SOP: return ms_dispatch<G_SOP>(0.f, n, w, is, vs + 1, 2, hist_bar, vs_bar, ws, accumulate, stream);
     default: return VJP_ERR_UNSUPPORTED;
     }
+}
+
+// ------------------------------------------------------------------ histogram (primal) by the same walk
+
+static MsShape ms_hist_shape(int64_t n, int64_t w) { return ms_shape(n < 1 ? 1 : n, w < 1 ? 1 : w, 0); }
+
+// number of partial tables launch_ms_hist writes (= its grid)
+int rbi_ms_hist_tables(int64_t n, int64_t w) { return ms_hist_shape(n, w).grid; }
+
+template <int CODE, bool COUNT_ZEROS>
+static int ms_hist_run(float S, int64_t n, int64_t w, const int64_t *is, const float *vs, float *part, unsigned *zeros,
+                       cudaStream_t stream) {
+    const MsShape s = ms_hist_shape(n, w);
+    const GenOp<CODE> op{S};
+    const size_t smem = (size_t)s.wpc * (size_t)w * 4;
+    if (s.wpc <= 16) {
+        auto k = ms_hist_kernel<CODE, 16, 8, COUNT_ZEROS>;
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess) return VJP_ERR_CUDA;
+        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op);
+    } else {
+        auto k = ms_hist_kernel<CODE, 32, 2, COUNT_ZEROS>;
+        if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess) return VJP_ERR_CUDA;
+        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op);
+    }
+    return last_launch_status();
+}
+
+// part[rbi_ms_hist_tables(n, w)][w] partial histograms of '*' (mul != 0; count_zeros: the lifted form) or satadd
+int launch_ms_hist(int mul, int count_zeros, float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
+                   float *part, unsigned *zeros, cudaStream_t stream) {
+    if (mul) {
+        return count_zeros ? ms_hist_run<G_MUL, true>(S, n, w, is, vs, part, zeros, stream)
+                           : ms_hist_run<G_MUL, false>(S, n, w, is, vs, part, zeros, stream);
+    }
+    return ms_hist_run<G_SATADD, false>(S, n, w, is, vs, part, zeros, stream);
 }
 
 }  // namespace vjp
