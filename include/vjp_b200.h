@@ -115,6 +115,24 @@ int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
 int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar,
              void *ws, size_t ws_bytes, void *stream);
 
+/* The '+' rule of vjp_scan (f32: xs_bar = reverse inclusive sum of ys_bar) for callers that cannot
+ * allocate and cannot pass a workspace (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc).  Same kernel as vjp_scan(VJP_OP_ADD, VJP_F32); its scratch (ticket + look-back slots, 131 328 bytes)
+ * is a static __device__ array inside the library, held by every GPU that loads the library until the process
+ * exits.  The call performs no cudaMalloc / cudaFree and calls no allocating routine: it clears the status words it
+ * needs with a memset on `stream` and launches.
+ *   n        at most vjp_scan_add_f32_noalloc_max_n() = 2^24 elements; larger n returns VJP_ERR_UNSUPPORTED
+ *            (nothing is enqueued): use vjp_scan with a caller-owned workspace.  n == 0: VJP_OK, no-op.
+ *   ys_bar   DEVICE, [n] f32, 16-byte aligned;  xs_bar: DEVICE, [n] f32, 16-byte aligned, may equal ys_bar
+ *            (in place) unless accumulate != 0, which adds the result to xs_bar.
+ *   NULL / misaligned pointer or n < 0: VJP_ERR_INVALID_ARG.  The scratch address could not be resolved on the
+ *   current device, or the launch failed: VJP_ERR_CUDA.
+ * ALL calls on a device share the one scratch array, and it keeps the last call's contents (each call re-clears
+ * what it needs): calls that may overlap on the GPU -- different streams, or graph branches that run
+ * concurrently -- race on it and give wrong results.  Calls on one stream are safe. */
+int64_t vjp_scan_add_f32_noalloc_max_n(void);
+int vjp_scan_add_f32_noalloc(int64_t n, const float *ys_bar, float *xs_bar, int accumulate, void *stream);
+
 /* Same, with HOST pointers for xs, ys_bar, xs_bar.  dev_scratch is a DEVICE buffer of at least
  * vjp_scan_host_scratch_bytes() bytes (holds the three arrays and the workspace). */
 size_t vjp_scan_host_scratch_bytes(const vjp_op_t *op, int64_t n);

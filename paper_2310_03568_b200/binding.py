@@ -25,7 +25,8 @@ F32, F64 = 0, 1
 
 EXPORTS = [
     "vjp_scan_arity", "vjp_version", "vjp_scan_workspace_bytes", "scan_forward", "vjp_scan",
-    "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_reduce_by_index_workspace_bytes",
+    "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_scan_add_f32_noalloc_max_n", "vjp_scan_add_f32_noalloc",
+    "vjp_reduce_by_index_workspace_bytes",
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
     "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
     "vjp_reduce_workspace_bytes", "reduce_forward", "vjp_reduce", "reduce_lifted",
@@ -91,6 +92,8 @@ def load() -> ctypes.CDLL:
         "vjp_scan": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_scan_host_scratch_bytes": (sz, [opp, i64]),
         "vjp_scan_host": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_scan_add_f32_noalloc_max_n": (i64, []),
+        "vjp_scan_add_f32_noalloc": (ctypes.c_int, [i64, vp, vp, ctypes.c_int, vp]),
         "vjp_reduce_by_index_workspace_bytes": (sz, [opp, i64, i64]),
         "reduce_by_index_forward": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_reduce_by_index": (ctypes.c_int, [opp, i64, i64, vp, vp, vp, vp, vp, sz, vp]),
@@ -223,6 +226,24 @@ def vjp_scan(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -
     o = op.c()
     _check(load().vjp_scan(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                            _stream(stream)), "vjp_scan")
+    return xs_bar
+
+
+def vjp_scan_add_f32_noalloc_max_n() -> int:
+    return load().vjp_scan_add_f32_noalloc_max_n()
+
+
+def vjp_scan_add_f32_noalloc(ys_bar: torch.Tensor, out: torch.Tensor, accumulate: bool = False, stream=None) -> torch.Tensor:
+    """The '+' scan VJP (f32) with the scratch in a static device array of the library: no workspace, no allocation
+    -- `out` must be given (this wrapper allocates nothing either).  n <= vjp_scan_add_f32_noalloc_max_n(); calls
+    that overlap on the GPU race on the shared scratch (include/vjp_b200.h)."""
+    if out is None:
+        raise VjpError("vjp_scan_add_f32_noalloc allocates nothing: pass out=")
+    ys_bar = _dev(ys_bar, torch.float32, what="ys_bar")
+    n = ys_bar.numel()
+    xs_bar = _out(out, torch.float32, n, ys_bar.device, "xs_bar")
+    _check(load().vjp_scan_add_f32_noalloc(n, _ptr(ys_bar), _ptr(xs_bar), int(accumulate), _stream(stream)),
+           "vjp_scan_add_f32_noalloc")
     return xs_bar
 
 

@@ -167,6 +167,17 @@ int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, 
     return launch_scan_vjp(op->code, op->dtype, n, xs, ys_bar, xs_bar, ws, op->accumulate, as_stream(stream));
 }
 
+int64_t vjp_scan_add_f32_noalloc_max_n(void) { return scan_noalloc_max_n(); }
+
+int vjp_scan_add_f32_noalloc(int64_t n, const float *ys_bar, float *xs_bar, int accumulate, void *stream) {
+    if (n < 0) return VJP_ERR_INVALID_ARG;
+    if (n > scan_noalloc_max_n()) return VJP_ERR_UNSUPPORTED;  // beyond the static scratch: use vjp_scan
+    if (n == 0) return VJP_OK;
+    if (!ys_bar || !xs_bar || !all_aligned(ys_bar, xs_bar)) return VJP_ERR_INVALID_ARG;
+    if (xs_bar == ys_bar && accumulate) return VJP_ERR_INVALID_ARG;
+    return launch_scan_add_f32_noalloc(n, ys_bar, xs_bar, accumulate != 0, as_stream(stream));
+}
+
 size_t vjp_scan_host_scratch_bytes(const vjp_op_t *op, int64_t n) {
     if (!op_ok(op) || !scan_supported(op) || n < 0) return 0;
     const size_t arr = align_up((size_t)n * vjp_scan_arity(op) * dtype_bytes(op->dtype), 256);

@@ -50,6 +50,9 @@ int launch_scan_forward(int code, int dtype, int64_t n, const void *xs, void *ys
                         cudaStream_t stream);
 int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *ys_bar,
                     void *xs_bar, void *ws, int accumulate, cudaStream_t stream);
+// '+' f32 scan VJP with its scratch in a static device array (no workspace, no allocation); n <= scan_noalloc_max_n()
+int64_t scan_noalloc_max_n();
+int launch_scan_add_f32_noalloc(int64_t n, const float *ys_bar, float *xs_bar, int accumulate, cudaStream_t stream);
 
 // -------------------------------------------------------------- reduce-by-index (special) -
 size_t rbi_special_workspace_bytes(int code, int dtype, int64_t n, int64_t w);

@@ -19,8 +19,17 @@
 // 128-bit coalesced global accesses.  A tile's processing index comes from an atomic ticket.
 #include <cooperative_groups.h>
 
+#include <atomic>
+
 #include "internal.h"
 #include "scan_ops.cuh"
+
+// Scratch of the entry point that allocates nothing (vjp_scan_add_f32_noalloc, at the end of this file): the ticket
+// word and the look-back slots of the '+' scan for up to VJP_NOALLOC_MAX_N = 2^24 elements = 1024 tiles of 16 384
+// elements, one 128-byte slot each, + the 256-byte ticket region: 131 328 bytes.  Held by every GPU that loads the
+// library until the process exits.  In HOST code this name is only a stand-in for the symbol, not a device address:
+// host code gets the address with cudaGetSymbolAddress (noalloc_scratch_ptr below).
+static __device__ __align__(256) unsigned char vjp_noalloc_scratch[256 + 1024 * 128];
 
 namespace vjp {
 
@@ -554,6 +563,49 @@ int launch_scan_vjp(int code, int dtype, int64_t n, const void *xs, const void *
     }
 #undef F
     return VJP_ERR_UNSUPPORTED;
+}
+
+// ------------------------------------------------------------------ no-allocation entry point
+//
+// vjp_scan_add_f32_noalloc: the '+' rule of the scan VJP (xs_bar = reverse inclusive sum of ys_bar) for
+// callers that can neither allocate a workspace nor let the library do it (CUDA graph capture, serving loops):
+// the same kernel as vjp_scan with VJP_OP_ADD / f32, its look-back scratch in the static device array above.
+
+constexpr int64_t NOALLOC_MAX_N = (int64_t)1 << 24;
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static_assert(sizeof(vjp_noalloc_scratch) >= WS_ALIGN + 8 * TileSlots<float>::STRIDE *
+                                                 (size_t)(NOALLOC_MAX_N / (CfgAddF32::NT * CfgAddF32::IPT)),
+              "static scratch too small for NOALLOC_MAX_N");
+
+int64_t scan_noalloc_max_n() { return NOALLOC_MAX_N; }
+
+// Device address of the static scratch on the CURRENT device: resolved once per device, with that device current.
+static char *noalloc_scratch_ptr() {
+    static std::atomic<char *> cache[NOALLOC_MAX_DEVICES];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= NOALLOC_MAX_DEVICES) return nullptr;
+    char *p = cache[dev].load(std::memory_order_acquire);
+    if (p == nullptr) {
+        void *sym = nullptr;
+        if (cudaGetSymbolAddress(&sym, vjp_noalloc_scratch) != cudaSuccess || sym == nullptr) {
+            cudaGetLastError();
+            return nullptr;
+        }
+        p = static_cast<char *>(sym);
+        cache[dev].store(p, std::memory_order_release);
+    }
+    return p;
+}
+
+// n in [1, NOALLOC_MAX_N] (checked by the caller).  No cudaMalloc / cudaFree: the status words are cleared with a
+// memset on `stream` (run_scan), then the kernel is launched.
+int launch_scan_add_f32_noalloc(int64_t n, const float *ys_bar, float *xs_bar, int accumulate, cudaStream_t stream) {
+    if (lookback_bytes<float>(tiles_of(n, CfgAddF32::NT * CfgAddF32::IPT)) > sizeof(vjp_noalloc_scratch))
+        return VJP_ERR_UNSUPPORTED;
+    char *ws = noalloc_scratch_ptr();
+    if (ws == nullptr) return VJP_ERR_CUDA;
+    return run_scan<OpAdd<float>, CfgAddF32::NT, CfgAddF32::IPT, true, MODE_SCAN>(n, ys_bar, xs_bar, nullptr, ws,
+                                                                                  accumulate, stream);
 }
 
 }  // namespace vjp
