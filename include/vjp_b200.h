@@ -217,6 +217,8 @@ int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorte
  * reduce-by-index form P:L464-466; ISWIM P:L655-657): the arrays are transposed, the scalar rule runs on each of
  * the d columns (any scalar operator the scalar entry point accepts in f32: ADD, MIN, MAX, MUL, SATADD for
  * reduce_by_index; ADD, MUL, MIN, MAX for scan), and the result is transposed back (op.accumulate fused there).
+ * reduce_by_index with MUL, d a power of two and 1024 < num_bins * d <= 12288 skips the transposes: the d histograms
+ * are one histogram over (bin, column) pairs, computed on the flat arrays with virtual keys is[j / d] * d + j % d.
  * d <= 4096. */
 size_t vjp_reduce_by_index_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins);
 int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins, const int64_t *is,

@@ -168,7 +168,7 @@ VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (D
     "c5_rbi_satadd": 36, "c5_rbi_satadd_sorted": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
     "f4_scan_matmul3": 144, "f4_scan_min": 16,
-    "f3_rbi_vec_mul": 16 + 28 * 4,   # per ROW of d = 4: two transposes (read + write 4 d each way) + d scalar '*' VJPs at 28 B
+    "f3_rbi_vec_mul": (8 + 16) + (8 + 16 + 16),   # per ROW of d = 4, fused: lifted primal (key + row) + sweep (key + row read, row written)
     "f1_sop_inv": 40, "f1_sop_general": 40, "f1_sop_general_sorted": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
 }
 PRIMAL_BYTES_PER_ELEM = {

@@ -389,12 +389,27 @@ VecWs vec_carve(void *ws, int64_t n, int64_t d, int64_t w, size_t inner_bytes) {
     return v;
 }
 bool vec_op_ok(const vjp_op_t *op) { return op_ok(op) && op->dtype == VJP_F32; }
+// `map2 (*)` on rows of d = 2^ld scalars: d histograms = ONE histogram over (bin, column) pairs, run as
+// a scalar '*' problem on the flat arrays with virtual keys -- no transposes, keys read once per row.  Returns ld, or
+// 0 if this form does not apply (then: transpose + the scalar rule per column).
+int vec_mul_fused_ld(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins) {
+    if (op->code != VJP_OP_MUL || op->force_general || d < 2 || (d & (d - 1)) != 0) return 0;
+    int ld = 0;
+    while (((int64_t)1 << ld) < d) ld++;
+    return rbi_mul_vec_fused(n, num_bins, ld) ? ld : 0;
+}
 }  // namespace
 
 size_t vjp_reduce_by_index_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins) {
     if (!vec_op_ok(op) || n < 0 || d < 1 || num_bins < 0) return 0;
     const size_t inner = vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
-    return inner ? vec_carve(nullptr, n, d, num_bins, inner).total : 0;
+    if (!inner) return 0;
+    size_t need = vec_carve(nullptr, n, d, num_bins, inner).total;
+    if (const int ld = vec_mul_fused_ld(op, n, d, num_bins)) {
+        const size_t fused = rbi_special_workspace_bytes(VJP_OP_MUL, VJP_F32, n << ld, num_bins << ld);
+        if (fused > need) need = fused;
+    }
+    return need;
 }
 
 int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins, const int64_t *is,
@@ -407,9 +422,12 @@ int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t nu
     const bool needs_vs = rbi_route(op) != 1;
     if (!is || !vss_bar || !ws || (num_bins > 0 && !hist_bar) || (needs_vs && !vss)) return VJP_ERR_INVALID_ARG;
     if (!all_aligned(is, vss, hist_bar, vss_bar, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < vjp_reduce_by_index_vec_workspace_bytes(op, n, d, num_bins)) return VJP_ERR_WORKSPACE;
+    if (const int ld = vec_mul_fused_ld(op, n, d, num_bins))
+        return launch_rbi_mul(n << ld, num_bins << ld, is, static_cast<const float *>(vss), static_cast<const float *>(hist_bar),
+                              static_cast<float *>(vss_bar), nullptr, nullptr, ws, op->accumulate != 0, as_stream(stream), ld);
     const size_t inner = vjp_reduce_by_index_workspace_bytes(op, n, num_bins);
     const VecWs v = vec_carve(ws, n, d, num_bins, inner);
-    if (ws_bytes < v.total) return VJP_ERR_WORKSPACE;
     cudaStream_t s = as_stream(stream);
     int rc;
     if (needs_vs && (rc = launch_rows_to_cols(n, d, v.ncol, static_cast<const float *>(vss), v.cols, s)) != VJP_OK) return rc;

@@ -69,7 +69,10 @@ int launch_rbi_minmax(int code, int64_t n, int64_t w, const int64_t *is, const f
 // MUL: lifted primal into ws, then (zeros, prod_nz) and / or the return sweep.
 int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
                    const float *hist_bar, float *vs_bar, int64_t *zeros, float *prod_nz, void *ws,
-                   int accumulate, cudaStream_t stream);
+                   int accumulate, cudaStream_t stream, int ld = 0);
+// `map2 (*)` on rows of 2^ld scalars as ONE scalar '*' problem on the flat arrays with virtual keys (bin, column):
+// can launch_rbi_mul take (n << ld, w << ld, ..., ld)?
+bool rbi_mul_vec_fused(int64_t n, int64_t w, int ld);
 
 // -------------------------------------------------------------- reduce-by-index (general) -
 size_t rbi_general_workspace_bytes(int64_t n, int64_t w);
@@ -82,7 +85,7 @@ size_t rbi_multiscan_workspace_bytes(int64_t n, int64_t w);
 // the same walk as a plain histogram for '*' / satadd (rbi_kernels.cu uses it for 1024 < w <= 12288)
 int rbi_ms_hist_tables(int64_t n, int64_t w);
 int launch_ms_hist(int mul, int count_zeros, float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
-                   float *part, unsigned *zeros, cudaStream_t stream);
+                   float *part, unsigned *zeros, int ld, cudaStream_t stream);
 int launch_rbi_multiscan_vjp(int gcode, double param, int64_t n, int64_t w, const int64_t *is, const float *vs,
                              const float *hist_bar, float *vs_bar, void *ws, int accumulate, cudaStream_t stream);
 int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorted_keys,

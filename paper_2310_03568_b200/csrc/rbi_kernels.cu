@@ -1131,11 +1131,12 @@ bool rbi_cached_supported(int64_t w) { return w <= ((int64_t)CB_PART << CB_MAX_S
 // Accumulates into part[G][w]; returns G in *G_out.
 template <int ACC, bool COUNT_ZEROS>
 static int run_cached(int64_t n, int64_t w, const int64_t *is, const float *vs, float *part,
-                      unsigned *zeros, float S, int *G_out, cudaStream_t stream) {
+                      unsigned *zeros, float S, int *G_out, cudaStream_t stream, int ld = 0) {
     const int G = cached_grid(n, w);
     *G_out = cached_tables(n, w);
     if (cached_walk(w))
-        return launch_ms_hist(ACC == ACC_MUL, COUNT_ZEROS, S, n, w, is, vs, part, zeros, stream);
+        return launch_ms_hist(ACC == ACC_MUL, COUNT_ZEROS, S, n, w, is, vs, part, zeros, ld, stream);
+    if (ld != 0) return VJP_ERR_UNSUPPORTED;  // virtual keys: the walk only (rbi_mul_vec_fused)
     if (w <= CS_SLOTS) {
         auto kern = rbi_cached_small_kernel<ACC, COUNT_ZEROS>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CS_SMEM) != cudaSuccess)
@@ -1196,11 +1197,12 @@ rbi_mul_finish_kernel(int64_t w, int G, const float *__restrict__ part,
 
 // Return sweep (Fig. 3): no zero in the bin -> (y / a) * ybar; exactly one
 // zero and a is that zero -> y^{>0} * ybar; otherwise 0.  Out-of-range keys get 0.
-template <bool SMEM>
+// VEC: flat arrays of the vectorised operator with virtual keys is[j >> ld] << ld | (j & (d - 1)) (see ms_hist_kernel).
+template <bool SMEM, bool VEC = false>
 __global__ void __launch_bounds__(RBI_NT)
 rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                      const float *__restrict__ vs, const float2 *__restrict__ coef,
-                     float *__restrict__ vs_bar, int accumulate) {
+                     float *__restrict__ vs_bar, int accumulate, int ld = 0) {
     extern __shared__ uint4 smem_raw[];
     float2 *sh = reinterpret_cast<float2 *>(smem_raw);
     if (SMEM) {
@@ -1211,7 +1213,18 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     for (int64_t q = blockIdx.x * (int64_t)RBI_NT + threadIdx.x; q * 4 < n; q += stride) {
         int64_t k[4];
         float v[4], o[4];
-        const int cnt = load_keys4(is, q * 4, n, k);
+        int cnt;
+        if constexpr (VEC) {
+            cnt = (int)min((int64_t)4, n - q * 4);
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                const int64_t idx = q * 4 + j;
+                const int64_t kr = j < cnt ? __ldg(is + (idx >> ld)) : (int64_t)-1;
+                k[j] = in_range(kr, w >> ld) ? (kr << ld) | (idx & (((int64_t)1 << ld) - 1)) : (int64_t)-1;
+            }
+        } else {
+            cnt = load_keys4(is, q * 4, n, k);
+        }
         load_vals4(vs, q * 4, cnt, v);
         // the four coefficient gathers are issued together (clamped index, unconditional load): one L2 round
         // trip per quad instead of four dependent ones (profiles/r2c: 32 long-scoreboard stall cycles per issue)
@@ -1249,9 +1262,15 @@ static MulWs mul_carve(void *ws, int64_t w) {
     return m;
 }
 
+bool rbi_mul_vec_fused(int64_t n, int64_t w, int ld) {
+    return ld > 0 && ld < 12 && cached_walk(w << ld) && (n << ld) < (int64_t)0xfffffffell;
+}
+
+// ld > 0: n, w, vs, hist_bar, vs_bar are the FLAT sizes / arrays of `map2 (*)` on rows of 2^ld scalars, `is` has
+// n >> ld keys (rbi_mul_vec_fused says whether this form is available).
 int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
                    const float *hist_bar, float *vs_bar, int64_t *zeros, float *prod_nz, void *ws,
-                   int accumulate, cudaStream_t stream) {
+                   int accumulate, cudaStream_t stream, int ld) {
     if (w == 0) {
         if (vs_bar && n > 0 && !accumulate &&
             cudaMemsetAsync(vs_bar, 0, (size_t)n * sizeof(float), stream) != cudaSuccess)
@@ -1262,7 +1281,7 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     MulWs m = mul_carve(ws, w);
     if (cudaMemsetAsync(m.zeros, 0, (size_t)w * 4, stream) != cudaSuccess) return VJP_ERR_CUDA;
     int G = 0;
-    const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream);
+    const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream, ld);
     if (rc != VJP_OK) return rc;
     if (fold_chains(G) == 32)
         VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<32><<<fold_grid(w), 1024, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
@@ -1273,7 +1292,11 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     if (vs_bar && n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         const size_t bytes = (size_t)w * sizeof(float2);
-        if (bytes <= GATHER_SMEM_MAX / 2)
+        if (ld > 0) {  // w <= 12288 virtual bins: 96 KB of coefficients at most
+            auto kern = rbi_mul_sweep_kernel<true, true>;
+            if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 12288 * 8) != cudaSuccess) return VJP_ERR_CUDA;
+            VJP_LAUNCH(K_MUL_SWEEP, stream) kern<<<bytes > 48 * 1024 ? NUM_SMS_B200 * 2 : grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar, accumulate, ld);
+        } else if (bytes <= GATHER_SMEM_MAX / 2)
             VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<true><<<grid, RBI_NT, bytes, stream>>>(n, w, is, vs, m.coef, vs_bar, accumulate);
         else
             VJP_LAUNCH(K_MUL_SWEEP, stream) rbi_mul_sweep_kernel<false><<<grid, RBI_NT, 0, stream>>>(n, w, is, vs, m.coef, vs_bar, accumulate);

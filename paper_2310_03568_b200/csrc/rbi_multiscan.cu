@@ -332,10 +332,14 @@ ms_backward_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const f
 // epilogue folds the CTA's warp tables in warp order into ONE partial table per CTA (deterministic), which the fold
 // kernels of rbi_kernels.cu combine.  COUNT_ZEROS (the lifted '*' of P:L460): an exact zero is counted in zeros[bin]
 // and takes no part in the product.
-template <int CODE, int WMAX, int D, bool COUNT_ZEROS>
+// VEC (the vectorised operator `map2 (.)` on rows of d = 2^ld scalars, eq. 3 P:L252-263 / P:L464-466): reduce_by_index
+// with map2 (.) is d independent histograms = ONE histogram over (bin, column) pairs.  The [n][d] values are walked as
+// a flat array of n * d scalars whose element j has the virtual key is[j >> ld] * d + (j & (d - 1)), with w * d
+// virtual bins: the keys are read once per row, nothing is transposed.  Here n and w are the FLAT sizes.
+template <int CODE, int WMAX, int D, bool COUNT_ZEROS, bool VEC>
 __global__ void __launch_bounds__(WMAX * 32, 1)
 ms_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float *__restrict__ vs,
-               float *__restrict__ part, unsigned *zeros, int64_t R, GenOp<CODE> op) {
+               float *__restrict__ part, unsigned *zeros, int64_t R, GenOp<CODE> op, int ld) {
     extern __shared__ float ms_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, wpc = blockDim.x >> 5;
     float *tab = ms_smem + (size_t)warp * (size_t)w;
@@ -349,11 +353,10 @@ ms_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float
     float vn[D];
     auto fetch = [&](int64_t rb) {
         if (rb + D <= rfull) {
-            const int64_t *kp = is + rb * 32 + lane;
             const float *vp = vs + rb * 32 + lane;
 #pragma unroll
             for (int d = 0; d < D; d++) {
-                kn[d] = __ldg(kp + d * 32);
+                kn[d] = __ldg(is + (VEC ? (rb * 32 + lane + d * 32) >> ld : rb * 32 + lane + d * 32));
                 vn[d] = __ldg(vp + d * 32);
             }
         } else {
@@ -361,7 +364,7 @@ ms_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float
             for (int d = 0; d < D; d++) {
                 const int64_t idx = (rb + d) * 32 + lane;
                 const bool ok = (rb + d < r1) & (idx < n);
-                kn[d] = ok ? __ldg(is + idx) : (int64_t)-1;
+                kn[d] = ok ? __ldg(is + (VEC ? idx >> ld : idx)) : (int64_t)-1;
                 vn[d] = ok ? __ldg(vs + idx) : 1.f;
             }
         }
@@ -374,6 +377,10 @@ ms_hist_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is, const float
         for (int d = 0; d < D; d++) {
             k[d] = kn[d];
             v[d] = vn[d];
+            if constexpr (VEC) {  // virtual key (bin, column); a key outside [0, w >> ld) stays out of range
+                const int64_t col = ((rb + d) * 32 + lane) & (((int64_t)1 << ld) - 1);
+                k[d] = (uint64_t)k[d] < (uint64_t)(w >> ld) ? (k[d] << ld) | col : (int64_t)-1;
+            }
         }
         fetch(rb + D);
 #pragma unroll
@@ -538,32 +545,37 @@ static MsShape ms_hist_shape(int64_t n, int64_t w) { return ms_shape(n < 1 ? 1 :
 // number of partial tables launch_ms_hist writes (= its grid)
 int rbi_ms_hist_tables(int64_t n, int64_t w) { return ms_hist_shape(n, w).grid; }
 
-template <int CODE, bool COUNT_ZEROS>
+template <int CODE, bool COUNT_ZEROS, bool VEC>
 static int ms_hist_run(float S, int64_t n, int64_t w, const int64_t *is, const float *vs, float *part, unsigned *zeros,
-                       cudaStream_t stream) {
+                       int ld, cudaStream_t stream) {
     const MsShape s = ms_hist_shape(n, w);
     const GenOp<CODE> op{S};
     const size_t smem = (size_t)s.wpc * (size_t)w * 4;
     if (s.wpc <= 16) {
-        auto k = ms_hist_kernel<CODE, 16, 8, COUNT_ZEROS>;
+        auto k = ms_hist_kernel<CODE, 16, 8, COUNT_ZEROS, VEC>;
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess) return VJP_ERR_CUDA;
-        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op);
+        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op, ld);
     } else {
-        auto k = ms_hist_kernel<CODE, 32, 2, COUNT_ZEROS>;
+        auto k = ms_hist_kernel<CODE, 32, 2, COUNT_ZEROS, VEC>;
         if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MS_SMEM_BUDGET) != cudaSuccess) return VJP_ERR_CUDA;
-        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op);
+        VJP_LAUNCH(K_MS_HIST, stream) k<<<s.grid, s.wpc * 32, smem, stream>>>(n, w, is, vs, part, zeros, s.R, op, ld);
     }
     return last_launch_status();
 }
 
-// part[rbi_ms_hist_tables(n, w)][w] partial histograms of '*' (mul != 0; count_zeros: the lifted form) or satadd
+// part[rbi_ms_hist_tables(n, w)][w] partial histograms of '*' (mul != 0; count_zeros: the lifted form) or satadd.
+// ld > 0 ('*' with zero counts only): the vectorised form, n and w flat (see ms_hist_kernel).
 int launch_ms_hist(int mul, int count_zeros, float S, int64_t n, int64_t w, const int64_t *is, const float *vs,
-                   float *part, unsigned *zeros, cudaStream_t stream) {
-    if (mul) {
-        return count_zeros ? ms_hist_run<G_MUL, true>(S, n, w, is, vs, part, zeros, stream)
-                           : ms_hist_run<G_MUL, false>(S, n, w, is, vs, part, zeros, stream);
+                   float *part, unsigned *zeros, int ld, cudaStream_t stream) {
+    if (ld > 0) {
+        if (!mul || !count_zeros) return VJP_ERR_UNSUPPORTED;
+        return ms_hist_run<G_MUL, true, true>(S, n, w, is, vs, part, zeros, ld, stream);
     }
-    return ms_hist_run<G_SATADD, false>(S, n, w, is, vs, part, zeros, stream);
+    if (mul) {
+        return count_zeros ? ms_hist_run<G_MUL, true, false>(S, n, w, is, vs, part, zeros, 0, stream)
+                           : ms_hist_run<G_MUL, false, false>(S, n, w, is, vs, part, zeros, 0, stream);
+    }
+    return ms_hist_run<G_SATADD, false, false>(S, n, w, is, vs, part, zeros, 0, stream);
 }
 
 }  // namespace vjp

@@ -88,3 +88,29 @@ def test_f3_rbi_vec_full_size(opname):
         assert nrel(got, ref) <= 1e-4
     else:
         assert np.array_equal(got.astype(np.float64), ref)
+
+
+# `map2 (*)` with d a power of two and 1024 < w * d <= 12288 runs FUSED: one scalar '*' problem on the flat [n * d] array
+# with virtual keys (bin, column) -- no transposes (csrc: ms_hist_kernel<VEC>, rbi_mul_sweep_kernel<VEC>).  The shapes
+# below sit on both sides of every condition (d = 6: not a power of two; w * d = 1024 and 12292: outside the range).
+@pytest.mark.parametrize("n,d,w", [(1, 2, 600), (33, 4, 300), (50021, 4, 1024), (100003, 2, 513), (65537, 8, 1536),
+                                   (40001, 16, 768), (70001, 4, 3072), (30011, 4, 256), (30011, 4, 3073), (30011, 6, 500)])
+def test_rbi_vec_mul_fused_matches_oracle(n, d, w):
+    data = W.f3_rbi_vec("mul", n=n, d=d, w=w, zero_rate=min(0.3, 0.7 * w / n))
+    is_ = data["is_"].copy()
+    is_[::41] = w + 5                       # out of range on the high side: the virtual key must not alias bin 0 ... d
+    is_[::43] = -1
+    ref = oracle.vjp_rbi_vec("mul", w, is_, data["vss"], data["hist_bar"])
+    got = B.vjp_reduce_by_index_vec(B.Op.of("mul"), w, dev(is_), dev(data["vss"]), dev(data["hist_bar"])).cpu().numpy()
+    assert nrel(got, ref) <= 1e-4
+    oob = (is_ < 0) | (is_ >= w)
+    assert not got.reshape(n, d)[oob].any()
+    # the three branches of Fig. 3 per (bin, column): compare per column against the scalar entry point as well
+    for c in (0, d - 1):
+        col = B.vjp_reduce_by_index(B.Op.of("mul"), w, dev(is_), dev(data["vss"][:, c]), dev(data["hist_bar"][:, c]))
+        assert nrel(got.reshape(n, d)[:, c], col.cpu().numpy()) <= 1e-4
+    # accumulate: out += contribution
+    prior = np.random.default_rng(n).standard_normal((n, d)).astype(np.float32)
+    out = dev(prior).view(-1)
+    B.vjp_reduce_by_index_vec(B.Op.of("mul", accumulate=True), w, dev(is_), dev(data["vss"]), dev(data["hist_bar"]), out=out)
+    assert nrel(out.cpu().numpy().reshape(n, d).astype(np.float64) - prior, ref) <= 1e-4
