@@ -48,6 +48,7 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
         "seg_reverse_vjp_kernel": 16 + 4,
         "ms_forward_kernel": 8 + 4 + 4,              # is + vs, l written
         "ms_backward_kernel": 8 + 4 + 4 + 4,         # is + vs + l, vs_bar written
+        "ms_hist_kernel": 8 + 4,                     # is + vs
     }
     return float(table.get(name, 0.0))
 
