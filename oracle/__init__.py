@@ -271,3 +271,54 @@ def vjp_scan_vec(op, xss, yss_bar):
     """xss_bar [n, d] of the inclusive scan with map2 (.) over rows of d scalars: the scalar rule per column."""
     xss, yss_bar = _f64(xss), _f64(yss_bar)
     return np.stack([vjp_scan(op, xss[:, c], yss_bar[:, c]) for c in range(xss.shape[1])], axis=1)
+
+
+# ------------------------------------------------------------------ exclusive scan (NEXT row f4) -------------
+#
+# scan^exc (used by the paper in Fig. 2, P:L146-149):  ys_0 = e,  ys_i = x_0 (.) ... (.) x_{i-1}.  Output i of the
+# exclusive scan IS output i-1 of the inclusive scan of P:L515-529 (and output 0 is the constant e), so with the shift
+# matrix S (S y)_i = y_{i-1}:  d ys^exc / d xs = S . d ys^inc / d xs,  and  xs_bar = (d ys^inc / d xs)^T (S^T ys_bar):
+# the inclusive return sweep (P:L553-558) applied to ys_bar moved down by one element, with a zero in the last place.
+# x_{n-1} enters no output: its adjoint is 0.
+
+def scan_neutral(op, q: int = 0):
+    """The neutral element e of a scan operator as a row of its arity."""
+    op = _opcode(op)
+    if op == ADD:
+        return np.array([0.0])
+    if op == MUL:
+        return np.array([1.0])
+    if op == MIN:
+        return np.array([np.inf])
+    if op == MAX:
+        return np.array([-np.inf])
+    if op == LINREC:
+        return np.array([1.0, 0.0])          # (a, b) = (1, 0): the identity map x -> 1 x + 0
+    if op == MATMUL:
+        return np.eye(q).ravel()
+    raise ValueError("not a scan operator")
+
+
+def scan_exclusive_forward(op, xs, q: int = 0):
+    """Exclusive scan: ys_0 = e, ys_i = x_0 (.) ... (.) x_{i-1}."""
+    xs = _f64(xs)
+    e = scan_neutral(op, q)
+    n = xs.size // e.size
+    ys = np.empty((n, e.size))
+    if n:
+        ys[0] = e
+        ys[1:] = scan_forward(op, xs, q).reshape(n, e.size)[:-1]
+    return ys.reshape(xs.shape)
+
+
+def vjp_scan_exclusive(op, xs, ys_bar, q: int = 0):
+    """Input adjoints of the exclusive scan: the inclusive return sweep on S^T ys_bar (see above)."""
+    xs, ys_bar = _f64(xs), _f64(ys_bar)
+    if xs.shape != ys_bar.shape:
+        raise ValueError("xs and ys_bar differ in shape")
+    d = scan_neutral(op, q).size
+    n = xs.size // d
+    moved = np.zeros((n, d))
+    if n:
+        moved[:-1] = ys_bar.reshape(n, d)[1:]
+    return vjp_scan(op, xs, moved.reshape(xs.shape), q)
