@@ -115,6 +115,18 @@ int scan_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
 int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar,
              void *ws, size_t ws_bytes, void *stream);
 
+/* Exclusive scan, the scan^exc of the paper's Fig. 2: ys_0 = e (the operator's neutral element),
+ * ys_i = x_0 (.) ... (.) x_{i-1}, and its input adjoints.  Output i is output i - 1 of the inclusive scan, so
+ * xs_bar = (the inclusive rule above) applied to ys_bar moved down by one element with a zero in the last place;
+ * x_{n-1} enters no output and gets adjoint 0.  Same operators, layouts, alignment and error behaviour as scan_forward
+ * / vjp_scan (xs may be NULL for ADD; op.accumulate adds to xs_bar); outputs must not alias inputs.  The workspace
+ * holds one array of n elements in addition to the inclusive calls' (vjp_scan_exclusive_workspace_bytes). */
+size_t vjp_scan_exclusive_workspace_bytes(const vjp_op_t *op, int64_t n);
+int scan_exclusive_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys,
+                           void *ws, size_t ws_bytes, void *stream);
+int vjp_scan_exclusive(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar,
+                       void *ws, size_t ws_bytes, void *stream);
+
 /* The '+' rule of vjp_scan (f32: xs_bar = reverse inclusive sum of ys_bar) for callers that cannot
  * allocate and cannot pass a workspace (code under CUDA graph capture, tight serving loops, harnesses that forbid
  * cudaMalloc).  Same kernel as vjp_scan(VJP_OP_ADD, VJP_F32); its scratch (ticket + look-back slots, 131 328 bytes)

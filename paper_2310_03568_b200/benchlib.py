@@ -169,13 +169,14 @@ VJP_BYTES_PER_ELEM = {  # algorithmic bytes of the whole VJP call per element (D
     "c5_rbi_satadd": 36, "c5_rbi_satadd_sorted": 88,
     "f2_reduce_add": 4, "f2_reduce_min": 8, "f2_reduce_mul": 12,   # fill / read + zero-fill / read, read, write
     "f4_scan_matmul3": 144, "f4_scan_min": 16,
+    "f4_scan_exc_linrec": 32 + 16,   # the inclusive rule + the move of ys_bar by one element (read 8, write 8)
     "f3_rbi_vec_mul": (8 + 16) + (8 + 16 + 16),   # per ROW of d = 4, fused: lifted primal (key + row) + sweep (key + row read, row written)
     "f1_sop_inv": 40, "f1_sop_general": 40, "f1_sop_general_sorted": 40,   # primal pass (8 + 8 read) + sweep (8 + 8 read, 8 write): the invertible rule's bytes, used for both rules
 }
 PRIMAL_BYTES_PER_ELEM = {
     "c1_rbi_add": 12, "c2_rbi_min": 12, "c2_rbi_mul": 12, "c3_scan_add_f32": 8, "c3_scan_mul_f64": 16,
     "c3_scan_linrec_f32": 16, "c4_scan_matmul2": 32, "c4_scan_matmul5": 200, "c5_rbi_satadd": 12, "c5_rbi_satadd_sorted": 12,
-    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f1_sop_inv": 16, "f1_sop_general": 16, "f1_sop_general_sorted": 16, "f3_rbi_vec_mul": 8 + 4 * 4,
+    "f2_reduce_add": 4, "f2_reduce_min": 4, "f2_reduce_mul": 4, "f4_scan_matmul3": 72, "f4_scan_min": 8, "f4_scan_exc_linrec": 16 + 16, "f1_sop_inv": 16, "f1_sop_general": 16, "f1_sop_general_sorted": 16, "f3_rbi_vec_mul": 8 + 4 * 4,
 }
 
 
@@ -226,16 +227,21 @@ class RbiCase:
 
 
 class ScanCase:
-    def __init__(self, op: B.Op, d):
-        self.op, self.n = op, int(d["n"])
+    def __init__(self, op: B.Op, d, exclusive: bool = False):
+        self.op, self.n, self.exclusive = op, int(d["n"]), exclusive
         self.xs, self.yb = to_dev(d["xs"]), to_dev(d["ys_bar"])
         self.out = torch.empty_like(self.yb)
-        self.ws = torch.empty(max(256, B.vjp_scan_workspace_bytes(op, self.n)), dtype=torch.uint8, device="cuda")
+        need = B.vjp_scan_exclusive_workspace_bytes(op, self.n) if exclusive else B.vjp_scan_workspace_bytes(op, self.n)
+        self.ws = torch.empty(max(256, need), dtype=torch.uint8, device="cuda")
 
     def vjp(self):
+        if self.exclusive:
+            return B.vjp_scan_exclusive(self.op, self.xs, self.yb, out=self.out, ws=self.ws)
         return B.vjp_scan(self.op, self.xs, self.yb, out=self.out, ws=self.ws)
 
     def primal(self):
+        if self.exclusive:
+            return B.scan_exclusive_forward(self.op, self.xs, out=self.out, ws=self.ws)
         return B.scan_forward(self.op, self.xs, out=self.out, ws=self.ws)
 
 
@@ -362,6 +368,8 @@ def case_table(scale=1.0):
     t.append(("f4_scan_matmul3", "f4 scan matmul 3x3 f32 n=2^22 (NEXT row)",
               scan("matmul3", lambda: W.c4_scan_matmul(3, n=sz(1 << 22)))))
     t.append(("f4_scan_min", "f4 scan min f32 n=2^26 (NEXT row)", scan("min", lambda: W.c3_scan_add(n=n3))))
+    t.append(("f4_scan_exc_linrec", "f4 scan^exc (exclusive) linrec f32x2 n=2^26 (NEXT row)",
+              lambda: ScanCase(B.Op.of("linrec"), W.c3_scan_linrec(n=n3), exclusive=True)))
     for opname in ("add", "min", "mul"):  # NEXT row f2 (not a BASELINE config): reduce VJP, n = 2^24
         t.append(("f2_reduce_" + opname, "f2 reduce %s f32 n=2^24 (NEXT row)" % opname,
                   lambda opname=opname: ReduceCase(B.Op.of(opname), W.f2_reduce(opname, n=sz(1 << 24)))))

@@ -26,6 +26,7 @@ F32, F64 = 0, 1
 EXPORTS = [
     "vjp_scan_arity", "vjp_version", "vjp_scan_workspace_bytes", "scan_forward", "vjp_scan",
     "vjp_scan_host_scratch_bytes", "vjp_scan_host", "vjp_scan_add_f32_noalloc_max_n", "vjp_scan_add_f32_noalloc",
+    "vjp_scan_exclusive_workspace_bytes", "scan_exclusive_forward", "vjp_scan_exclusive",
     "vjp_reduce_by_index_workspace_bytes",
     "reduce_by_index_forward", "vjp_reduce_by_index", "vjp_reduce_by_index_host_scratch_bytes",
     "vjp_reduce_by_index_host", "vjp_reduce_by_index_host_async", "rbi_argext", "rbi_zero_prod", "rbi_sort_perm",
@@ -92,6 +93,9 @@ def load() -> ctypes.CDLL:
         "vjp_scan": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_scan_host_scratch_bytes": (sz, [opp, i64]),
         "vjp_scan_host": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
+        "vjp_scan_exclusive_workspace_bytes": (sz, [opp, i64]),
+        "scan_exclusive_forward": (ctypes.c_int, [opp, i64, vp, vp, vp, sz, vp]),
+        "vjp_scan_exclusive": (ctypes.c_int, [opp, i64, vp, vp, vp, vp, sz, vp]),
         "vjp_scan_add_f32_noalloc_max_n": (i64, []),
         "vjp_scan_add_f32_noalloc": (ctypes.c_int, [i64, vp, vp, ctypes.c_int, vp]),
         "vjp_reduce_by_index_workspace_bytes": (sz, [opp, i64, i64]),
@@ -226,6 +230,41 @@ def vjp_scan(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -
     o = op.c()
     _check(load().vjp_scan(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                            _stream(stream)), "vjp_scan")
+    return xs_bar
+
+
+def vjp_scan_exclusive_workspace_bytes(op: Op, n: int) -> int:
+    o = op.c()
+    return load().vjp_scan_exclusive_workspace_bytes(ctypes.byref(o), n)
+
+
+def scan_exclusive_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
+    """ys_0 = e, ys_i = x_0 (.) ... (.) x_{i-1} (scan^exc, P:L146-149)."""
+    xs = _dev(xs, op.torch_dtype, what="xs")
+    n = _scan_n(op, xs)
+    ys = torch.empty_like(xs) if out is None else _out(out, op.torch_dtype, xs.numel(), xs.device)
+    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n), xs.device, ws)
+    o = op.c()
+    _check(load().scan_exclusive_forward(ctypes.byref(o), n, _ptr(xs), _ptr(ys), _ptr(ws), ws.numel(), _stream(stream)),
+           "scan_exclusive_forward")
+    return ys
+
+
+def vjp_scan_exclusive(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
+    """xs_bar = J^T ys_bar of the exclusive scan.  xs may be None for '+'."""
+    ys_bar = _dev(ys_bar, op.torch_dtype, what="ys_bar")
+    if xs is not None:
+        xs = _dev(xs, op.torch_dtype, what="xs")
+        if xs.shape != ys_bar.shape:
+            raise VjpError("xs and ys_bar differ in shape")
+    n = _scan_n(op, ys_bar)
+    if out is None and op.accumulate:
+        raise VjpError("accumulate needs the tensor to add to (out=)")
+    xs_bar = torch.empty_like(ys_bar) if out is None else _out(out, op.torch_dtype, ys_bar.numel(), ys_bar.device)
+    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n), ys_bar.device, ws)
+    o = op.c()
+    _check(load().vjp_scan_exclusive(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
+                                     _stream(stream)), "vjp_scan_exclusive")
     return xs_bar
 
 

@@ -63,7 +63,7 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "seg_reverse_vjp_kernel", "sort_export_kernel",
     "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel",
     "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel", "rows_to_cols / cols_to_rows",
-    "ms_forward_kernel", "ms_seg_agg / ms_carry_kernel", "ms_backward_kernel", "ms_hist_kernel"};
+    "ms_forward_kernel", "ms_seg_agg / ms_carry_kernel", "ms_backward_kernel", "ms_hist_kernel", "shift_words_kernel"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];
@@ -165,6 +165,66 @@ int vjp_scan(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, 
     if (xs_bar == ys_bar && (op->code != VJP_OP_ADD || op->accumulate)) return VJP_ERR_INVALID_ARG;  // in place: '+' only
     if (ws_bytes < scan_workspace_bytes(op->code, op->dtype, n)) return VJP_ERR_WORKSPACE;
     return launch_scan_vjp(op->code, op->dtype, n, xs, ys_bar, xs_bar, ws, op->accumulate, as_stream(stream));
+}
+
+// ------------------------------------------------------------------ exclusive scan -------
+// Words of the neutral element of a scan operator (EW = arity * dtype words); returns EW.
+static int neutral_words(const vjp_op_t *op, ShiftFill &f) {
+    const int arity = vjp_scan_arity(op);
+    const bool f64 = op->dtype == VJP_F64;
+    for (int i = 0; i < 32; i++) f.w[i] = 0u;
+    switch (op->code) {
+    case VJP_OP_ADD: break;
+    case VJP_OP_MUL: if (f64) f.w[1] = 0x3ff00000u; else f.w[0] = 0x3f800000u; break;
+    case VJP_OP_MIN: f.w[0] = 0x7f800000u; break;   // +inf
+    case VJP_OP_MAX: f.w[0] = 0xff800000u; break;   // -inf
+    case VJP_OP_LINREC: f.w[0] = 0x3f800000u; break;  // (a, b) = (1, 0)
+    default: {
+        const int q = arity == 4 ? 2 : arity == 9 ? 3 : 5;
+        for (int i = 0; i < q; i++) f.w[i * q + i] = 0x3f800000u;
+    }
+    }
+    return arity * (f64 ? 2 : 1);
+}
+static size_t exc_tmp_bytes(const vjp_op_t *op, int64_t n) {
+    return align_up((size_t)n * vjp_scan_arity(op) * dtype_bytes(op->dtype), 256);
+}
+
+size_t vjp_scan_exclusive_workspace_bytes(const vjp_op_t *op, int64_t n) {
+    if (!op_ok(op) || !scan_supported(op) || n < 0) return 0;
+    return exc_tmp_bytes(op, n) + scan_workspace_bytes(op->code, op->dtype, n);
+}
+
+int scan_exclusive_forward(const vjp_op_t *op, int64_t n, const void *xs, void *ys, void *ws, size_t ws_bytes,
+                           void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!xs || !ys || !ws || !all_aligned(xs, ys, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < vjp_scan_exclusive_workspace_bytes(op, n)) return VJP_ERR_WORKSPACE;
+    ShiftFill fill;
+    const int ew = neutral_words(op, fill);
+    char *tmp = static_cast<char *>(ws), *inner = tmp + exc_tmp_bytes(op, n);
+    const int rc = launch_scan_forward(op->code, op->dtype, n, xs, tmp, inner, as_stream(stream));
+    if (rc != VJP_OK) return rc;
+    return launch_shift_words(n * ew, ew, tmp, ys, fill, as_stream(stream));   // ys_0 = e, ys_i = inclusive_{i-1}
+}
+
+int vjp_scan_exclusive(const vjp_op_t *op, int64_t n, const void *xs, const void *ys_bar, void *xs_bar, void *ws,
+                       size_t ws_bytes, void *stream) {
+    if (!op_ok(op) || n < 0) return VJP_ERR_INVALID_ARG;
+    if (!scan_supported(op)) return VJP_ERR_UNSUPPORTED;
+    if (n == 0) return VJP_OK;
+    if (!ys_bar || !xs_bar || !ws || (!xs && op->code != VJP_OP_ADD)) return VJP_ERR_INVALID_ARG;
+    if (!all_aligned(xs, ys_bar, xs_bar, ws)) return VJP_ERR_INVALID_ARG;
+    if (ws_bytes < vjp_scan_exclusive_workspace_bytes(op, n)) return VJP_ERR_WORKSPACE;
+    ShiftFill fill;
+    const int ew = neutral_words(op, fill);
+    char *tmp = static_cast<char *>(ws), *inner = tmp + exc_tmp_bytes(op, n);
+    // S^T ys_bar: the adjoint of output i + 1 belongs to inclusive output i; nothing flows into the last one
+    const int rc = launch_shift_words(n * ew, -ew, ys_bar, tmp, fill, as_stream(stream));
+    if (rc != VJP_OK) return rc;
+    return launch_scan_vjp(op->code, op->dtype, n, xs, tmp, xs_bar, inner, op->accumulate, as_stream(stream));
 }
 
 int64_t vjp_scan_add_f32_noalloc_max_n(void) { return scan_noalloc_max_n(); }

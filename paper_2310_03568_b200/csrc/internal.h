@@ -30,7 +30,7 @@ enum KernelId : int {
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
     K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP, K_VEC_TRANSPOSE,
-    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD, K_MS_HIST,
+    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD, K_MS_HIST, K_SHIFT_WORDS,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
@@ -95,6 +95,10 @@ int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorte
 int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream);
 int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, int accumulate,
                         cudaStream_t stream);
+
+// exclusive scan: move an array by `sh` 32-bit words (vec_rules.cu); fill = the words of the neutral element
+struct ShiftFill { uint32_t w[32]; };
+int launch_shift_words(int64_t nwords, int sh, const void *in, void *out, const ShiftFill &fill, cudaStream_t stream);
 
 // -------------------------------------------------------------------------- sumOfProd ---
 size_t rbi_sop_workspace_bytes(int64_t w);

@@ -52,4 +52,29 @@ int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, 
     return last_launch_status();
 }
 
+// ------------------------------------------------------------------ exclusive scan (scan^exc) ---
+//
+// Output i of the exclusive scan is output i - 1 of the inclusive one (output 0 is the neutral element), so the
+// exclusive variants are the inclusive kernels plus a move by one element (api.cu).  An element of 4 ... 100 bytes is
+// in general not 16-byte aligned after the move, so this works on 32-bit words:
+//   sh > 0:  out[i] = i < sh ? fill[i] : in[i - sh]      (towards higher indices, the neutral element in front)
+//   sh < 0:  out[i] = i - sh < nwords ? in[i - sh] : 0   (towards lower indices, zeros behind)
+__global__ void __launch_bounds__(TR_NT)
+shift_words_kernel(int64_t nwords, int sh, const uint32_t *__restrict__ in, uint32_t *__restrict__ out, ShiftFill fill) {
+    const int64_t stride = (int64_t)gridDim.x * TR_NT;
+    for (int64_t i = blockIdx.x * (int64_t)TR_NT + threadIdx.x; i < nwords; i += stride) {
+        uint32_t v;
+        if (sh > 0) v = i < sh ? fill.w[i] : __ldg(in + i - sh);
+        else v = i - sh < nwords ? __ldg(in + i - sh) : 0u;
+        out[i] = v;
+    }
+}
+
+int launch_shift_words(int64_t nwords, int sh, const void *in, void *out, const ShiftFill &fill, cudaStream_t stream) {
+    if (nwords == 0) return VJP_OK;
+    VJP_LAUNCH(K_SHIFT_WORDS, stream) shift_words_kernel<<<tr_grid(nwords), TR_NT, 0, stream>>>(
+        nwords, sh, static_cast<const uint32_t *>(in), static_cast<uint32_t *>(out), fill);
+    return last_launch_status();
+}
+
 }  // namespace vjp
