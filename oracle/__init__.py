@@ -267,10 +267,17 @@ def vjp_rbi_vec(op, num_bins, is_, vss, hist_bar, S: float = 0.0):
     return np.stack(cols, axis=1)
 
 
-def vjp_scan_vec(op, xss, yss_bar):
-    """xss_bar [n, d] of the inclusive scan with map2 (.) over rows of d scalars: the scalar rule per column."""
+def vjp_scan_vec(op, xss, yss_bar, q: int = 0):
+    """xss_bar [n, d * a] of the inclusive scan whose operator applies (.) (arity a) to each of the d blocks of a row:
+    a = 1 is map2 (.) on rows of d scalars (ISWIM); a > 1 is an operator with a block-diagonal Jacobian of
+    d DIFFERENT blocks (non-redundant BDS: "the computation of rs_bar is performed with k different scans").
+    Either way: the rule of the small operator per block column."""
     xss, yss_bar = _f64(xss), _f64(yss_bar)
-    return np.stack([vjp_scan(op, xss[:, c], yss_bar[:, c]) for c in range(xss.shape[1])], axis=1)
+    a = _load().orc_scan_arity(_opcode(op), q)
+    d = xss.shape[1] // a
+    cols = [vjp_scan(op, np.ascontiguousarray(xss[:, c * a:(c + 1) * a]), np.ascontiguousarray(yss_bar[:, c * a:(c + 1) * a]), q)
+            .reshape(xss.shape[0], a) for c in range(d)]
+    return np.concatenate(cols, axis=1)
 
 
 # ------------------------------------------------------------------ exclusive scan (NEXT row f4) -------------
