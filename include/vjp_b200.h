@@ -231,6 +231,9 @@ int rbi_sort_perm(int64_t n, int64_t num_bins, const int64_t *is, int64_t *sorte
  * reduce_by_index; ADD, MUL, MIN, MAX for scan), and the result is transposed back (op.accumulate fused there).
  * reduce_by_index with MUL, d a power of two and 1024 < num_bins * d <= 12288 skips the transposes: the d histograms
  * are one histogram over (bin, column) pairs, computed on the flat arrays with virtual keys is[j / d] * d + j % d.
+ * vjp_scan_vec also takes the operators of arity a > 1 (LINREC, MATMUL2 / 3 / 5): rows are d blocks of a scalars, the
+ * operator applies (.) to every block -- a block-diagonal Jacobian of d DIFFERENT blocks (non-redundant BDS,
+ * rs_bar by d scans with the scaled-down operator); xss, yss_bar, xss_bar are [n][d * a].
  * d <= 4096. */
 size_t vjp_reduce_by_index_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins);
 int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t num_bins, const int64_t *is,

@@ -443,21 +443,27 @@ def vjp_reduce_by_index_vec(op: Op, num_bins: int, is_: torch.Tensor, vss, hist_
 
 
 def vjp_scan_vec(op: Op, xss, yss_bar: torch.Tensor, out=None, ws=None, stream=None) -> torch.Tensor:
-    """xss_bar [n, d] of the inclusive scan with map2 (.) on rows of d scalars (ISWIM)."""
+    """xss_bar [n, d * a] of the inclusive scan whose operator applies `op` (arity a) to each of the d blocks of a row:
+    a = 1 is map2 (.) on rows of d scalars (ISWIM); a > 1 (linrec, matmul) is a block-diagonal operator of
+    d different blocks (non-redundant BDS)."""
     if yss_bar.dim() != 2:
-        raise VjpError("yss_bar must be [n, d]")
-    n, d = yss_bar.shape
-    yss_bar = _dev(yss_bar, torch.float32, n * d, "yss_bar")
+        raise VjpError("yss_bar must be [n, d * arity]")
+    a = scan_arity(op)
+    if a < 1 or yss_bar.shape[1] % a:
+        raise VjpError("row length is not a multiple of the operator's arity")
+    n, da = yss_bar.shape
+    d = da // a
+    yss_bar = _dev(yss_bar, torch.float32, n * da, "yss_bar")
     if xss is not None:
-        xss = _dev(xss, torch.float32, n * d, "xss")
+        xss = _dev(xss, torch.float32, n * da, "xss")
     if out is None and op.accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
-    xss_bar = _out(out, torch.float32, n * d, yss_bar.device, "xss_bar")
+    xss_bar = _out(out, torch.float32, n * da, yss_bar.device, "xss_bar")
     o = op.c()
     ws = _workspace(load().vjp_scan_vec_workspace_bytes(ctypes.byref(o), n, d), yss_bar.device, ws)
     _check(load().vjp_scan_vec(ctypes.byref(o), n, d, _ptr(xss), _ptr(yss_bar), _ptr(xss_bar), _ptr(ws), ws.numel(),
                                _stream(stream)), "vjp_scan_vec")
-    return xss_bar.view(n, d)
+    return xss_bar.view(n, da)
 
 
 # ------------------------------------------------------------------ sumOfProd ------------

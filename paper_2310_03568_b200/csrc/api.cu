@@ -435,15 +435,15 @@ struct VecWs {
     size_t total;
 };
 // columns are padded to a multiple of 4 floats so that every column start is 16-byte aligned
-VecWs vec_carve(void *ws, int64_t n, int64_t d, int64_t w, size_t inner_bytes) {
+VecWs vec_carve(void *ws, int64_t n, int64_t d, int64_t w, size_t inner_bytes, int64_t a = 1) {
     VecWs v;
     v.ncol = (n + 3) / 4 * 4;
     v.wcol = (w + 3) / 4 * 4;
     char *p = static_cast<char *>(ws);
     auto take = [&](size_t bytes) { char *r = p; p += align_up(bytes < 16 ? 16 : bytes, 256); return r; };
-    v.cols = reinterpret_cast<float *>(take((size_t)v.ncol * d * 4));
-    v.outs = reinterpret_cast<float *>(take((size_t)v.ncol * d * 4));
-    v.hbs = reinterpret_cast<float *>(take((size_t)v.wcol * d * 4));
+    v.cols = reinterpret_cast<float *>(take((size_t)v.ncol * d * a * 4));
+    v.outs = reinterpret_cast<float *>(take((size_t)v.ncol * d * a * 4));
+    v.hbs = reinterpret_cast<float *>(take((size_t)v.wcol * d * a * 4));
     v.inner = take(inner_bytes);
     v.total = (size_t)(p - static_cast<char *>(ws));
     return v;
@@ -503,34 +503,40 @@ int vjp_reduce_by_index_vec(const vjp_op_t *op, int64_t n, int64_t d, int64_t nu
 }
 
 size_t vjp_scan_vec_workspace_bytes(const vjp_op_t *op, int64_t n, int64_t d) {
-    if (!vec_op_ok(op) || n < 0 || d < 1 || vjp_scan_arity(op) != 1) return 0;
+    if (!vec_op_ok(op) || n < 0 || d < 1 || vjp_scan_arity(op) < 1) return 0;
     const size_t inner = vjp_scan_workspace_bytes(op, n);
-    return inner ? vec_carve(nullptr, n, d, n, inner).total : 0;  // hbs holds the transposed output adjoints
+    return inner ? vec_carve(nullptr, n, d, n, inner, vjp_scan_arity(op)).total : 0;  // hbs holds the transposed output adjoints
 }
 
+// Rows of d entries of a = arity(op) floats.  a = 1: scan with map2 (.) (ISWIM).  a > 1 (LINREC, MATMUL*):
+// the operator applies (.) to each of the d blocks of a row, its Jacobian is block-diagonal with d DIFFERENT blocks
+// (non-redundant BDS), and "the computation of rs_bar is performed with k different scans, each of them
+// using a scaled-down operator": the block columns are gathered, the small operator's rule runs on each, and the
+// result is put back.
 int vjp_scan_vec(const vjp_op_t *op, int64_t n, int64_t d, const void *xss, const void *yss_bar, void *xss_bar,
                  void *ws, size_t ws_bytes, void *stream) {
     if (!op_ok(op) || n < 0 || d < 1) return VJP_ERR_INVALID_ARG;
-    if (!vec_op_ok(op) || !scan_supported(op) || vjp_scan_arity(op) != 1 || d > 4096) return VJP_ERR_UNSUPPORTED;
+    if (!vec_op_ok(op) || !scan_supported(op) || vjp_scan_arity(op) < 1 || d > 4096) return VJP_ERR_UNSUPPORTED;
     if (n == 0) return VJP_OK;
+    const int a = vjp_scan_arity(op);
     const bool needs_xs = op->code != VJP_OP_ADD;
     if (!yss_bar || !xss_bar || !ws || (needs_xs && !xss)) return VJP_ERR_INVALID_ARG;
     if (!all_aligned(xss, yss_bar, xss_bar, ws)) return VJP_ERR_INVALID_ARG;
     const size_t inner = vjp_scan_workspace_bytes(op, n);
-    const VecWs v = vec_carve(ws, n, d, n, inner);  // hbs holds the transposed output adjoints
+    const VecWs v = vec_carve(ws, n, d, n, inner, a);  // hbs holds the transposed output adjoints
     if (ws_bytes < v.total) return VJP_ERR_WORKSPACE;
     cudaStream_t s = as_stream(stream);
     int rc;
-    if (needs_xs && (rc = launch_rows_to_cols(n, d, v.ncol, static_cast<const float *>(xss), v.cols, s)) != VJP_OK) return rc;
-    if ((rc = launch_rows_to_cols(n, d, v.wcol, static_cast<const float *>(yss_bar), v.hbs, s)) != VJP_OK) return rc;
+    if (needs_xs && (rc = launch_rows_to_cols(n, d, v.ncol, static_cast<const float *>(xss), v.cols, s, a)) != VJP_OK) return rc;
+    if ((rc = launch_rows_to_cols(n, d, v.wcol, static_cast<const float *>(yss_bar), v.hbs, s, a)) != VJP_OK) return rc;
     vjp_op_t col = *op;
     col.accumulate = 0;
     for (int64_t c = 0; c < d; c++) {  // ISWIM: scan (map2 (.)) = map (scan (.)) on the transpose
-        rc = vjp_scan(&col, n, needs_xs ? v.cols + c * v.ncol : nullptr, v.hbs + c * v.wcol, v.outs + c * v.ncol,
+        rc = vjp_scan(&col, n, needs_xs ? v.cols + c * v.ncol * a : nullptr, v.hbs + c * v.wcol * a, v.outs + c * v.ncol * a,
                       v.inner, inner, stream);
         if (rc != VJP_OK) return rc;
     }
-    return launch_cols_to_rows(n, d, v.ncol, v.outs, static_cast<float *>(xss_bar), op->accumulate != 0, s);
+    return launch_cols_to_rows(n, d, v.ncol, v.outs, static_cast<float *>(xss_bar), op->accumulate != 0, s, a);
 }
 
 // --------------------------------------------------------------------------- sumOfProd ----

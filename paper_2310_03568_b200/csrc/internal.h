@@ -92,9 +92,10 @@ int launch_rbi_sort_perm(int64_t n, int64_t w, const int64_t *is, int64_t *sorte
                          int64_t *perm, void *ws, cudaStream_t stream);
 
 // ---------------------------------------------------------------- vectorised operators ---
-int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream);
+// a = floats per entry (1: scalars; > 1: the blocks of a block-diagonal operator); cstride in entries
+int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream, int a = 1);
 int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, int accumulate,
-                        cudaStream_t stream);
+                        cudaStream_t stream, int a = 1);
 
 // exclusive scan: move an array by `sh` 32-bit words (vec_rules.cu); fill = the words of the neutral element
 struct ShiftFill { uint32_t w[32]; };

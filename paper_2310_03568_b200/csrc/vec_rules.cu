@@ -13,24 +13,27 @@ namespace vjp {
 constexpr int TR_NT = 256;
 
 // out[c * cstride + r] = in[r * d + c]   ([n][d] -> d columns of stride cstride); flat over the input, so the
-// reads are coalesced and a warp writes d runs of 32 / d consecutive floats
+// reads are coalesced and a warp writes d runs of 32 / d consecutive floats.  An "entry" is `a` consecutive floats
+// (a = 1: scalars; a > 1: the blocks of a block-diagonal operator); cstride counts entries.
 __global__ void __launch_bounds__(TR_NT)
-rows_to_cols_kernel(int64_t n, int64_t d, int64_t cstride, const float *__restrict__ in, float *__restrict__ out) {
-    const int64_t total = n * d, stride = (int64_t)gridDim.x * TR_NT;
+rows_to_cols_kernel(int64_t n, int64_t d, int64_t cstride, const float *__restrict__ in, float *__restrict__ out, int a) {
+    const int64_t total = n * d * a, stride = (int64_t)gridDim.x * TR_NT;
     for (int64_t e = blockIdx.x * (int64_t)TR_NT + threadIdx.x; e < total; e += stride) {
-        const int64_t r = e / d, c = e - r * d;
-        out[c * cstride + r] = __ldg(in + e);
+        const int64_t ent = e / a, j = e - ent * a;
+        const int64_t r = ent / d, c = ent - r * d;
+        out[(c * cstride + r) * a + j] = __ldg(in + e);
     }
 }
 
 // out[r * d + c] (+)= in[c * cstride + r]; flat over the output: coalesced writes
 __global__ void __launch_bounds__(TR_NT)
 cols_to_rows_kernel(int64_t n, int64_t d, int64_t cstride, const float *__restrict__ in, float *__restrict__ out,
-                    int accumulate) {
-    const int64_t total = n * d, stride = (int64_t)gridDim.x * TR_NT;
+                    int accumulate, int a) {
+    const int64_t total = n * d * a, stride = (int64_t)gridDim.x * TR_NT;
     for (int64_t e = blockIdx.x * (int64_t)TR_NT + threadIdx.x; e < total; e += stride) {
-        const int64_t r = e / d, c = e - r * d;
-        const float v = __ldg(in + c * cstride + r);
+        const int64_t ent = e / a, j = e - ent * a;
+        const int64_t r = ent / d, c = ent - r * d;
+        const float v = __ldg(in + (c * cstride + r) * a + j);
         out[e] = accumulate ? out[e] + v : v;
     }
 }
@@ -40,15 +43,15 @@ static int tr_grid(int64_t total) {
     return (int)(need < 1 ? 1 : (need < cap ? need : cap));
 }
 
-int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream) {
+int launch_rows_to_cols(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, cudaStream_t stream, int a) {
     if (n * d == 0) return VJP_OK;
-    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) rows_to_cols_kernel<<<tr_grid(n * d), TR_NT, 0, stream>>>(n, d, cstride, in, out);
+    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) rows_to_cols_kernel<<<tr_grid(n * d * a), TR_NT, 0, stream>>>(n, d, cstride, in, out, a);
     return last_launch_status();
 }
 int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, float *out, int accumulate,
-                        cudaStream_t stream) {
+                        cudaStream_t stream, int a) {
     if (n * d == 0) return VJP_OK;
-    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) cols_to_rows_kernel<<<tr_grid(n * d), TR_NT, 0, stream>>>(n, d, cstride, in, out, accumulate);
+    VJP_LAUNCH(K_VEC_TRANSPOSE, stream) cols_to_rows_kernel<<<tr_grid(n * d * a), TR_NT, 0, stream>>>(n, d, cstride, in, out, accumulate, a);
     return last_launch_status();
 }
 

@@ -114,3 +114,29 @@ def test_rbi_vec_mul_fused_matches_oracle(n, d, w):
     out = dev(prior).view(-1)
     B.vjp_reduce_by_index_vec(B.Op.of("mul", accumulate=True), w, dev(is_), dev(data["vss"]), dev(data["hist_bar"]), out=out)
     assert nrel(out.cpu().numpy().reshape(n, d).astype(np.float64) - prior, ref) <= 1e-4
+
+
+# Non-redundant block-diagonal sparsity: an operator that applies linrec / a q x q product to each of the
+# d blocks of its element = d scans with the scaled-down operator (vjp_scan_vec with an operator of arity > 1).
+@pytest.mark.parametrize("n", [1, 129, 4097, 30011])
+@pytest.mark.parametrize("opname,q,d", [("linrec", 0, 3), ("matmul2", 2, 2), ("matmul3", 3, 2), ("matmul5", 5, 2), ("linrec", 0, 1)])
+def test_scan_bds_vjp_matches_oracle(opname, q, d, n):
+    rng = np.random.default_rng([n, d, q])
+    a = 2 if opname == "linrec" else q * q
+    if opname == "linrec":
+        blocks = [np.stack([rng.uniform(0.9, 1.0, n), rng.standard_normal(n)], axis=1) for _ in range(d)]
+    else:
+        blocks = [W.c4_scan_matmul(q, n=n, seed=7 + c)["xs"].reshape(n, a) for c in range(d)]
+    xss = np.concatenate(blocks, axis=1).astype(np.float32)
+    ybar = rng.standard_normal((n, d * a)).astype(np.float32)
+    got = B.vjp_scan_vec(B.Op.of(opname), dev(xss), dev(ybar)).cpu().numpy()
+    ref = oracle.vjp_scan_vec("linrec" if opname == "linrec" else "matmul", xss, ybar, q=q)
+    assert got.shape == (n, d * a) and nrel(got, ref) <= 1e-4
+    for c in range(d):    # every block column equals the small operator's own VJP on that column
+        one = B.vjp_scan(B.Op.of(opname), dev(np.ascontiguousarray(xss[:, c * a:(c + 1) * a])),
+                         dev(np.ascontiguousarray(ybar[:, c * a:(c + 1) * a]))).cpu().numpy().reshape(n, a)
+        assert nrel(got[:, c * a:(c + 1) * a], one) <= 1e-5
+    prior = rng.standard_normal((n, d * a)).astype(np.float32)
+    out = dev(prior).view(-1)
+    B.vjp_scan_vec(B.Op.of(opname, accumulate=True), dev(xss), dev(ybar), out=out)
+    assert nrel(out.cpu().numpy().reshape(n, d * a).astype(np.float64) - prior, ref) <= 1e-4
