@@ -341,6 +341,7 @@ rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 // TAGGED = false: w <= 65536, slot = bin, 2-byte entries.  TAGGED = true: 32768 slots of
 // (bin >> 15) << 16 | prefix; a slot that holds another bin does not filter.
 constexpr int MMF_NT = 1024;
+constexpr int MMF_REFRESH_AT = 3;  // iterations of a CTA before its filter is refreshed from the table (1: 0.094, 3: 0.088, 1+4: 0.091 ms)
 constexpr size_t MMF_SMEM = 128 * 1024;
 
 template <bool IS_MAX, bool TAGGED>
@@ -362,7 +363,21 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
     for (int i = threadIdx.x; i < (int)(MMF_SMEM / 16); i += MMF_NT) smem_raw[i] = make_uint4(~0u, ~0u, ~0u, ~0u);
     __syncthreads();
+    // A CTA sees only n / (148 w) elements of a bin (1.7 at w = 2^16): on its own its filter learns a bound per bin
+    // once and never profits from it.  After MMF_REFRESH_AT of its iterations (~1/9 of the input, ~28 elements per
+    // bin seen by the grid as a whole) it therefore takes the bounds of ALL CTAs from the table, with coalesced
+    // loads: any value the table has held is an upper bound of the bin's minimum, so the filter stays valid whatever
+    // races with the per-element updates below, and from then on ~3 % of the elements reach L2 instead of ~60 %.
+    const int64_t total_it = (n / 4 + stride - 1) / stride;
+    int64_t it = 0;
     while (q * 4 < n) {
+        if (!TAGGED && it == MMF_REFRESH_AT && total_it >= 2 * MMF_REFRESH_AT) {
+            for (int b = threadIdx.x; b < (int)w; b += MMF_NT) {
+                const uint32_t g16 = (uint32_t)(__ldcg(tab + b) >> 48);
+                if (g16 < f16[b]) f16[b] = (uint16_t)g16;
+            }
+        }
+        it++;
         // next iteration's loads fly while this one walks the table (its L2 round trips are dependent)
         int64_t kn[4] = {-1, -1, -1, -1};
         float vn[4] = {0.f, 0.f, 0.f, 0.f};
@@ -376,7 +391,10 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
         }
-        // one element at a time (filter, table read, update): a hot bin's elements meet a fresh bound
+        if (TAGGED || it == 1) {
+        // The CTA's first iteration (and bins >= 2^16): one element at a time (filter, table read, update), so that a
+        // hot bin's elements meet a fresh bound -- with an open filter every element of a hot bin would otherwise send
+        // its own atomic to the one L2 sector (Zipf keys: 14 % of the elements).
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             if (!in_range(k[j], w)) continue;
@@ -402,6 +420,37 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             } else {
                 f16[b] = (uint16_t)c16;
             }
+        }
+        } else {
+        // Later iterations (the filter knows every bin that is hot): the quad's table reads are issued TOGETHER and its
+        // atomics are not waited for one by one -- four dependent L2 round trips per quad were the kernel's whole
+        // duration (28 iterations x 4 x ~1 us; 71 % of the stall samples on the two L2 waits, profiles/r2e).  A
+        // thread's own duplicates of a bin are resolved in registers first (only the smallest key goes on).
+        unsigned long long key[4], cur[4];
+        bool pass[4];
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const uint32_t vk = ext_key<IS_MAX>(v[j]);
+            key[j] = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
+            pass[j] = in_range(k[j], w) && !((vk >> 16) > f16[in_range(k[j], w) ? k[j] : 0]);
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++)
+#pragma unroll
+            for (int i = 0; i < 4; i++)
+                if (i != j && pass[j] && pass[i] && k[i] == k[j] && (key[i] < key[j])) pass[j] = false;
+#pragma unroll
+        for (int j = 0; j < 4; j++) cur[j] = pass[j] ? __ldcg(tab + k[j]) : 0ull;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            if (pass[j] && key[j] < cur[j]) {
+                const unsigned long long old = atomicMin(tab + k[j], key[j]);
+                cur[j] = key[j] < old ? key[j] : old;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++)
+            if (pass[j]) f16[k[j]] = (uint16_t)(cur[j] >> 48);
         }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
