@@ -391,8 +391,8 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
         }
-        if (TAGGED || it == 1) {
-        // The CTA's first iteration (and bins >= 2^16): one element at a time (filter, table read, update), so that a
+        if (TAGGED) {
+        // Histograms wider than 2^16 bins (tagged filter): one element at a time (filter, table read, update), so that a
         // hot bin's elements meet a fresh bound -- with an open filter every element of a hot bin would otherwise send
         // its own atomic to the one L2 sector (Zipf keys: 14 % of the elements).
 #pragma unroll
@@ -420,6 +420,33 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             } else {
                 f16[b] = (uint16_t)c16;
             }
+        }
+        } else if (it == 1) {
+        // The CTA's FIRST iteration, filter still open: with Zipf keys 14 % of the lanes hold the same bin and each would
+        // send its own atomic to the one L2 sector (40 % of the kernel's stall samples sat in this one iteration of 28,
+        // profiles/r2e).  The lanes of a warp that hold the same bin elect the smallest key (match.any + redux.min; equal
+        // values: the lowest lane = the lowest index); only that lane goes to L2, and its result sets the bin's filter.
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            const bool inr = in_range(k[j], w);
+            const uint32_t vk = ext_key<IS_MAX>(v[j]);
+            const uint32_t b = inr ? (uint32_t)k[j] : (0x80000000u | (threadIdx.x & 31u));
+            const unsigned grp = __match_any_sync(FULL_MASK, b);
+            if (!inr) continue;
+            if ((grp & (grp - 1u)) != 0u) {  // my bin is held by more than one lane (a redux per distinct mask is slow:
+                                             // with 32 singleton groups it cost the uniform case 9 us)
+                const uint32_t vmin = __reduce_min_sync(grp, vk);
+                const unsigned best = __ballot_sync(grp, vk == vmin);
+                if ((int)(threadIdx.x & 31u) != __ffs(best) - 1) continue;
+            }
+            if ((vk >> 16) > f16[b]) continue;
+            const unsigned long long key = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
+            unsigned long long cur = __ldcg(tab + k[j]);
+            if (key < cur) {
+                cur = atomicMin(tab + k[j], key);
+                if (key < cur) cur = key;
+            }
+            f16[b] = (uint16_t)(cur >> 48);
         }
         } else {
         // Later iterations (the filter knows every bin that is hot): the quad's table reads are issued TOGETHER and its
