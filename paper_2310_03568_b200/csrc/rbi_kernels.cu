@@ -471,8 +471,8 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             if (pass[j] && key[j] < cur[j]) {
-                const unsigned long long old = atomicMin(tab + k[j], key[j]);
-                cur[j] = key[j] < old ? key[j] : old;
+                atomicMin(tab + k[j], key[j]);  // result unused: a fire-and-forget RED, no third round trip
+                cur[j] = key[j];                // the table now holds key or less: a valid bound for the filter
             }
         }
 #pragma unroll
