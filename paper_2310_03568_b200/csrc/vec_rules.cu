@@ -65,17 +65,23 @@ int launch_cols_to_rows(int64_t n, int64_t d, int64_t cstride, const float *in, 
 __global__ void __launch_bounds__(TR_NT)
 shift_words_kernel(int64_t nwords, int sh, const uint32_t *__restrict__ in, uint32_t *__restrict__ out, ShiftFill fill) {
     const int64_t stride = (int64_t)gridDim.x * TR_NT;
-    for (int64_t i = blockIdx.x * (int64_t)TR_NT + threadIdx.x; i < nwords; i += stride) {
-        uint32_t v;
-        if (sh > 0) v = i < sh ? fill.w[i] : __ldg(in + i - sh);
-        else v = i - sh < nwords ? __ldg(in + i - sh) : 0u;
-        out[i] = v;
+    auto word = [&](int64_t i) -> uint32_t {
+        if (sh > 0) return i < sh ? fill.w[i] : __ldg(in + i - sh);
+        return i - sh < nwords ? __ldg(in + i - sh) : 0u;
+    };
+    // four words per thread: the loads are 4-byte (the source is not 16-byte aligned after the move) but hit the same
+    // lines across the warp; the store is one 128-bit access
+    const int64_t nq = nwords >> 2;
+    for (int64_t qd = blockIdx.x * (int64_t)TR_NT + threadIdx.x; qd < nq; qd += stride) {
+        const int64_t i = qd * 4;
+        reinterpret_cast<uint4 *>(out)[qd] = make_uint4(word(i), word(i + 1), word(i + 2), word(i + 3));
     }
+    for (int64_t i = nq * 4 + blockIdx.x * (int64_t)TR_NT + threadIdx.x; i < nwords; i += stride) out[i] = word(i);
 }
 
 int launch_shift_words(int64_t nwords, int sh, const void *in, void *out, const ShiftFill &fill, cudaStream_t stream) {
     if (nwords == 0) return VJP_OK;
-    VJP_LAUNCH(K_SHIFT_WORDS, stream) shift_words_kernel<<<tr_grid(nwords), TR_NT, 0, stream>>>(
+    VJP_LAUNCH(K_SHIFT_WORDS, stream) shift_words_kernel<<<tr_grid((nwords + 3) / 4), TR_NT, 0, stream>>>(
         nwords, sh, static_cast<const uint32_t *>(in), static_cast<uint32_t *>(out), fill);
     return last_launch_status();
 }
