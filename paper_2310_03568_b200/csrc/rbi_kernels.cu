@@ -1260,14 +1260,20 @@ template <int CH>
 __global__ void __launch_bounds__(32 * CH)
 rbi_mul_finish_kernel(int64_t w, int G, const float *__restrict__ part,
                       const unsigned *__restrict__ zeros_u, const float *__restrict__ hist_bar,
-                      int64_t *zeros, float *prod_nz, float2 *coef) {
+                      int64_t *zeros, float *prod_nz, float2 *coef, int planes) {
     const int64_t k = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     const float p = fold_partials<ACC_MUL, CH>(w, G, part, k, 0.f);
     if (threadIdx.x < 32 && k < w) {
         const unsigned z = zeros_u[k];
         if (zeros) zeros[k] = (int64_t)z;
         if (prod_nz) prod_nz[k] = p;
-        if (coef) coef[k] = make_float2(p * hist_bar[k], __int_as_float((int)(z < 2u ? z : 2u)));
+        if (coef && !planes) coef[k] = make_float2(p * hist_bar[k], __int_as_float((int)(z < 2u ? z : 2u)));
+        if (coef && planes) {  // wide histograms (table gathered from L1 / L2): two planes of w floats, see the sweep
+            float *pl = reinterpret_cast<float *>(coef);
+            const float c = p * hist_bar[k];
+            pl[k] = z == 0u ? c : 0.f;
+            pl[w + k] = z == 1u ? c : 0.f;
+        }
     }
 }
 
@@ -1304,19 +1310,37 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         load_vals4(vs, q * 4, cnt, v);
         // the four coefficient gathers are issued together (clamped index, unconditional load): one L2 round
         // trip per quad instead of four dependent ones (profiles/r2c: 32 long-scoreboard stall cycles per issue)
-        float2 c[4];
+        if constexpr (SMEM) {
+            float2 c[4];
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            const int64_t kk = in_range(k[j], w) ? k[j] : 0;
-            c[j] = SMEM ? sh[kk] : __ldg(coef + kk);
-        }
+            for (int j = 0; j < 4; j++) c[j] = sh[in_range(k[j], w) ? k[j] : 0];
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            const int z = __float_as_int(c[j].y);
-            float r = 0.f;
-            if (z == 0) r = c[j].x / v[j];
-            else if (z == 1 && v[j] == 0.f) r = c[j].x;
-            o[j] = in_range(k[j], w) ? r : 0.f;
+            for (int j = 0; j < 4; j++) {
+                const int z = __float_as_int(c[j].y);
+                float r = 0.f;
+                if (z == 0) r = c[j].x / v[j];
+                else if (z == 1 && v[j] == 0.f) r = c[j].x;
+                o[j] = in_range(k[j], w) ? r : 0.f;
+            }
+        } else {
+            // Wide histograms: the table comes through L1 / L2.  Two planes of w floats instead of (c, zero class) pairs:
+            // plane 0 = (z == 0 ? c : 0) is all a non-zero element needs (adjoint = plane0 / v: 0 as soon as its bin holds
+            // a zero) -- a 4-byte gather from a table of 256 KB at w = 2^16 (pairs: 512 KB against ~200 KB of L1), its
+            // address a function of the key alone; only an element that is 0 itself reads plane 1 = (z == 1 ? c : 0).
+            const float *pl = reinterpret_cast<const float *>(coef);
+            float c[4];
+#pragma unroll
+            for (int j = 0; j < 4; j++) c[j] = __ldg(pl + (in_range(k[j], w) ? k[j] : 0));
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                float r = 0.f;
+                if (v[j] == 0.f) {  // IEEE equality: +-0 only (Q7); rare
+                    if (in_range(k[j], w)) r = __ldg(pl + w + k[j]);
+                } else if (c[j] != 0.f) {
+                    r = c[j] / v[j];
+                }
+                o[j] = in_range(k[j], w) ? r : 0.f;
+            }
         }
         store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
     }
@@ -1359,12 +1383,13 @@ int launch_rbi_mul(int64_t n, int64_t w, const int64_t *is, const float *vs,
     int G = 0;
     const int rc = run_cached<ACC_MUL, true>(n, w, is, vs, m.part, m.zeros, 0.f, &G, stream, ld);
     if (rc != VJP_OK) return rc;
+    const int planes = ld == 0 && (size_t)w * sizeof(float2) > GATHER_SMEM_MAX / 2;  // the sweep's table form
     if (fold_chains(G) == 32)
         VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<32><<<fold_grid(w), 1024, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
-                                                                                              vs_bar ? m.coef : nullptr);
+                                                                                              vs_bar ? m.coef : nullptr, planes);
     else
         VJP_LAUNCH(K_MUL_FINISH, stream) rbi_mul_finish_kernel<8><<<fold_grid(w), 256, 0, stream>>>(w, G, m.part, m.zeros, hist_bar, zeros, prod_nz,
-                                                                                            vs_bar ? m.coef : nullptr);
+                                                                                            vs_bar ? m.coef : nullptr, planes);
     if (vs_bar && n > 0) {
         const int grid = grid_for(n, RBI_NT, RBI_CTAS_PER_SM);
         const size_t bytes = (size_t)w * sizeof(float2);
