@@ -46,6 +46,9 @@ class _OpStruct(ctypes.Structure):
                 ("force_general", ctypes.c_int32), ("accumulate", ctypes.c_int32)]
 
 
+_OP_STRUCTS = {}
+
+
 @dataclass(frozen=True)
 class Op:
     """Operator descriptor (vjp_op_t)."""
@@ -62,7 +65,10 @@ class Op:
                   bool(accumulate))
 
     def c(self) -> _OpStruct:
-        return _OpStruct(self.code, self.dtype, self.param, int(self.force_general), int(self.accumulate))
+        o = _OP_STRUCTS.get(self)  # the library only reads the descriptor: one struct per distinct Op
+        if o is None:
+            o = _OP_STRUCTS[self] = _OpStruct(self.code, self.dtype, self.param, int(self.force_general), int(self.accumulate))
+        return o
 
     @property
     def torch_dtype(self):
@@ -208,7 +214,7 @@ def scan_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=None) -> to
     xs = _dev(xs, op.torch_dtype, what="xs")
     n = _scan_n(op, xs)
     ys = torch.empty_like(xs) if out is None else _out(out, op.torch_dtype, xs.numel(), xs.device)
-    ws = _workspace(vjp_scan_workspace_bytes(op, n), xs.device, ws)
+    ws = _workspace(vjp_scan_workspace_bytes(op, n) if ws is None else 0, xs.device, ws)
     o = op.c()
     _check(load().scan_forward(ctypes.byref(o), n, _ptr(xs), _ptr(ys), _ptr(ws), ws.numel(), _stream(stream)),
            "scan_forward")
@@ -226,7 +232,7 @@ def vjp_scan(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stream=None) -
     if out is None and op.accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
     xs_bar = torch.empty_like(ys_bar) if out is None else _out(out, op.torch_dtype, ys_bar.numel(), ys_bar.device)
-    ws = _workspace(vjp_scan_workspace_bytes(op, n), ys_bar.device, ws)
+    ws = _workspace(vjp_scan_workspace_bytes(op, n) if ws is None else 0, ys_bar.device, ws)
     o = op.c()
     _check(load().vjp_scan(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                            _stream(stream)), "vjp_scan")
@@ -243,7 +249,7 @@ def scan_exclusive_forward(op: Op, xs: torch.Tensor, out=None, ws=None, stream=N
     xs = _dev(xs, op.torch_dtype, what="xs")
     n = _scan_n(op, xs)
     ys = torch.empty_like(xs) if out is None else _out(out, op.torch_dtype, xs.numel(), xs.device)
-    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n), xs.device, ws)
+    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n) if ws is None else 0, xs.device, ws)
     o = op.c()
     _check(load().scan_exclusive_forward(ctypes.byref(o), n, _ptr(xs), _ptr(ys), _ptr(ws), ws.numel(), _stream(stream)),
            "scan_exclusive_forward")
@@ -261,7 +267,7 @@ def vjp_scan_exclusive(op: Op, xs, ys_bar: torch.Tensor, out=None, ws=None, stre
     if out is None and op.accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
     xs_bar = torch.empty_like(ys_bar) if out is None else _out(out, op.torch_dtype, ys_bar.numel(), ys_bar.device)
-    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n), ys_bar.device, ws)
+    ws = _workspace(vjp_scan_exclusive_workspace_bytes(op, n) if ws is None else 0, ys_bar.device, ws)
     o = op.c()
     _check(load().vjp_scan_exclusive(ctypes.byref(o), n, _ptr(xs), _ptr(ys_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                                      _stream(stream)), "vjp_scan_exclusive")
@@ -324,7 +330,7 @@ def reduce_by_index_forward(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.
     n = is_.numel()
     vs = _dev(vs, op.torch_dtype, n, "vs")
     hist = _out(out, op.torch_dtype, num_bins, is_.device, "hist")
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins) if ws is None else 0, is_.device, ws)
     o = op.c()
     _check(load().reduce_by_index_forward(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist),
                                           _ptr(ws), ws.numel(), _stream(stream)), "reduce_by_index_forward")
@@ -342,7 +348,7 @@ def vjp_reduce_by_index(op: Op, num_bins: int, is_: torch.Tensor, vs, hist_bar: 
     if out is None and op.accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
     vs_bar = _out(out, op.torch_dtype, n, is_.device, "vs_bar")
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins) if ws is None else 0, is_.device, ws)
     o = op.c()
     _check(load().vjp_reduce_by_index(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar),
                                       _ptr(vs_bar), _ptr(ws), ws.numel(), _stream(stream)),
@@ -388,7 +394,7 @@ def rbi_argext(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws=No
     vs = _dev(vs, torch.float32, n, "vs")
     arg = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
     ext = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins) if ws is None else 0, is_.device, ws)
     o = op.c()
     _check(load().rbi_argext(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(arg), _ptr(ext), _ptr(ws),
                              ws.numel(), _stream(stream)), "rbi_argext")
@@ -402,7 +408,7 @@ def rbi_zero_prod(op: Op, num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ws
     vs = _dev(vs, torch.float32, n, "vs")
     zeros = torch.empty(num_bins, dtype=torch.int64, device=is_.device)
     prod = torch.empty(num_bins, dtype=torch.float32, device=is_.device)
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins), is_.device, ws)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(op, n, num_bins) if ws is None else 0, is_.device, ws)
     o = op.c()
     _check(load().rbi_zero_prod(ctypes.byref(o), n, num_bins, _ptr(is_), _ptr(vs), _ptr(zeros), _ptr(prod),
                                 _ptr(ws), ws.numel(), _stream(stream)), "rbi_zero_prod")
@@ -415,7 +421,7 @@ def rbi_sort_perm(num_bins: int, is_: torch.Tensor, ws=None, stream=None):
     n = is_.numel()
     sk = torch.empty(n, dtype=torch.int64, device=is_.device)
     perm = torch.empty(n, dtype=torch.int64, device=is_.device)
-    ws = _workspace(vjp_reduce_by_index_workspace_bytes(Op(OP_SATADD), n, num_bins), is_.device, ws)
+    ws = _workspace(vjp_reduce_by_index_workspace_bytes(Op(OP_SATADD), n, num_bins) if ws is None else 0, is_.device, ws)
     _check(load().rbi_sort_perm(n, num_bins, _ptr(is_), _ptr(sk), _ptr(perm), _ptr(ws), ws.numel(),
                                 _stream(stream)), "rbi_sort_perm")
     return sk, perm
@@ -460,7 +466,7 @@ def vjp_scan_vec(op: Op, xss, yss_bar: torch.Tensor, out=None, ws=None, stream=N
         raise VjpError("accumulate needs the tensor to add to (out=)")
     xss_bar = _out(out, torch.float32, n * da, yss_bar.device, "xss_bar")
     o = op.c()
-    ws = _workspace(load().vjp_scan_vec_workspace_bytes(ctypes.byref(o), n, d), yss_bar.device, ws)
+    ws = _workspace(load().vjp_scan_vec_workspace_bytes(ctypes.byref(o), n, d) if ws is None else 0, yss_bar.device, ws)
     _check(load().vjp_scan_vec(ctypes.byref(o), n, d, _ptr(xss), _ptr(yss_bar), _ptr(xss_bar), _ptr(ws), ws.numel(),
                                _stream(stream)), "vjp_scan_vec")
     return xss_bar.view(n, da)
@@ -478,7 +484,7 @@ def rbi_sumofprod_forward(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, ou
     n = is_.numel()
     vs = _dev(vs, torch.float32, 2 * n, "vs")
     hist = _out(out, torch.float32, 2 * num_bins, is_.device, "hist")
-    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins), is_.device, ws)
+    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins) if ws is None else 0, is_.device, ws)
     _check(load().rbi_sumofprod_forward(n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist), _ptr(ws), ws.numel(),
                                         _stream(stream)), "rbi_sumofprod_forward")
     return hist.view(num_bins, 2)
@@ -496,7 +502,7 @@ def vjp_rbi_sumofprod(num_bins: int, is_: torch.Tensor, vs: torch.Tensor, hist_b
     if out is None and accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
     vs_bar = _out(out, torch.float32, 2 * n, is_.device, "vs_bar")
-    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins, general), is_.device, ws)
+    ws = _workspace(rbi_sumofprod_workspace_bytes(n, num_bins, general) if ws is None else 0, is_.device, ws)
     _check(load().vjp_rbi_sumofprod(n, num_bins, _ptr(is_), _ptr(vs), _ptr(hist_bar), _ptr(vs_bar), int(general),
                                     int(accumulate), _ptr(ws), ws.numel(), _stream(stream)), "vjp_rbi_sumofprod")
     return vs_bar.view(n, 2)
@@ -514,7 +520,7 @@ def reduce_forward(op: Op, xs: torch.Tensor, ws=None, stream=None) -> torch.Tens
     xs = _dev(xs, op.torch_dtype, what="xs")
     n = xs.numel()
     y = torch.empty(1, dtype=op.torch_dtype, device=xs.device)
-    ws = _workspace(vjp_reduce_workspace_bytes(op, n), xs.device, ws)
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n) if ws is None else 0, xs.device, ws)
     o = op.c()
     _check(load().reduce_forward(ctypes.byref(o), n, _ptr(xs), _ptr(y), _ptr(ws), ws.numel(), _stream(stream)),
            "reduce_forward")
@@ -532,7 +538,7 @@ def vjp_reduce(op: Op, xs, y_bar: torch.Tensor, n=None, out=None, ws=None, strea
     if out is None and op.accumulate:
         raise VjpError("accumulate needs the tensor to add to (out=)")
     xs_bar = _out(out, op.torch_dtype, n, y_bar.device, "xs_bar")
-    ws = _workspace(vjp_reduce_workspace_bytes(op, n), y_bar.device, ws)
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n) if ws is None else 0, y_bar.device, ws)
     o = op.c()
     _check(load().vjp_reduce(ctypes.byref(o), n, _ptr(xs), _ptr(y_bar), _ptr(xs_bar), _ptr(ws), ws.numel(),
                              _stream(stream)), "vjp_reduce")
@@ -545,7 +551,7 @@ def reduce_lifted(op: Op, xs: torch.Tensor, ws=None, stream=None):
     n = xs.numel()
     ai = torch.empty(1, dtype=torch.int64, device=xs.device)
     av = torch.empty(1, dtype=torch.float32, device=xs.device)
-    ws = _workspace(vjp_reduce_workspace_bytes(op, n), xs.device, ws)
+    ws = _workspace(vjp_reduce_workspace_bytes(op, n) if ws is None else 0, xs.device, ws)
     o = op.c()
     _check(load().reduce_lifted(ctypes.byref(o), n, _ptr(xs), _ptr(ai), _ptr(av), _ptr(ws), ws.numel(),
                                 _stream(stream)), "reduce_lifted")
