@@ -303,7 +303,7 @@ rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         float v[4];
         const int cnt = load_keys4(is, q * 4, n, k);
         load_vals4(vs, q * 4, cnt, v);
-        if (vs_bar) {
+        if (vs_bar && cnt > 0) {
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
         }
@@ -370,7 +370,9 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     // races with the per-element updates below, and from then on ~3 % of the elements reach L2 instead of ~60 %.
     const int64_t total_it = (n / 4 + stride - 1) / stride;
     int64_t it = 0;
-    while (q * 4 < n) {
+    // The loop is WARP-uniform (the first iteration uses warp-wide match / redux): a lane whose quads are used up goes
+    // on with an empty quad (keys -1: out of range, nothing loaded, nothing stored) until its warp is done.
+    while (__any_sync(FULL_MASK, q * 4 < n)) {
         if (!TAGGED && it == MMF_REFRESH_AT && total_it >= 2 * MMF_REFRESH_AT) {
             for (int b = threadIdx.x; b < (int)w; b += MMF_NT) {
                 const uint32_t g16 = (uint32_t)(__ldcg(tab + b) >> 48);
@@ -387,7 +389,7 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             cntn = load_keys4(is, qn * 4, n, kn);
             load_vals4(vs, qn * 4, cntn, vn);
         }
-        if (vs_bar) {
+        if (vs_bar && cnt > 0) {
             const float z[4] = {0.f, 0.f, 0.f, 0.f};
             store_vals4(vs_bar, q * 4, cnt, z);
         }

@@ -220,6 +220,25 @@ def test_rbi_minmax_vjp_bit_exact(opname, dist, n, w):
     assert np.array_equal(got.astype(np.float64), ref)
 
 
+@pytest.mark.parametrize("n,w", [(1, 9000), (5, 20000), (33, 65536), (130, 9000), (4097, 65536), (4099, 70000), (131075, 65536)])
+@pytest.mark.parametrize("opname", ["min", "max"])
+def test_rbi_minmax_wide_histogram_ragged_sizes(opname, n, w):
+    """The filtered kernel (w > 8192) uses warp-wide match / redux in its first iteration: sizes that leave the last warp
+    (and the last quad) partly empty, with every lane of a warp on ONE bin (the election) and with ties."""
+    rng = np.random.default_rng([n, w, 5])
+    for hot in (False, True):
+        is_ = (np.full(n, w - 1, dtype=np.int64) if hot else rng.integers(-2, w + 2, size=n, dtype=np.int64))
+        vs = np.round(rng.standard_normal(n), 1).astype(np.float32)      # rounding forces ties: the lowest index wins
+        hb = rng.standard_normal(w).astype(np.float32)
+        op = B.Op.of(opname)
+        arg, ext = B.rbi_argext(op, w, dev(is_), dev(vs))
+        got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+        ref, rarg, rext = oracle.vjp_rbi_minmax(opname, w, is_, vs, hb)
+        assert np.array_equal(arg.cpu().numpy(), rarg)
+        assert np.array_equal(ext.cpu().numpy().astype(np.float64), rext)
+        assert np.array_equal(got.astype(np.float64), ref)
+
+
 def test_rbi_min_signed_zero_is_a_tie_and_infinities_are_values():
     # -0.0 == +0.0 under the paper's "<" (Q6): the lower index wins whatever the sign bit
     is_ = np.array([0, 0, 1, 1, 2, 2, 2], dtype=np.int64)
