@@ -248,8 +248,8 @@ int vjp_scan_vec(const vjp_op_t *op, int64_t n, int64_t d, const void *xss, cons
 /* reduce_by_index with the invertible operator sumOfProd (sections 3.3 and 4.2.4 of the paper):
  *   (p1,s1) sumOfProd (p2,s2) = (p1 + p2 + s1*s2, s1 + s2), neutral (0,0)
  * Elements are f32 pairs: vs [n][2] = (p, s), hist / hist_bar [num_bins][2], vs_bar [n][2].
- * Primal: the fold of a bin has the closed form P = sum p + ((sum s)^2 - sum s^2) / 2, S = sum s, so the
- * histogram is three float atomicAdd histograms and a finish pass. */
+ * Primal: the fold of a bin has the closed form P = sum p + ((sum s)^2 - sum s^2) / 2 = sum (p - s^2 / 2) + S^2 / 2,
+ * S = sum s, so the histogram is two float atomicAdd histograms and a finish pass. */
 size_t rbi_sumofprod_workspace_bytes(int64_t n, int64_t num_bins, int use_general);
 int rbi_sumofprod_forward(int64_t n, int64_t num_bins, const int64_t *is, const float *vs, float *hist,
                           void *ws, size_t ws_bytes, void *stream);
