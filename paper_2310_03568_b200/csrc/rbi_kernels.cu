@@ -342,7 +342,10 @@ rbi_minmax_lifted_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
 // (bin >> 15) << 16 | prefix; a slot that holds another bin does not filter.
 constexpr int MMF_NT = 1024;
 constexpr int MMF_REFRESH_AT = 3;  // iterations of a CTA before its filter is refreshed from the table (1: 0.094, 3: 0.088, 1+4: 0.091 ms)
-constexpr size_t MMF_SMEM = 128 * 1024;
+constexpr size_t MMF_FILTER = 128 * 1024;          // the filter
+constexpr int MMF_SEED = 4;                        // elements of a thread's first quad that take part (1: Zipf +4 us, uniform -2 us)
+constexpr int MMF_SIDE = 4096;                     // + a side table of 32-bit slots (first-batch election)
+constexpr size_t MMF_SMEM = MMF_FILTER + MMF_SIDE * 4;
 
 template <bool IS_MAX, bool TAGGED>
 __global__ void __launch_bounds__(MMF_NT, 1)
@@ -363,6 +366,27 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     }
     for (int i = threadIdx.x; i < (int)(MMF_SMEM / 16); i += MMF_NT) smem_raw[i] = make_uint4(~0u, ~0u, ~0u, ~0u);
     __syncthreads();
+    if (!TAGGED) {
+        // Hot bins.  With an open filter every warp's first element of a hot bin (Zipf keys: 14 % of the elements in
+        // one bin) queues at the bin's one L2 sector, for its read and for its atomic: two contended round trips in
+        // which 35 % of the Zipf case's stall samples sat (profiles/r2e).  The CTA's first batch therefore elects, per
+        // bin, its smallest 16-bit prefix in shared memory first (one 32-bit atomicMin on a direct-mapped side table of
+        // (prefix, bin tag) words; bins that share a slot: the smaller prefix keeps it, the other bin just goes
+        // unseeded) and seeds the filter with it: only the holders of that prefix go to L2 at all.
+        uint32_t *side = reinterpret_cast<uint32_t *>(smem_raw) + MMF_FILTER / 4;
+#pragma unroll
+        for (int j = 0; j < MMF_SEED; j++)
+            if (in_range(k[j], w))
+                atomicMin(side + (k[j] & (MMF_SIDE - 1)), ((ext_key<IS_MAX>(v[j]) >> 16) << 16) | (uint32_t)(k[j] >> 12));
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < MMF_SEED; j++) {
+            if (!in_range(k[j], w)) continue;
+            const uint32_t e = side[k[j] & (MMF_SIDE - 1)];
+            if ((e & 0xffffu) == (uint32_t)(k[j] >> 12)) f16[k[j]] = (uint16_t)(e >> 16);  // every writer stores the same value
+        }
+        __syncwarp();  // no CTA barrier: a warp that runs ahead of another one's seeds only meets an open filter
+    }
     // A CTA sees only n / (148 w) elements of a bin (1.7 at w = 2^16): on its own its filter learns a bound per bin
     // once and never profits from it.  After MMF_REFRESH_AT of its iterations (~1/9 of the input, ~28 elements per
     // bin seen by the grid as a whole) it therefore takes the bounds of ALL CTAs from the table, with coalesced
@@ -442,6 +466,9 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                 if ((int)(threadIdx.x & 31u) != __ffs(best) - 1) continue;
             }
             if ((vk >> 16) > f16[b]) continue;
+            // Publish the candidate's own prefix BEFORE the L2 round trip: it is the prefix of a value the bin holds, so a
+            // valid bound at once, and the other warps' elements of a hot bin stop here instead of queueing at one L2 sector.
+            f16[b] = (uint16_t)(vk >> 16);
             const unsigned long long key = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
             unsigned long long cur = __ldcg(tab + k[j]);
             if (key < cur) {
@@ -469,7 +496,10 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             for (int i = 0; i < 4; i++)
                 if (i != j && pass[j] && pass[i] && k[i] == k[j] && (key[i] < key[j])) pass[j] = false;
 #pragma unroll
-        for (int j = 0; j < 4; j++) cur[j] = pass[j] ? __ldcg(tab + k[j]) : 0ull;
+        for (int j = 0; j < 4; j++) {
+            if (pass[j]) f16[k[j]] = (uint16_t)(key[j] >> 48);  // the candidate's own prefix is a valid bound at once
+            cur[j] = pass[j] ? __ldcg(tab + k[j]) : 0ull;
+        }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
             if (pass[j] && key[j] < cur[j]) {
