@@ -394,8 +394,8 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
     // races with the per-element updates below, and from then on ~3 % of the elements reach L2 instead of ~60 %.
     const int64_t total_it = (n / 4 + stride - 1) / stride;
     int64_t it = 0;
-    // The loop is WARP-uniform (the first iteration uses warp-wide match / redux): a lane whose quads are used up goes
-    // on with an empty quad (keys -1: out of range, nothing loaded, nothing stored) until its warp is done.
+    // The loop is WARP-uniform: a lane whose quads are used up goes on with an empty quad (keys -1: out of range,
+    // nothing loaded, nothing stored) until its warp is done.
     while (__any_sync(FULL_MASK, q * 4 < n)) {
         if (!TAGGED && it == MMF_REFRESH_AT && total_it >= 2 * MMF_REFRESH_AT) {
             for (int b = threadIdx.x; b < (int)w; b += MMF_NT) {
@@ -448,27 +448,15 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
             }
         }
         } else if (it == 1) {
-        // The CTA's FIRST iteration, filter still open: with Zipf keys 14 % of the lanes hold the same bin and each would
-        // send its own atomic to the one L2 sector (40 % of the kernel's stall samples sat in this one iteration of 28,
-        // profiles/r2e).  The lanes of a warp that hold the same bin elect the smallest key (match.any + redux.min; equal
-        // values: the lowest lane = the lowest index); only that lane goes to L2, and its result sets the bin's filter.
+        // The CTA's first iteration: one element at a time (filter, table read, atomic with its result, filter update).
+        // The hot bins were seeded above; everything else meets a fresh table, and batching the quad here -- as the
+        // later iterations do -- measured 8 us slower at uniform keys.
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            const bool inr = in_range(k[j], w);
+            if (!in_range(k[j], w)) continue;
             const uint32_t vk = ext_key<IS_MAX>(v[j]);
-            const uint32_t b = inr ? (uint32_t)k[j] : (0x80000000u | (threadIdx.x & 31u));
-            const unsigned grp = __match_any_sync(FULL_MASK, b);
-            if (!inr) continue;
-            if ((grp & (grp - 1u)) != 0u) {  // my bin is held by more than one lane (a redux per distinct mask is slow:
-                                             // with 32 singleton groups it cost the uniform case 9 us)
-                const uint32_t vmin = __reduce_min_sync(grp, vk);
-                const unsigned best = __ballot_sync(grp, vk == vmin);
-                if ((int)(threadIdx.x & 31u) != __ffs(best) - 1) continue;
-            }
+            const uint32_t b = (uint32_t)k[j];
             if ((vk >> 16) > f16[b]) continue;
-            // Publish the candidate's own prefix BEFORE the L2 round trip: it is the prefix of a value the bin holds, so a
-            // valid bound at once, and the other warps' elements of a hot bin stop here instead of queueing at one L2 sector.
-            f16[b] = (uint16_t)(vk >> 16);
             const unsigned long long key = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
             unsigned long long cur = __ldcg(tab + k[j]);
             if (key < cur) {
