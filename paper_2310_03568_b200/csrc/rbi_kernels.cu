@@ -470,34 +470,40 @@ rbi_minmax_filtered_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         // atomics are not waited for one by one -- four dependent L2 round trips per quad were the kernel's whole
         // duration (28 iterations x 4 x ~1 us; 71 % of the stall samples on the two L2 waits, profiles/r2e).  A
         // thread's own duplicates of a bin are resolved in registers first (only the smallest key goes on).
-        unsigned long long key[4], cur[4];
+        unsigned long long cur[4];
+        uint32_t b[4], vk[4];
         bool pass[4];
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            const uint32_t vk = ext_key<IS_MAX>(v[j]);
-            key[j] = ((unsigned long long)vk << 32) | (unsigned)(q * 4 + j);
-            pass[j] = in_range(k[j], w) && !((vk >> 16) > f16[in_range(k[j], w) ? k[j] : 0]);
+            const bool inr = in_range(k[j], w);
+            b[j] = inr ? (uint32_t)k[j] : 0u;
+            vk[j] = ext_key<IS_MAX>(v[j]);
+            pass[j] = inr && !((vk[j] >> 16) > f16[b[j]]);
         }
 #pragma unroll
-        for (int j = 0; j < 4; j++)
+        for (int j = 1; j < 4; j++)
 #pragma unroll
-            for (int i = 0; i < 4; i++)
-                if (i != j && pass[j] && pass[i] && k[i] == k[j] && (key[i] < key[j])) pass[j] = false;
+            for (int i = 0; i < j; i++)
+                if (pass[i] && pass[j] && b[i] == b[j]) {  // i < j: on equal values the lower index stays
+                    if (vk[i] <= vk[j]) pass[j] = false;
+                    else pass[i] = false;
+                }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            if (pass[j]) f16[k[j]] = (uint16_t)(key[j] >> 48);  // the candidate's own prefix is a valid bound at once
-            cur[j] = pass[j] ? __ldcg(tab + k[j]) : 0ull;
+            if (pass[j]) f16[b[j]] = (uint16_t)(vk[j] >> 16);  // the candidate's own prefix is a valid bound at once
+            cur[j] = pass[j] ? __ldcg(tab + b[j]) : 0ull;
         }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
-            if (pass[j] && key[j] < cur[j]) {
-                atomicMin(tab + k[j], key[j]);  // result unused: a fire-and-forget RED, no third round trip
-                cur[j] = key[j];                // the table now holds key or less: a valid bound for the filter
+            const unsigned long long key = ((unsigned long long)vk[j] << 32) | (unsigned)(q * 4 + j);
+            if (pass[j] && key < cur[j]) {
+                atomicMin(tab + b[j], key);  // result unused: a fire-and-forget RED, no third round trip
+                cur[j] = key;                // the table now holds key or less: a valid bound for the filter
             }
         }
 #pragma unroll
         for (int j = 0; j < 4; j++)
-            if (pass[j]) f16[k[j]] = (uint16_t)(cur[j] >> 48);
+            if (pass[j]) f16[b[j]] = (uint16_t)(cur[j] >> 48);
         }
 #pragma unroll
         for (int j = 0; j < 4; j++) {
