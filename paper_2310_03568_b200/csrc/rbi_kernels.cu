@@ -944,6 +944,7 @@ VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint3
 constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
 constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
 constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9;
+constexpr int CB_PROBE = 4, CB_HOLD = 8;    // batches before the first decision / in full mode after a lean batch went bad
 
 // w > CS_SLOTS.  A CTA of 1024 threads owns a table of up to CB_PART bins in shared memory.  A
 // histogram wider than that is SPLIT over the 2^c CTAs of a group by the low c bits of the bin
@@ -965,6 +966,17 @@ constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9
 // Barriers: [claim] B1 [plain updates] B2 [CAS, caches].  Two elements never own one bin in a round
 // because all claims precede B1; the plain updates (between B1 and B2) never overlap a CAS (after
 // B2, before the next batch's B1).
+//
+// LEAN mode: the register entry and the cache look-up are a third of the instructions of a batch and absorb
+// nothing when no bin is hot (uniform keys).  The CTA therefore measures what they absorb: after CB_PROBE batches
+// with fewer than a quarter of the threads at >= 2 absorbed elements it skips steps 0 (and the register entry);
+// every lean batch counts its losers at B2 (free: the barrier carries the count), and a batch in which more than
+// 3/8 of the threads hold a loser -- uniform keys: 12 % -- puts the full machinery back for CB_HOLD batches.
+// Either mode is correct on any input (a cached or register-held partial product is just one more factor, folded
+// into the table at the end); the switch only moves instructions.
+template <bool B>
+struct BoolC { static constexpr bool value = B; };
+
 template <int ACC, bool COUNT_ZEROS, int U>
 __global__ void __launch_bounds__(CB_NT, 1)
 rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restrict__ is,
@@ -996,7 +1008,21 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     int64_t q0 = group * (int64_t)(CB_NT * U);  // CTA-uniform: no thread leaves the barriers early
     int64_t k[NI];
     float v[NI];
+    const int64_t nwhole = n >> 2;  // quads that exist in full
     auto load_batch = [&](int64_t q, int64_t (&kk)[NI], float (&vv)[NI]) {
+        if (q + CB_NT * U <= nwhole) {  // CTA-uniform: the whole batch exists, no per-thread guards
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int64_t qq = q + u * CB_NT + threadIdx.x;
+                const longlong2 *pk = reinterpret_cast<const longlong2 *>(is) + 2 * qq;
+                const longlong2 a = ldg_stream_ll2(pk), c = ldg_stream_ll2(pk + 1);
+                const uint4 x = ldg_stream(reinterpret_cast<const uint4 *>(vs) + qq);
+                kk[u * 4 + 0] = a.x; kk[u * 4 + 1] = a.y; kk[u * 4 + 2] = c.x; kk[u * 4 + 3] = c.y;
+                vv[u * 4 + 0] = __uint_as_float(x.x); vv[u * 4 + 1] = __uint_as_float(x.y);
+                vv[u * 4 + 2] = __uint_as_float(x.z); vv[u * 4 + 3] = __uint_as_float(x.w);
+            }
+            return;
+        }
 #pragma unroll
         for (int u = 0; u < U; u++) {
             int64_t k4[4] = {-1, -1, -1, -1};
@@ -1022,6 +1048,7 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     // at 0 -- the displaced pair takes the element's place on the normal path.
     uint32_t rb = CB_EMPTY, rcnt = 0;
     float racc = OP::neutral();
+    int until = CB_PROBE;       // CTA-uniform: > 0 full-mode batches until the next decision, < 0 lean mode
     load_batch(q0, k, v);
     for (;;) {
         // after the last batch of the input: one more round of the same machinery for the register
@@ -1054,7 +1081,13 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
             v[0] = racc;
             rcnt = 1;  // keeps the loop below from re-installing it
             rb = CB_EMPTY;
+            until = 1 << 30;  // full mode: 1024 partial products of one hot bin go through the caches, not through 1024 CAS
         }
+        // one straight-line body per mode (a run-time flag inside one body cost both modes 7-11 %: the branches end
+        // the basic blocks the loads are scheduled across)
+        auto body = [&](auto LEAN_T) {
+        constexpr bool lean = decltype(LEAN_T)::value;
+        if constexpr (!lean) {
 #pragma unroll
         for (int j = 0; j < NI; j++) {  // register entry
             if (b[j] == CB_EMPTY) continue;
@@ -1073,22 +1106,40 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 rcnt--;
             }
         }
-        uint32_t t[NI];
-#pragma unroll
-        for (int j = 0; j < NI; j++) t[j] = tg[b[j] & (CB_SLOTS - 1)];
+        }
         uint32_t coldm = 0;  // bit j: pending and not resident in the warp's cache
         uint32_t hotm = 0;   // bit j: pending and resident
+        if constexpr (!lean) {
+            uint32_t t[NI];
 #pragma unroll
-        for (int j = 0; j < NI; j++) {
-            // a valid tag never equals CB_EMPTY's, and b == CB_EMPTY matches no tag
-            const bool hot = (t[j] >> 2) == b[j] / CB_SLOTS;
-            const bool cold = !hot & (b[j] != CB_EMPTY);
-            hotm |= (uint32_t)hot << j;
-            coldm |= (uint32_t)cold << j;
-            if (hot & ((t[j] & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t[j] + 1;  // racing lanes store the same word
-            if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
+            for (int j = 0; j < NI; j++) t[j] = tg[b[j] & (CB_SLOTS - 1)];
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                // a valid tag never equals CB_EMPTY's, and b == CB_EMPTY matches no tag
+                const bool hot = (t[j] >> 2) == b[j] / CB_SLOTS;
+                const bool cold = !hot & (b[j] != CB_EMPTY);
+                hotm |= (uint32_t)hot << j;
+                coldm |= (uint32_t)cold << j;
+                if (hot & ((t[j] & 3u) != 3u)) tg[b[j] & (CB_SLOTS - 1)] = t[j] + 1;  // racing lanes store the same word
+                if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < NI; j++) {
+                const bool cold = b[j] != CB_EMPTY;
+                coldm |= (uint32_t)cold << j;
+                if (cold) claimA[b[j]] = (uint16_t)(id0 + j);
+            }
         }
-        __syncthreads();  // B1
+        bool plain_b1 = true;
+        if constexpr (!lean) {
+            if (--until == 0) {  // B1, carrying the decision: threads with a cache hit now or a register hit lately
+                const int busy = __syncthreads_count(hotm != 0 || rcnt > 1);
+                until = busy < CB_NT / 4 ? -1 : CB_PROBE;
+                plain_b1 = false;
+            }
+        }
+        if (plain_b1) __syncthreads();  // B1
         {
             uint16_t c[NI];
             float o[NI];
@@ -1105,7 +1156,12 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 coldm &= ~((uint32_t)win << j);
             }
         }
-        __syncthreads();  // B2: the plain updates are done before any CAS touches the table
+        // B2: the plain updates are done before any CAS touches the table
+        if constexpr (lean) {
+            if (__syncthreads_count(coldm != 0) > CB_NT * 3 / 8) until = CB_HOLD;  // this batch's losers still take the path below
+        } else {
+            __syncthreads();
+        }
         if (__any_sync(FULL_MASK, coldm != 0)) {
 #pragma unroll
             for (int j = 0; j < NI; j++) {  // losers: ONE compare-and-swap; a failure means the bin is contended
@@ -1117,7 +1173,7 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 }
             }
         }
-        if (__any_sync(FULL_MASK, hotm != 0)) {
+        if (!lean && __any_sync(FULL_MASK, hotm != 0)) {
 #pragma unroll
             for (int j = 0; j < NI; j++) {  // hits: the resident entry cannot change before the installs below
                 uint8_t *c = cl + (b[j] & (CB_SLOTS - 1));
@@ -1146,6 +1202,8 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
                 }
             }
         }
+        };
+        if (until < 0) body(BoolC<true>{}); else body(BoolC<false>{});
         if (drain) break;
 #pragma unroll
         for (int j = 0; j < NI; j++) {

@@ -422,3 +422,42 @@ def test_rbi_host_entry_points_match_the_device_path(opname):
     out = torch.empty(n, dtype=torch.float32).pin_memory()
     B.vjp_reduce_by_index_host(op, w, hi, hv, hh, out, scratch)
     assert same(out.numpy(), want[0])
+
+
+@pytest.mark.parametrize("phases", ["uniform-hot-uniform", "hot-uniform-hot", "hot-bin-per-stripe"])
+@pytest.mark.parametrize("w", [40000, 1 << 16])
+def test_rbi_mul_wide_histogram_key_skew_changes_along_the_input(w, phases):
+    """'*' at w > 12 288 (rbi_cached_big_kernel) switches per CTA between its full machinery (register entry + warp
+    caches) and a lean claim-round-only mode on what the hot paths absorb and on how many claim rounds are lost.  Keys
+    whose skew changes along the input drive every CTA through both switches; the product per bin, the zero counts and
+    the VJP (Fig. 3) must not depend on it."""
+    n = 1 << 23                                   # 28 batches per CTA: several decisions in each phase
+    rng = np.random.default_rng([w, len(phases)])
+    uni = rng.integers(-1, w + 1, size=n, dtype=np.int64)
+    hot = np.where(rng.random(n) < 0.6, rng.integers(0, 4, n) * 2 + (np.arange(n) & 1), uni).astype(np.int64)
+    third = np.arange(n) * 3 // n
+    if phases == "uniform-hot-uniform":
+        is_ = np.where(third == 1, hot, uni)
+    elif phases == "hot-uniform-hot":
+        is_ = np.where(third == 1, uni, hot)
+    else:                                         # stripes of 2^16 elements, each with its own single hot bin
+        is_ = np.where(rng.random(n) < 0.5, (np.arange(n) >> 16) * 37 % w, uni).astype(np.int64)
+    vs = rng.uniform(0.995, 1.005, n).astype(np.float32)
+    vs[rng.random(n) < 1e-5] = 0.0
+    hb = rng.standard_normal(w).astype(np.float32)
+    op = B.Op.of("mul")
+    got = B.vjp_reduce_by_index(op, w, dev(is_), dev(vs), dev(hb)).cpu().numpy()
+    ref, rz, rp = oracle.vjp_rbi_mul(w, is_, vs, hb)
+    z, p = B.rbi_zero_prod(op, w, dev(is_), dev(vs))
+    assert np.array_equal(z.cpu().numpy(), rz)
+    p = p.cpu().numpy().astype(np.float64)
+    ok = (np.abs(rp) > 1e-30) & (np.abs(rp) < 1e30)
+    assert ok.sum() > w // 2
+    assert np.max(np.abs(p[ok] - rp[ok]) / np.abs(rp[ok]), initial=0.0) <= 1e-4
+    assert nrel(got, ref) <= 1e-4
+    # the same keys through satadd's primal (the other operator of the kernel): bit-exact against the oracle when
+    # every value is a multiple of 2^-10 and S is never reached (exact f32 sums in any order)
+    q = (rng.integers(0, 8, n) * 2.0 ** -10).astype(np.float32)
+    sat = B.Op.of("satadd", S=float(1 << 20))
+    h = B.reduce_by_index_forward(sat, w, dev(is_), dev(q)).cpu().numpy()
+    assert np.array_equal(h.astype(np.float64), oracle.reduce_by_index_forward("satadd", w, is_, q, S=float(1 << 20)))
