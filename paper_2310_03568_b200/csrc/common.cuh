@@ -30,6 +30,43 @@ VJP_DEVINL void stg_stream(uint4 *p, const uint4 &v) {
                  : "memory");
 }
 
+// L2 eviction hints for the lifted primal of '*' and the return sweep over the same (is, vs) that follows it.  The primal's
+// 128-bit streaming loads carry an explicit evict_normal policy -- plain ld.global.nc.L1::no_allocate lines do not stay in
+// L2 long enough for the sweep to meet them -- and the sweep reads and writes evict_first.  '*' VJP at w = 2^10 with L2
+// flushed between calls (fresh inputs): 0.120 -> 0.112 ms uniform, 0.130 -> 0.118 ms Zipf; back to back 0.115 -> 0.113,
+// 0.123 -> 0.119 ms (the sweep 44.9 -> 35.3 us, the primal + 4 us: it no longer meets lines the previous call's sweep
+// left).  An evict_last fraction (0.4, 0.55) on the primal added nothing.  NOT used in the scan kernels: the same hint on
+// every streaming load cost the scan primals 3-8 % (5x5: 0.327 -> 0.409 ms; written lines compete with the kept ones), on
+// the forward pass of a scan VJP alone it moved the VJP by +-2 %, evict_first in the reverse scan kernel cost 1-5 %; in the
+// sumOfProd kernels the effect was inside the run-to-run spread (+-5 % between processes).
+VJP_DEVINL uint64_t l2_policy_stream() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+VJP_DEVINL uint64_t l2_policy_normal() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+VJP_DEVINL longlong2 ldg_hint_ll2(const longlong2 *p, uint64_t pol) {
+    longlong2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.s64 {%0,%1}, [%2], %3;" : "=l"(r.x), "=l"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+VJP_DEVINL uint4 ldg_hint(const uint4 *p, uint64_t pol) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+                 : "l"(p), "l"(pol));
+    return r;
+}
+VJP_DEVINL void stg_hint(uint4 *p, const uint4 &v, uint64_t pol) {
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.u32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y),
+                 "r"(v.z), "r"(v.w), "l"(pol)
+                 : "memory");
+}
+
 // ------------------------------------------------------------------ POD word helpers ---
 
 // Copy a POD state to / from global memory through L2 (look-back payloads: written once by one

@@ -851,12 +851,13 @@ rbi_cached_small_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         longlong2 a, b;
         uint4 v;
     };
+    const uint64_t keep = l2_policy_normal();
     auto fetch = [&](uint32_t q, Quad &x) {  // warp-uniform q; only whole batches are fetched here
         if (q + 32 <= nfull) {
             const longlong2 *kp = reinterpret_cast<const longlong2 *>(is) + 2 * (size_t)(q + lane);
-            x.a = ldg_stream_ll2(kp);
-            x.b = ldg_stream_ll2(kp + 1);
-            x.v = ldg_stream(reinterpret_cast<const uint4 *>(vs) + (q + lane));
+            x.a = ldg_hint_ll2(kp, keep);
+            x.b = ldg_hint_ll2(kp + 1, keep);
+            x.v = ldg_hint(reinterpret_cast<const uint4 *>(vs) + (q + lane), keep);
         }
     };
     auto run = [&](const Quad &x) {
@@ -941,6 +942,10 @@ VJP_DEVINL bool claim_update_big(bool act, uint32_t b, float x, float *vl, uint3
     return ev;
 }
 
+// The next batch is prefetched into registers (true) or, by cp.async.bulk.prefetch, into L2 and loaded at the top of its own
+// iteration (false: 12 registers fewer, so U = 2 fits without spills).  Lifted '*' at w = 2^16, uniform / Zipf keys:
+// registers U = 1 0.125 / 0.222 ms; L2 U = 1 0.125 / 0.236; L2 U = 2 (half the barriers) 0.129 / 0.237.
+constexpr bool CB_REGPF = true;
 constexpr int CB_U = 1;               // quads per thread per batch (2 spills at 64 registers: 0.17 -> 0.24 ms)
 constexpr uint32_t CB_RW = 8, CB_RMAX = 63;  // register entry: kept by a bin with more than 1/(1+CB_RW) of the elements
 constexpr size_t CB_SMEM = (size_t)CB_PART * 6 + (size_t)CB_WARPS * CB_SLOTS * 9;
@@ -1009,14 +1014,15 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
     int64_t k[NI];
     float v[NI];
     const int64_t nwhole = n >> 2;  // quads that exist in full
+    const uint64_t keep = l2_policy_normal();
     auto load_batch = [&](int64_t q, int64_t (&kk)[NI], float (&vv)[NI]) {
         if (q + CB_NT * U <= nwhole) {  // CTA-uniform: the whole batch exists, no per-thread guards
 #pragma unroll
             for (int u = 0; u < U; u++) {
                 const int64_t qq = q + u * CB_NT + threadIdx.x;
                 const longlong2 *pk = reinterpret_cast<const longlong2 *>(is) + 2 * qq;
-                const longlong2 a = ldg_stream_ll2(pk), c = ldg_stream_ll2(pk + 1);
-                const uint4 x = ldg_stream(reinterpret_cast<const uint4 *>(vs) + qq);
+                const longlong2 a = ldg_hint_ll2(pk, keep), c = ldg_hint_ll2(pk + 1, keep);
+                const uint4 x = ldg_hint(reinterpret_cast<const uint4 *>(vs) + qq, keep);
                 kk[u * 4 + 0] = a.x; kk[u * 4 + 1] = a.y; kk[u * 4 + 2] = c.x; kk[u * 4 + 3] = c.y;
                 vv[u * 4 + 0] = __uint_as_float(x.x); vv[u * 4 + 1] = __uint_as_float(x.y);
                 vv[u * 4 + 2] = __uint_as_float(x.z); vv[u * 4 + 3] = __uint_as_float(x.w);
@@ -1054,10 +1060,15 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
         // after the last batch of the input: one more round of the same machinery for the register
         // entries (1024 CAS on one hot cell would serialise); q0 is CTA-uniform
         const bool drain = q0 >= nquads;
-        int64_t kn[NI];
-        float vn[NI];
+        int64_t kn[CB_REGPF ? NI : 1];
+        float vn[CB_REGPF ? NI : 1];
         const int64_t qn = q0 + stride;
-        load_batch(qn, kn, vn);  // next batch's loads fly while this one is processed (none past the end)
+        if constexpr (CB_REGPF) {
+            load_batch(qn, kn, vn);  // next batch's loads fly while this one is processed (none past the end)
+        } else if (qn + CB_NT * U <= nwhole) {  // next batch on its way into L2: no registers held across the body
+            prefetch_tile_l2<CB_WARPS>(is + 4 * qn, (int64_t)CB_NT * U * 32);
+            prefetch_tile_l2<CB_WARPS>(vs + 4 * qn, (int64_t)CB_NT * U * 16);
+        }
         uint32_t b[NI];  // table index of a pending element, CB_EMPTY = nothing pending
         uint32_t zm = 0;
 #pragma unroll
@@ -1205,10 +1216,14 @@ rbi_cached_big_kernel(int64_t n, int64_t w, int cl_log2, const int64_t *__restri
         };
         if (until < 0) body(BoolC<true>{}); else body(BoolC<false>{});
         if (drain) break;
+        if constexpr (CB_REGPF) {
 #pragma unroll
-        for (int j = 0; j < NI; j++) {
-            k[j] = kn[j];
-            v[j] = vn[j];
+            for (int j = 0; j < NI; j++) {
+                k[j] = kn[j];
+                v[j] = vn[j];
+            }
+        } else {
+            load_batch(qn, k, v);
         }
         q0 = qn;
     }
@@ -1377,6 +1392,7 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
         __syncthreads();
     }
     const int64_t stride = (int64_t)gridDim.x * RBI_NT;
+    const uint64_t strm = l2_policy_stream();
     for (int64_t q = blockIdx.x * (int64_t)RBI_NT + threadIdx.x; q * 4 < n; q += stride) {
         int64_t k[4];
         float v[4], o[4];
@@ -1389,10 +1405,20 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                 const int64_t kr = j < cnt ? __ldg(is + (idx >> ld)) : (int64_t)-1;
                 k[j] = in_range(kr, w >> ld) ? (kr << ld) | (idx & (((int64_t)1 << ld) - 1)) : (int64_t)-1;
             }
+        } else if (q * 4 + 4 <= n) {
+            const longlong2 *pk = reinterpret_cast<const longlong2 *>(is) + 2 * q;
+            const longlong2 a = ldg_hint_ll2(pk, strm), b = ldg_hint_ll2(pk + 1, strm);
+            k[0] = a.x; k[1] = a.y; k[2] = b.x; k[3] = b.y;
+            cnt = 4;
         } else {
             cnt = load_keys4(is, q * 4, n, k);
         }
-        load_vals4(vs, q * 4, cnt, v);
+        if (!VEC && cnt == 4) {
+            const uint4 x = ldg_hint(reinterpret_cast<const uint4 *>(vs) + q, strm);
+            v[0] = __uint_as_float(x.x); v[1] = __uint_as_float(x.y); v[2] = __uint_as_float(x.z); v[3] = __uint_as_float(x.w);
+        } else {
+            load_vals4(vs, q * 4, cnt, v);
+        }
         // the four coefficient gathers are issued together (clamped index, unconditional load): one L2 round
         // trip per quad instead of four dependent ones (profiles/r2c: 32 long-scoreboard stall cycles per issue)
         if constexpr (SMEM) {
@@ -1427,7 +1453,11 @@ rbi_mul_sweep_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                 o[j] = in_range(k[j], w) ? r : 0.f;
             }
         }
-        store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
+        if (!VEC && cnt == 4 && accumulate == 0)
+            stg_hint(reinterpret_cast<uint4 *>(vs_bar) + q,
+                     make_uint4(__float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]), __float_as_uint(o[3])), strm);
+        else
+            store_adj4(vs_bar, q * 4, cnt, o, accumulate != 0);
     }
 }
 
