@@ -72,6 +72,39 @@ def event_time_ms(fn, reps: int, warmup: int = 3, inner: int = 4):
     return out
 
 
+def graph_time_ms(fn, reps: int, inner: int = 8):
+    """Per-call device times (ms) of fn() replayed from a CUDA graph: `inner` calls are captured once (the library
+    only enqueues on the given stream and never allocates or synchronises, so its calls can be captured) and every
+    sample replays the graph between two CUDA events -- no host work per call, so a 5 us kernel is timed as such.
+    Returns None if the capture fails (the eager timing of event_time_ms then stands alone)."""
+    side = torch.cuda.Stream()
+    try:
+        g = torch.cuda.CUDAGraph()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            fn()  # first call on this stream outside the capture (lazy function attributes, static set-up)
+            side.synchronize()
+            with torch.cuda.graph(g, stream=side, capture_error_mode="thread_local"):
+                for _ in range(inner):
+                    fn()
+        torch.cuda.synchronize()
+        for _ in range(3):
+            g.replay()
+        torch.cuda.synchronize()
+        out = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            g.replay()
+            b.record()
+            b.synchronize()
+            out.append(a.elapsed_time(b) / inner)
+        return out
+    except Exception:  # noqa: BLE001 -- a capture that fails must not take the bench down
+        torch.cuda.synchronize()
+        return None
+
+
 class ClockSampler:
     """Samples SM clocks and throttle reasons while a timed region runs: NVML in a thread (a few ms
     per sample: the timed region of the default run is well under a second), nvidia-smi as fallback."""
@@ -301,13 +334,20 @@ class ReduceCase:
         return B.reduce_forward(self.op, self.xs, ws=self.ws)
 
 
-def measure_case(key, label, case, reps, peak_gbs):
+def measure_case(key, label, case, reps, peak_gbs, graph=True):
     """VJP and primal timings of one case (median over reps, CUDA events)."""
     tv = statistics.median(event_time_ms(case.vjp, reps))
     tp = statistics.median(event_time_ms(case.primal, reps))
     n = case.n
     vb, pb = VJP_BYTES_PER_ELEM[key] * n, PRIMAL_BYTES_PER_ELEM[key] * n
     gbs = vb / (tv * 1e-3) / 1e9
+    extra = {}
+    if graph:  # the same calls replayed from a CUDA graph: what a C caller in a tight loop sees (no Python per call)
+        gv, gp = graph_time_ms(case.vjp, reps), graph_time_ms(case.primal, reps)
+        if gv is not None and gp is not None:
+            gv, gp = statistics.median(gv), statistics.median(gp)
+            extra = {"vjp_ms_graph": round(gv, 4), "primal_ms_graph": round(gp, 4),
+                     "frac_graph": round(vb / (gv * 1e-3) / 1e9 / peak_gbs, 3)}
     return {
         "case": label, "n": n, "vjp_ms": round(tv, 4), "primal_ms": round(tp, 4),
         "vjp_gelem_s": round(n / (tv * 1e-3) / 1e9, 3),
@@ -316,6 +356,7 @@ def measure_case(key, label, case, reps, peak_gbs):
         "vjp_alg_gbs": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak_gbs, 3),
         "frac_of_8tbs": round(gbs / NORTH_STAR_PEAK_GBS, 3),
         "primal_alg_gbs": round(pb / (tp * 1e-3) / 1e9, 1),
+        **extra,
     }
 
 
