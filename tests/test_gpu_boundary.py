@@ -299,3 +299,46 @@ def test_no_write_outside_outputs_and_workspaces(n):
         B.vjp_reduce(op, xs, yb1, out=out, ws=ws)
     for c in checks:
         c()
+
+
+# ------------------------------------------------------------------ CUDA graph capture ------------
+
+def test_calls_can_be_captured_in_a_cuda_graph_and_replayed():
+    """The library only enqueues on the caller's stream (no allocation, no synchronisation: include/vjp_b200.h), so a
+    sequence of calls can be captured into a CUDA graph -- bench.py times its step that way.  Every replay must give
+    the oracle's result again (outputs are poisoned in between; workspaces are re-initialised by the calls)."""
+    n, w = 100003, 20000
+    dm, dx = W.c2_rbi_min(n=n, w=w, dist="zipf"), W.c2_rbi_mul(n=n, w=w, dist="uniform", zero_rate=1e-3)
+    ds = W.c3_scan_linrec(n=n)
+    op_min, op_mul, op_lin = B.Op.of("min"), B.Op.of("mul"), B.Op.of("linrec")
+    g_min = [dev(dm["is_"]), dev(dm["vs"]), dev(dm["hist_bar"])]
+    g_mul = [dev(dx["is_"]), dev(dx["vs"]), dev(dx["hist_bar"])]
+    xs, yb = dev(ds["xs"]), dev(ds["ys_bar"])
+    o_min, o_mul, o_lin = torch.empty(n, device="cuda"), torch.empty(n, device="cuda"), torch.empty_like(yb)
+    ws_rbi = torch.empty(max(B.vjp_reduce_by_index_workspace_bytes(op_min, n, w),
+                             B.vjp_reduce_by_index_workspace_bytes(op_mul, n, w)), dtype=torch.uint8, device="cuda")
+    ws_scan = torch.empty(B.vjp_scan_workspace_bytes(op_lin, n), dtype=torch.uint8, device="cuda")
+
+    def calls():
+        B.vjp_reduce_by_index(op_min, w, *g_min, out=o_min, ws=ws_rbi)
+        B.vjp_reduce_by_index(op_mul, w, *g_mul, out=o_mul, ws=ws_rbi)
+        B.vjp_scan(op_lin, xs, yb, out=o_lin, ws=ws_scan)
+
+    calls()  # first call outside the capture (function attributes are set lazily)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side, capture_error_mode="thread_local"):
+        calls()
+    ref_min = oracle.vjp_rbi_minmax("min", w, dm["is_"], dm["vs"], dm["hist_bar"])[0]
+    ref_mul = oracle.vjp_rbi_mul(w, dx["is_"], dx["vs"], dx["hist_bar"])[0]
+    ref_lin = oracle.vjp_scan("linrec", ds["xs"], ds["ys_bar"])
+    for _ in range(3):
+        for o in (o_min, o_mul, o_lin):
+            o.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(o_min.cpu().numpy().astype(np.float64), np.asarray(ref_min, dtype=np.float64))  # a copy: bit-identical
+        assert nrel(o_mul.cpu().numpy(), ref_mul) <= 1e-4
+        assert nrel(o_lin.cpu().numpy(), ref_lin) <= 1e-4
