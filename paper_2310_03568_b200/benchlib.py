@@ -41,6 +41,7 @@ def kernel_bytes_per_elem(name: str, elem_bytes: int = 4) -> float:
         "rbi_forward_kernel": 8 + elem_bytes,
         "scan_lookback_kernel<MODE_SCAN>": 2 * elem_bytes,
         "scan_lookback_kernel<MODE_TILEAGG>": elem_bytes,
+        "tile_agg_tma_kernel": elem_bytes,
         "scan_vjp_reverse_kernel": 3 * elem_bytes,
         "sort_hist_kernel": 8,                       # first pass reads int64 keys (4 on later passes)
         "sort_scatter_kernel": 24,                   # read 12, write 12

@@ -63,7 +63,7 @@ const char *const KERNEL_NAMES[K_COUNT] = {
     "seg_reverse_vjp_kernel", "sort_export_kernel",
     "reduce_partial_kernel", "reduce_finish_kernel", "reduce_sweep_kernel", "reduce_pack_kernel",
     "sop_forward_kernel", "sop_finish_kernel", "sop_inv_sweep_kernel", "rows_to_cols / cols_to_rows",
-    "ms_forward_kernel", "ms_seg_agg / ms_carry_kernel", "ms_backward_kernel", "ms_hist_kernel", "shift_words_kernel"};
+    "ms_forward_kernel", "ms_seg_agg / ms_carry_kernel", "ms_backward_kernel", "ms_hist_kernel", "shift_words_kernel", "tile_agg_tma_kernel"};
 constexpr int PROF_MAX = 8192;
 struct ProfRec { int kid; cudaEvent_t a, b; };
 long long g_launches[K_COUNT];

@@ -30,7 +30,7 @@ enum KernelId : int {
     K_SORT_HIST, K_U32_SCAN, K_SORT_SCATTER, K_SEG_FORWARD, K_SEG_REVERSE, K_SORT_EXPORT,
     K_REDUCE_PARTIAL, K_REDUCE_FINISH, K_REDUCE_SWEEP, K_REDUCE_PACK,
     K_SOP_FORWARD, K_SOP_FINISH, K_SOP_SWEEP, K_VEC_TRANSPOSE,
-    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD, K_MS_HIST, K_SHIFT_WORDS,
+    K_MS_FORWARD, K_MS_CARRY, K_MS_BACKWARD, K_MS_HIST, K_SHIFT_WORDS, K_SCAN_TILEAGG_TMA,
     K_COUNT
 };
 void prof_begin(int kid, cudaStream_t s);
