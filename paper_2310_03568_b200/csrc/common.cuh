@@ -135,12 +135,13 @@ struct BlockScan {
 
     // Exclusive scan of one state per thread.  Returns the exclusive prefix of this thread
     // (within the block) and the block total in `total` (valid in every thread).
-    template <bool REVT>
+    // ENTRY_SYNC = false: the caller knows that nobody can still be reading `scratch` (the first scan of a CTA)
+    template <bool REVT, bool ENTRY_SYNC = true>
     static VJP_DEVINL S exclusive(const S &local, S &total, uint32_t *scratch) {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         const int plane = REVT ? 31 - lane : lane;
         const int pwarp = REVT ? NW - 1 - warp : warp;
-        __syncthreads();  // scratch may still be read by a previous call
+        if (ENTRY_SYNC) __syncthreads();  // scratch may still be read by a previous call
         S incl = local;
         // wide states (25- and 50-word 5x5 states): keep the loop rolled -- fully unrolled, the 5x5
         // VJP kernel was 11 400 instructions (182 KB), more than the instruction cache holds, and
@@ -177,6 +178,68 @@ struct BlockScan {
             ex = M::combine(wp, ex);
         }
         return ex;
+    }
+};
+
+// Two independent exclusive scans of one block in ONE pass: scan A runs from the END of the tile (thread t has
+// processing rank NT-1-t, as BlockScan with REVT), scan B from its start.  They share every barrier -- three instead
+// of six per tile -- and the two cross-warp scans run side by side in warps 0 and 1.  The reverse kernel of the scan
+// VJP needs exactly this pair (the reverse lin_o scan and the forward prefixes); ncu showed its warps mostly waiting
+// at barriers (2x2: 6.6 of 16 stall cycles per issue).
+template <class MA, class MB, int NT>
+struct BlockScanDual {
+    using SA = typename MA::State;
+    using SB = typename MB::State;
+    static constexpr int NW = NT / 32, WA = sizeof(SA) / 4, WB = sizeof(SB) / 4;
+    static constexpr int SMEM_WORDS = (NW + 1) * (WA + WB);
+    static_assert(NW >= 2, "two warps run the cross-warp scans");
+
+    template <class M, class S>
+    static VJP_DEVINL void cross_warp(uint32_t *tot, int lane) {  // tot[w] = total of processing-warp w -> its exclusive prefix
+        constexpr int SW = sizeof(S) / 4;
+        S wt = (lane < NW) ? load_state_smem<S>(tot + lane * SW) : M::identity();
+        S wi = wt;
+#pragma unroll
+        for (int off = 1; off < NW; off <<= 1) {
+            S o = shfl_state(wi, lane - off);
+            if (lane >= off) wi = M::combine(o, wi);
+        }
+        S wex = shfl_state(wi, lane - 1);
+        if (lane == 0) wex = M::identity();
+        __syncwarp();
+        if (lane < NW) store_state_smem(tot + lane * SW, wex);
+        if (lane == NW - 1) store_state_smem(tot + NW * SW, wi);
+    }
+
+    template <bool ENTRY_SYNC = true>
+    static VJP_DEVINL void exclusive(const SA &la, SA &ta, SA &exa, const SB &lb, SB &tb, SB &exb, uint32_t *scratch) {
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const int pwa = NW - 1 - warp;  // processing rank of this warp in scan A
+        uint32_t *sa = scratch, *sb = scratch + (NW + 1) * WA;
+        if (ENTRY_SYNC) __syncthreads();  // scratch may still be read by a previous call
+        SA ia = la;
+        SB ib = lb;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const SA oa = shfl_state(ia, lane + off);
+            if (31 - lane >= off) ia = MA::combine(oa, ia);
+            const SB ob = shfl_state(ib, lane - off);
+            if (lane >= off) ib = MB::combine(ob, ib);
+        }
+        exa = shfl_state(ia, lane + 1);
+        if (lane == 31) exa = MA::identity();
+        exb = shfl_state(ib, lane - 1);
+        if (lane == 0) exb = MB::identity();
+        if (lane == 0) store_state_smem(sa + pwa * WA, ia);
+        if (lane == 31) store_state_smem(sb + warp * WB, ib);
+        __syncthreads();
+        if (warp == 0) cross_warp<MA, SA>(sa, lane);
+        if (warp == 1) cross_warp<MB, SB>(sb, lane);
+        __syncthreads();
+        ta = load_state_smem<SA>(sa + NW * WA);
+        tb = load_state_smem<SB>(sb + NW * WB);
+        if (pwa > 0) exa = MA::combine(load_state_smem<SA>(sa + pwa * WA), exa);
+        if (warp > 0) exb = MB::combine(load_state_smem<SB>(sb + warp * WB), exb);
     }
 };
 

@@ -130,7 +130,7 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
         for (int j = IPT - 2; j >= 0; j--) acc = Op::combine(Op::from_elem(r + j * EW), acc);
     }
     S total;
-    S ex = BS::template exclusive<REV>(acc, total, scratch);
+    S ex = BS::template exclusive<REV, false>(acc, total, scratch);  // the CTA's only scan
     if (MODE == MODE_TILEAGG) {  // aggregate only: no dependency on other tiles, pure streaming
         if (threadIdx.x == 0) store_state_cg(fpre + t, total);
         return;
@@ -371,7 +371,7 @@ tile_agg_tma_kernel(const __grid_constant__ CUtensorMap tm, const uint32_t *__re
 //     rbar_i = ybar_i + u_{i+1},   xbar_i = (d(r_{i-1} (.) x_i)/dx_i)^T rbar_i,   u_n = 0,
 // and element i acts on the incoming u as the affine map z -> (ybar_i + z) * X_i^T.
 template <class Op, int NT, int IPT>
-__global__ void __launch_bounds__(NT, (Op::EW <= 4 ? 1024 / NT : 1))
+__global__ void __launch_bounds__(NT, (Op::EW <= 4 ? (NT <= 256 ? 3 : 1024 / NT) : 1))  // 256 threads: 3 CTAs fit the shared memory
 scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
                         uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
                         const typename Op::Fwd *__restrict__ fpre,
@@ -385,7 +385,9 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     using St = Stage<NT, RW>;
     using RBS = BlockScan<RM, NT>;
     using FBS = BlockScan<FM, NT>;
-    constexpr int SCR = RBS::SMEM_WORDS > FBS::SMEM_WORDS ? RBS::SMEM_WORDS : FBS::SMEM_WORDS;
+    using DBS = BlockScanDual<RM, FM, NT>;
+    constexpr bool DUAL = sizeof(RS) + sizeof(FS) <= 96;  // narrow states: both block scans in one pass (half the barriers)
+    constexpr int SCR = DBS::SMEM_WORDS;                  // >= either single scan's scratch
     extern __shared__ uint4 smem[];
     uint4 *sx = smem;
     uint4 *sy = smem + St::SMEM_BYTES / 16;
@@ -429,7 +431,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
 #pragma unroll
         for (int j = 0; j < IPT; j++) facc = Op::combine(facc, Op::from_elem(rx + j * EW));
         FS ftotal;
-        const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+        const FS fex = FBS::template exclusive<false, false>(facc, ftotal, scratch);
         FS rp[IPT];
         rp[0] = Op::combine(load_state_cg(fpre + t), fex);
 #pragma unroll
@@ -474,10 +476,14 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     RS racc;
     racc.b = bacc;
     racc.l = Op::lin_of(facc);  // forward product of the thread's range: the c of lin_o, transposed
-    RS rtotal;
-    const RS rex = RBS::template exclusive<true>(racc, rtotal, scratch);
-    FS ftotal;
-    const FS fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+    RS rtotal, rex;
+    FS ftotal, fex;
+    if constexpr (DUAL) {
+        DBS::template exclusive<false>(racc, rtotal, rex, facc, ftotal, fex, scratch);  // the CTA's first use of scratch
+    } else {
+        rex = RBS::template exclusive<true, false>(racc, rtotal, scratch);
+        fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+    }
 
     // The forward prefixes r_{i-1} of the thread's elements depend only on fpre[t] and fex, not on the reverse
     // look-back: they are computed BEFORE the barrier that waits for warp 0, so that warps 1 .. N-1 work (and
@@ -550,9 +556,7 @@ static size_t scan_smem_bytes() {
 template <class Op, int NT, int IPT>
 static size_t vjp_smem_bytes() {
     using St = Stage<NT, IPT * Op::EW>;
-    using RBS = BlockScan<RevMonoid<Op>, NT>;
-    using FBS = BlockScan<FwdMonoid<Op>, NT>;
-    constexpr int SCR = RBS::SMEM_WORDS > FBS::SMEM_WORDS ? RBS::SMEM_WORDS : FBS::SMEM_WORDS;
+    constexpr int SCR = BlockScanDual<RevMonoid<Op>, FwdMonoid<Op>, NT>::SMEM_WORDS;
     return 2 * St::SMEM_BYTES + (SCR + sizeof(typename RevMonoid<Op>::State) / 4) * 4;
 }
 
