@@ -386,7 +386,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     using RBS = BlockScan<RM, NT>;
     using FBS = BlockScan<FM, NT>;
     using DBS = BlockScanDual<RM, FM, NT>;
-    constexpr bool DUAL = sizeof(RS) + sizeof(FS) <= 96;  // narrow states: both block scans in one pass (half the barriers)
+    constexpr bool DUAL = sizeof(RS) + sizeof(FS) <= 192;  // narrow states: both block scans in one pass (half the barriers)
     constexpr int SCR = DBS::SMEM_WORDS;                  // >= either single scan's scratch
     extern __shared__ uint4 smem[];
     uint4 *sx = smem;
@@ -723,7 +723,7 @@ using CfgAddF32 = ScanCfg<OpAdd<float>, 512, 32, 512, 32>;
 using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
 using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
-using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 1024, 8>;
+using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 512, 8>;
 using CfgMinF32 = ScanCfg<OpMinMax<float, false>, 512, 32, 512, 16, true>;
 using CfgMaxF32 = ScanCfg<OpMinMax<float, true>, 512, 32, 512, 16, true>;
 using CfgMat2 = ScanCfg<OpMatMul<2, float, double, float>, 512, 8, 256, 8, true>;
