@@ -445,7 +445,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
             racc.l = Op::lin_combine(c, racc.l);
         }
         RS rtotal;
-        const RS rex = RBS::template exclusive<true>(racc, rtotal, scratch);
+        const RS rex = RBS::template exclusive<true, false>(racc, rtotal, scratch + FBS::SMEM_WORDS);  // own scratch: no entry barrier
         if (threadIdx.x < 32) {
             RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
             __syncwarp();
@@ -482,7 +482,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
         DBS::template exclusive<false>(racc, rtotal, rex, facc, ftotal, fex, scratch);  // the CTA's first use of scratch
     } else {
         rex = RBS::template exclusive<true, false>(racc, rtotal, scratch);
-        fex = FBS::template exclusive<false>(facc, ftotal, scratch);
+        fex = FBS::template exclusive<false, false>(facc, ftotal, scratch + RBS::SMEM_WORDS);  // own scratch: no entry barrier
     }
 
     // The forward prefixes r_{i-1} of the thread's elements depend only on fpre[t] and fex, not on the reverse
