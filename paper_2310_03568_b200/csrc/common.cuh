@@ -397,13 +397,27 @@ template <int NT, int RW>
 struct TileStage {
     static_assert(RW % 4 == 0, "row must be a whole number of 16-byte chunks");
     static constexpr int CPR = RW / 4;                       // chunks per row
-    static constexpr int PITCH_C = (CPR % 2 == 0) ? CPR + 1 : CPR;  // pitch in chunks
+    // Rows of 4 chunks (64 bytes): a dense layout with the chunk index XOR-ed with bits 1-2 of the row (what the TMA
+    // unit's 64B swizzle does) instead of a padded pitch.  The padded pitch of 5 chunks keeps "chunk c of my row"
+    // conflict-free but puts chunks t and t + 7 of a coalesced tile copy on one bank group: 14.3 M of the linrec reverse
+    // kernel's 54 M shared-memory wavefronts were bank conflicts (ncu, profiles/r2i_scan_vjp.txt); the XOR layout is
+    // conflict-free on both sides.  Rows of 8 chunks are conflict-free with a pitch of 9 and keep it (row_ptr users).
+    static constexpr bool SWZ = CPR == 4;
+    static constexpr int PITCH_C = SWZ ? CPR : ((CPR % 2 == 0) ? CPR + 1 : CPR);  // pitch in chunks
     static constexpr int TILE_WORDS = NT * RW;
     static constexpr int TILE_CHUNKS = NT * CPR;
     static constexpr int SMEM_BYTES = NT * PITCH_C * 16;
 
     // global (tile-relative chunk index) -> shared chunk index
-    static VJP_DEVINL int smem_chunk(int c) { return (c / CPR) * PITCH_C + (c % CPR); }
+    static VJP_DEVINL int smem_chunk(int c) {
+        if constexpr (SWZ) return c ^ ((c >> 3) & 3);
+        else return (c / CPR) * PITCH_C + (c % CPR);
+    }
+    // chunk j of `row` -> shared chunk index
+    static VJP_DEVINL int row_chunk(int row, int j) {
+        if constexpr (SWZ) return row * CPR + (j ^ ((row >> 1) & 3));
+        else return row * PITCH_C + j;
+    }
 
     // Load `valid_words` words (<= TILE_WORDS) starting at `g` (16-byte aligned) into the staged
     // layout; the rest of the tile is filled with the word pattern fill[w % FW].
@@ -455,20 +469,21 @@ struct TileStage {
 
     // A row is contiguous in shared memory (the padding sits between rows).
     static VJP_DEVINL uint32_t *row_ptr(uint4 *smem, int row) {
+        static_assert(!SWZ, "a swizzled row is not contiguous");
         return reinterpret_cast<uint32_t *>(smem + row * PITCH_C);
     }
     // Row access for the owning thread: whole row <-> registers.
     static VJP_DEVINL void read_row(const uint4 *smem, int row, uint32_t (&r)[RW]) {
 #pragma unroll
         for (int c = 0; c < CPR; c++) {
-            const uint4 v = smem[row * PITCH_C + c];
+            const uint4 v = smem[row_chunk(row, c)];
             r[4 * c + 0] = v.x; r[4 * c + 1] = v.y; r[4 * c + 2] = v.z; r[4 * c + 3] = v.w;
         }
     }
     static VJP_DEVINL void write_row(uint4 *smem, int row, const uint32_t (&r)[RW]) {
 #pragma unroll
         for (int c = 0; c < CPR; c++)
-            smem[row * PITCH_C + c] = make_uint4(r[4 * c + 0], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
+            smem[row_chunk(row, c)] = make_uint4(r[4 * c + 0], r[4 * c + 1], r[4 * c + 2], r[4 * c + 3]);
     }
 };
 

@@ -722,7 +722,7 @@ static int run_vjp(int64_t n, const void *xs, const void *ys_bar, void *xs_bar, 
 using CfgAddF32 = ScanCfg<OpAdd<float>, 512, 32, 512, 32>;
 using CfgAddF64 = ScanCfg<OpAdd<double>, 512, 16, 512, 16>;
 using CfgMulF32 = ScanCfg<OpMul<float>, 512, 32, 512, 16>;
-using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 1024, 8>;
+using CfgMulF64 = ScanCfg<OpMul<double>, 512, 16, 512, 8>;
 using CfgLinRec = ScanCfg<OpLinRec<float>, 512, 16, 512, 8>;
 using CfgMinF32 = ScanCfg<OpMinMax<float, false>, 512, 32, 512, 16, true>;
 using CfgMaxF32 = ScanCfg<OpMinMax<float, true>, 512, 32, 512, 16, true>;
