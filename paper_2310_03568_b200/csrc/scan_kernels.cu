@@ -371,7 +371,7 @@ tile_agg_tma_kernel(const __grid_constant__ CUtensorMap tm, const uint32_t *__re
 //     rbar_i = ybar_i + u_{i+1},   xbar_i = (d(r_{i-1} (.) x_i)/dx_i)^T rbar_i,   u_n = 0,
 // and element i acts on the incoming u as the affine map z -> (ybar_i + z) * X_i^T.
 template <class Op, int NT, int IPT>
-__global__ void __launch_bounds__(NT, (Op::EW <= 4 ? (NT <= 256 ? 3 : 1024 / NT) : 1))  // 256 threads: 3 CTAs fit the shared memory
+__global__ void __launch_bounds__(NT, (Op::EW <= 4 ? (NT <= 256 ? 3 : 1024 / NT) : (Op::EW == 9 ? 2 : 1)))  // 256 threads: 3 CTAs fit the shared memory
 scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restrict__ ybar,
                         uint32_t *__restrict__ xbar, int64_t n, int num_tiles,
                         const typename Op::Fwd *__restrict__ fpre,
@@ -386,7 +386,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     using RBS = BlockScan<RM, NT>;
     using FBS = BlockScan<FM, NT>;
     using DBS = BlockScanDual<RM, FM, NT>;
-    constexpr bool DUAL = sizeof(RS) + sizeof(FS) <= 192;  // narrow states: both block scans in one pass (half the barriers)
+    constexpr bool DUAL = sizeof(RS) + sizeof(FS) <= 96;  // narrow states: both block scans in one pass (half the barriers)
     constexpr int SCR = DBS::SMEM_WORDS;                  // >= either single scan's scratch
     extern __shared__ uint4 smem[];
     uint4 *sx = smem;
