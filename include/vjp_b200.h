@@ -13,6 +13,10 @@
  *     (a cudaStream_t passed as void*; NULL = the legacy default stream) and returns.
  *     The *_host entry points are the exception: their data pointers are HOST pointers, they
  *     copy host->device, run the same kernels, copy the result back and synchronise `stream`.
+ *     Because a device-pointer call only enqueues, it may be issued on a stream that is being
+ *     CAPTURED into a CUDA graph (after one call of the same kind outside the capture: kernel
+ *     attributes are set on first use); replaying the graph repeats the call on the same buffers
+ *     (tests/test_gpu_boundary.py, bench.py).  The scan VJP passes a TMA tensor map by value.
  *   - Scan elements are [n][d] contiguous row-major, d = vjp_scan_arity(op): 1 ('+', '*'),
  *     2 (linear recurrence (a,b)), 4 (2x2 row-major matrix), 9 (3x3), 25 (5x5 row-major matrix).
  *   - Bin indices `is` are int64.  An index outside [0, num_bins) -- negative
