@@ -644,10 +644,9 @@ static int run_tile_agg_tma(int64_t n, const void *xs, typename Op::Fwd *fpre, c
             return VJP_ERR_UNSUPPORTED;
     }
     auto kern = tile_agg_tma_kernel<Op, NT, IPT>;
-    static const int per_gpu = [&] {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        return resident_ctas(kern, NT, C::SMEM);
-    }();
+    // per call: the attribute belongs to the current device (a process may drive several GPUs)
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM) != cudaSuccess) return VJP_ERR_CUDA;
+    static const int per_gpu = resident_ctas(kern, NT, C::SMEM);
     const unsigned grid = (unsigned)(nt < per_gpu ? nt : per_gpu);
     VJP_LAUNCH(K_SCAN_TILEAGG_TMA, stream)
     kern<<<grid, NT, C::SMEM, stream>>>(tm, static_cast<const uint32_t *>(xs), n, (int)nt, fpre);
