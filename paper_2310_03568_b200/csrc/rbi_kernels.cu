@@ -241,15 +241,20 @@ rbi_vjp_add_kernel(int64_t n, int64_t w, const int64_t *__restrict__ is,
                    const T *__restrict__ hist_bar, T *__restrict__ vs_bar, int accumulate) {
     extern __shared__ uint4 smem_raw[];
     T *sh = reinterpret_cast<T *>(smem_raw);
+    const int64_t stride = (int64_t)gridDim.x * RBI_NT;
+    int64_t q = blockIdx.x * (int64_t)RBI_NT + threadIdx.x;
+    // the keys of the thread's first quad are in flight while the table is staged (config 1 is one quad per thread: its
+    // two dependent round trips become one; prefetching every next quad too cost the n = 2^26 case 4 %)
+    int64_t k[4] = {-1, -1, -1, -1};
+    int cnt = 0;
+    if (q * 4 < n) cnt = load_keys4(is, q * 4, n, k);
     if (SMEM) {
-        for (int k = threadIdx.x; k < (int)w; k += RBI_NT) sh[k] = hist_bar[k];
+        for (int i = threadIdx.x; i < (int)w; i += RBI_NT) sh[i] = hist_bar[i];
         __syncthreads();
     }
-    const int64_t stride = (int64_t)gridDim.x * RBI_NT;
-    for (int64_t q = blockIdx.x * (int64_t)RBI_NT + threadIdx.x; q * 4 < n; q += stride) {
-        int64_t k[4];
+    for (bool first = true; q * 4 < n; q += stride, first = false) {
+        if (!first) cnt = load_keys4(is, q * 4, n, k);
         T o[4];
-        const int cnt = load_keys4(is, q * 4, n, k);
 #pragma unroll
         for (int j = 0; j < 4; j++)
             o[j] = in_range(k[j], w) ? (SMEM ? sh[k[j]] : __ldg(hist_bar + k[j])) : T(0);
