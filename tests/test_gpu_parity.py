@@ -21,7 +21,7 @@ import os
 
 # VJP_TEST_MAX_N caps the problem sizes (the compute-sanitizer runs under profiles/ use 16385)
 MAX_N = int(os.environ.get("VJP_TEST_MAX_N", "0")) or None
-SIZES = [1, 2, 33, 127, 128, 129, 383, 384, 385, 511, 513, 639, 640, 641, 767, 768, 769, 1023, 1025, 2047, 2049, 4095, 4096, 4097,
+SIZES = [1, 2, 33, 127, 128, 129, 383, 384, 385, 511, 513, 639, 640, 641, 767, 768, 769, 1023, 1025, 1535, 1536, 1537, 2047, 2048, 2049, 4095, 4096, 4097,
          8191, 8192, 8193, 12345, 16383, 16384, 16385, 32769, 100003, 300007]
 if MAX_N:
     SIZES = [n for n in SIZES if n <= MAX_N]
@@ -93,6 +93,21 @@ def test_scan_vjp_matches_oracle(name, n):
     got = B.vjp_scan(op, dev(xs), dev(ys_bar)).cpu().numpy()
     ref = oracle.vjp_scan(oname, xs, ys_bar, q=q)
     if name in ("min_f32", "max_f32"):   # a selection: every adjoint is a sum of ys_bar entries, order-dependent only in rounding
+        assert np.array_equal(got != 0, ref != 0)
+    assert nrel(got, ref) <= TOL[op.torch_dtype]
+
+
+@pytest.mark.parametrize("name", ["mul_f64", "linrec", "min_f32", "matmul2"])
+def test_scan_vjp_persistent_aggregate_ring(name):
+    """n = 5 000 011: the TMA-fed aggregate pass of the scan VJP is a persistent kernel -- here its CTAs take 4-9 tiles each,
+    so every ring slot is refilled and waited for with both mbarrier parities, and the last tile is ragged (filled by hand)."""
+    n = 5_000_011
+    if MAX_N and n > MAX_N:
+        pytest.skip("size cap")
+    op, oname, q, xs, ys_bar = scan_inputs(name, n)
+    got = B.vjp_scan(op, dev(xs), dev(ys_bar)).cpu().numpy()
+    ref = oracle.vjp_scan(oname, xs, ys_bar, q=q)
+    if name == "min_f32":
         assert np.array_equal(got != 0, ref != 0)
     assert nrel(got, ref) <= TOL[op.torch_dtype]
 
