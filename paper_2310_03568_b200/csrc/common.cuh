@@ -211,8 +211,12 @@ struct BlockScanDual {
         if (lane == NW - 1) store_state_smem(tot + NW * SW, wi);
     }
 
-    template <bool ENTRY_SYNC = true>
-    static VJP_DEVINL void exclusive(const SA &la, SA &ta, SA &exa, const SB &lb, SB &tb, SB &exb, uint32_t *scratch) {
+    struct NoHook { VJP_DEVINL void operator()(const uint32_t *) const {} };
+    // after_total_a(words): called by all lanes of warp 0 as soon as scan A's block total sits in shared memory (one
+    // barrier before every thread has it): the reverse scan kernel publishes its tile aggregate from there
+    template <bool ENTRY_SYNC = true, class Hook = NoHook>
+    static VJP_DEVINL void exclusive(const SA &la, SA &ta, SA &exa, const SB &lb, SB &tb, SB &exb, uint32_t *scratch,
+                                     Hook after_total_a = Hook()) {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         const int pwa = NW - 1 - warp;  // processing rank of this warp in scan A
         uint32_t *sa = scratch, *sb = scratch + (NW + 1) * WA;
@@ -233,7 +237,11 @@ struct BlockScanDual {
         if (lane == 0) store_state_smem(sa + pwa * WA, ia);
         if (lane == 31) store_state_smem(sb + warp * WB, ib);
         __syncthreads();
-        if (warp == 0) cross_warp<MA, SA>(sa, lane);
+        if (warp == 0) {
+            cross_warp<MA, SA>(sa, lane);
+            __syncwarp();
+            after_total_a(sa + NW * WA);
+        }
         if (warp == 1) cross_warp<MB, SB>(sb, lane);
         __syncthreads();
         ta = load_state_smem<SA>(sa + NW * WA);

@@ -61,14 +61,17 @@ static LookbackWs<S> lookback_carve(char *base, int64_t num_tiles, size_t *zero_
 // Warp 0 of the block: publish the tile aggregate, look back, publish the inclusive prefix.
 // Returns (in every lane of warp 0) the fold of all tiles processed before tile p.
 // `words`: sizeof(State) bytes of shared memory.
-template <class M>
+// PUBLISHED: the tile aggregate (or, for p = 0, the prefix) has been published already.
+template <class M, bool PUBLISHED = false>
 VJP_DEVINL typename M::State tile_prefix_warp0(const TileSlots<typename M::State> &ts, int p,
                                                const typename M::State &total, uint32_t *words) {
     using S = typename M::State;
     const int lane = threadIdx.x & 31;
-    if (lane == 0) store_state_smem(words, total);
-    __syncwarp();
-    ts.publish(p, words, p == 0 ? TILE_PREFIX : TILE_AGG);
+    if (!PUBLISHED) {
+        if (lane == 0) store_state_smem(words, total);
+        __syncwarp();
+        ts.publish(p, words, p == 0 ? TILE_PREFIX : TILE_AGG);
+    }
     if (p == 0) return M::identity();
     const S pre = lookback_warp<M>(ts, p);
     __syncwarp();
@@ -479,7 +482,10 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     RS rtotal, rex;
     FS ftotal, fex;
     if constexpr (DUAL) {
-        DBS::template exclusive<false>(racc, rtotal, rex, facc, ftotal, fex, scratch);  // the CTA's first use of scratch
+        // the CTA's first use of scratch; warp 0 publishes the tile aggregate one barrier early, straight from the scan
+        DBS::template exclusive<false>(racc, rtotal, rex, facc, ftotal, fex, scratch, [&](const uint32_t *tot) {
+            ws.ts.publish(p, tot, p == 0 ? TILE_PREFIX : TILE_AGG);
+        });
     } else {
         rex = RBS::template exclusive<true, false>(racc, rtotal, scratch);
         fex = FBS::template exclusive<false, false>(facc, ftotal, scratch + RBS::SMEM_WORDS);  // own scratch: no entry barrier
@@ -496,7 +502,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     }
 
     if (threadIdx.x < 32) {
-        RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
+        RS pre = tile_prefix_warp0<RM, DUAL>(ws.ts, p, rtotal, bcast);
         __syncwarp();
         if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
     }
