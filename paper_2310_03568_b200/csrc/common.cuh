@@ -125,6 +125,8 @@ VJP_DEVINL S load_state_smem(const uint32_t *src) {
 // "earlier / later" refer to PROCESSING order.  With REVT = false thread t has processing rank
 // t; with REVT = true thread t has rank NT-1-t (a scan that runs from the end of the tile).
 
+struct NoHook { VJP_DEVINL void operator()(const uint32_t *) const {} };
+
 template <class M, int NT>
 struct BlockScan {
     using S = typename M::State;
@@ -136,8 +138,10 @@ struct BlockScan {
     // Exclusive scan of one state per thread.  Returns the exclusive prefix of this thread
     // (within the block) and the block total in `total` (valid in every thread).
     // ENTRY_SYNC = false: the caller knows that nobody can still be reading `scratch` (the first scan of a CTA)
-    template <bool REVT, bool ENTRY_SYNC = true>
-    static VJP_DEVINL S exclusive(const S &local, S &total, uint32_t *scratch) {
+    // after_total(words): called by all lanes of warp 0 as soon as the block total sits in shared memory, one barrier
+    // before every thread has it (the look-back kernels publish their tile aggregate from there)
+    template <bool REVT, bool ENTRY_SYNC = true, class Hook = NoHook>
+    static VJP_DEVINL S exclusive(const S &local, S &total, uint32_t *scratch, Hook after_total = Hook()) {
         const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
         const int plane = REVT ? 31 - lane : lane;
         const int pwarp = REVT ? NW - 1 - warp : warp;
@@ -170,6 +174,8 @@ struct BlockScan {
             __syncwarp();
             if (lane < NW) store_state_smem(scratch + lane * SW, wex);
             if (lane == NW - 1) store_state_smem(scratch + NW * SW, wi);
+            __syncwarp();
+            after_total(scratch + NW * SW);
         }
         __syncthreads();
         total = load_state_smem<S>(scratch + NW * SW);
@@ -211,7 +217,6 @@ struct BlockScanDual {
         if (lane == NW - 1) store_state_smem(tot + NW * SW, wi);
     }
 
-    struct NoHook { VJP_DEVINL void operator()(const uint32_t *) const {} };
     // after_total_a(words): called by all lanes of warp 0 as soon as scan A's block total sits in shared memory (one
     // barrier before every thread has it): the reverse scan kernel publishes its tile aggregate from there
     template <bool ENTRY_SYNC = true, class Hook = NoHook>

@@ -133,14 +133,17 @@ scan_lookback_kernel(const uint32_t *__restrict__ in, uint32_t *__restrict__ out
         for (int j = IPT - 2; j >= 0; j--) acc = Op::combine(Op::from_elem(r + j * EW), acc);
     }
     S total;
-    S ex = BS::template exclusive<REV, false>(acc, total, scratch);  // the CTA's only scan
+    // the CTA's only scan; in MODE_SCAN warp 0 publishes the tile aggregate straight from its cross-warp phase
+    S ex = BS::template exclusive<REV, false>(acc, total, scratch, [&](const uint32_t *tot) {
+        if (MODE == MODE_SCAN) ws.ts.publish(p, tot, p == 0 ? TILE_PREFIX : TILE_AGG);
+    });
     if (MODE == MODE_TILEAGG) {  // aggregate only: no dependency on other tiles, pure streaming
         if (threadIdx.x == 0) store_state_cg(fpre + t, total);
         return;
     }
 
     if (threadIdx.x < 32) {
-        S pre = tile_prefix_warp0<M>(ws.ts, p, total, bcast);
+        S pre = tile_prefix_warp0<M, true>(ws.ts, p, total, bcast);
         __syncwarp();
         if (threadIdx.x == 0) store_state_smem(bcast, pre);
     }
@@ -448,9 +451,10 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
             racc.l = Op::lin_combine(c, racc.l);
         }
         RS rtotal;
-        const RS rex = RBS::template exclusive<true, false>(racc, rtotal, scratch + FBS::SMEM_WORDS);  // own scratch: no entry barrier
+        const RS rex = RBS::template exclusive<true, false>(racc, rtotal, scratch + FBS::SMEM_WORDS,  // own scratch: no entry barrier
+                                                            [&](const uint32_t *tot) { ws.ts.publish(p, tot, p == 0 ? TILE_PREFIX : TILE_AGG); });
         if (threadIdx.x < 32) {
-            RS pre = tile_prefix_warp0<RM>(ws.ts, p, rtotal, bcast);
+            RS pre = tile_prefix_warp0<RM, true>(ws.ts, p, rtotal, bcast);
             __syncwarp();
             if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
         }
@@ -487,7 +491,8 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
             ws.ts.publish(p, tot, p == 0 ? TILE_PREFIX : TILE_AGG);
         });
     } else {
-        rex = RBS::template exclusive<true, false>(racc, rtotal, scratch);
+        rex = RBS::template exclusive<true, false>(racc, rtotal, scratch,
+                                                   [&](const uint32_t *tot) { ws.ts.publish(p, tot, p == 0 ? TILE_PREFIX : TILE_AGG); });
         fex = FBS::template exclusive<false, false>(facc, ftotal, scratch + RBS::SMEM_WORDS);  // own scratch: no entry barrier
     }
 
@@ -502,7 +507,7 @@ scan_vjp_reverse_kernel(const uint32_t *__restrict__ xs, const uint32_t *__restr
     }
 
     if (threadIdx.x < 32) {
-        RS pre = tile_prefix_warp0<RM, DUAL>(ws.ts, p, rtotal, bcast);
+        RS pre = tile_prefix_warp0<RM, true>(ws.ts, p, rtotal, bcast);  // the aggregate went out from the scan
         __syncwarp();
         if (threadIdx.x == 0) store_state_smem(bcast, pre.b);
     }
